@@ -1,0 +1,232 @@
+"""oracle -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+
+ctypes access to oracle.cpp, the plain CPU statement of the SPOTLIGHT search hot path
+(arxiv/paper_2606_27262).  Only tests/, __graft_entry__.smoke() and
+bench.py's cpu_baseline / --impl reference legs may import this package.  It imports nothing from
+paper_2606_27262_b200 and the product imports nothing from here.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+from typing import List, Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "oracle.cpp")
+_SO = os.path.join(_HERE, "liboracle.so")
+
+CXXFLAGS = ["-O2", "-fopenmp", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC"]
+
+
+def build(force: bool = False) -> str:
+    """g++ oracle.cpp -> liboracle.so (rebuilt when the source is newer)."""
+    if force or (not os.path.exists(_SO)) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        subprocess.run(["g++", *CXXFLAGS, "-o", _SO, _SRC], check=True)
+    return _SO
+
+
+_lib = None
+_i32p = ctypes.POINTER(ctypes.c_int32)
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_SO)
+        vp, i32, i64, f64 = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+        L.orc_num_threads.restype = ctypes.c_int
+        L.orc_delay_table.argtypes = [f64, f64, i32, f64, f64, f64, i32, i32, vp]
+        L.orc_nout.argtypes = [vp, i32, i32, i64, i32, vp]
+        L.orc_decimate.argtypes = [vp, i32, i64, i32, vp]
+        L.orc_dedisperse_u16.argtypes = [vp, i32, i64, vp, i32, vp, vp, vp]
+        L.orc_dedisperse_u8.argtypes = [vp, i32, i64, vp, i32, vp, vp, vp]
+        L.orc_dedisperse_point_u8.argtypes = [vp, i32, i64, vp, i32, i64, vp]
+        L.orc_stats.argtypes = [vp, i64, vp, vp]
+        L.orc_mean_sigma.argtypes = [i64, i64, ctypes.c_uint64, vp, vp]
+        L.orc_boxcar_snr.argtypes = [vp, i64, i32, vp]
+        L.orc_best_width.argtypes = [vp, i64, vp, i32, vp, vp]
+        L.orc_snr_at.argtypes = [vp, i64, i32, i64, vp]
+        L.orc_search_plane.argtypes = [vp, i32, vp, vp, vp, i32, f64, vp, vp, vp, vp, vp, vp, vp]
+        for name in ("orc_delay_table", "orc_nout", "orc_decimate", "orc_dedisperse_u16", "orc_dedisperse_u8",
+                     "orc_dedisperse_point_u8", "orc_stats", "orc_mean_sigma", "orc_boxcar_snr", "orc_best_width",
+                     "orc_snr_at", "orc_search_plane"):
+            getattr(L, name).restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def _ptr(a: Optional[np.ndarray]):
+    return None if a is None else a.ctypes.data
+
+
+def _check(rc: int, what: str):
+    if rc != 0:
+        raise RuntimeError(f"oracle: {what} failed (rc={rc})")
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+# ---- A. plan -----------------------------------------------------------------------------------
+def delay_table(fch1: float, foff: float, nchan: int, tsamp: float, dm_lo: float, dm_step: float, ndm: int,
+                decim: int) -> np.ndarray:
+    out = np.empty((ndm, nchan), dtype=np.int32)
+    _check(lib().orc_delay_table(fch1, foff, nchan, tsamp, dm_lo, dm_step, ndm, decim, _ptr(out)), "delay_table")
+    return out
+
+
+def nout(delay: np.ndarray, nsamp: int, decim: int) -> np.ndarray:
+    delay = np.ascontiguousarray(delay, dtype=np.int32)
+    out = np.empty(delay.shape[0], dtype=np.int32)
+    _check(lib().orc_nout(_ptr(delay), delay.shape[0], delay.shape[1], nsamp, decim, _ptr(out)), "nout")
+    return out
+
+
+# ---- B. decimation and dedispersion -----------------------------------------------------------------
+def decimate(x: np.ndarray, k: int) -> np.ndarray:
+    x = np.ascontiguousarray(x, dtype=np.uint8)
+    nchan, nsamp = x.shape
+    y = np.empty((nchan, nsamp // k), dtype=np.uint16)
+    _check(lib().orc_decimate(_ptr(x), nchan, nsamp, k, _ptr(y)), "decimate")
+    return y
+
+
+def dedisperse(y: np.ndarray, delay: np.ndarray, nout_: np.ndarray) -> Tuple[np.ndarray, np.ndarray]:
+    """DM transform of one range.  y is uint8 (k = 1) or uint16 (decimated).  Returns (packed rows, row offsets)."""
+    delay = np.ascontiguousarray(delay, dtype=np.int32)
+    nout_ = np.ascontiguousarray(nout_, dtype=np.int32)
+    y = np.ascontiguousarray(y)
+    nchan, nk = y.shape
+    ndm = delay.shape[0]
+    rowoff = np.zeros(ndm + 1, dtype=np.int64)
+    np.cumsum(nout_.astype(np.int64), out=rowoff[1:])
+    out = np.empty(int(rowoff[-1]), dtype=np.int32)
+    if y.dtype == np.uint8:
+        rc = lib().orc_dedisperse_u8(_ptr(y), nchan, nk, _ptr(delay), ndm, _ptr(nout_), _ptr(rowoff), _ptr(out))
+    elif y.dtype == np.uint16:
+        rc = lib().orc_dedisperse_u16(_ptr(y), nchan, nk, _ptr(delay), ndm, _ptr(nout_), _ptr(rowoff), _ptr(out))
+    else:
+        raise TypeError("dedisperse wants uint8 or uint16 input")
+    _check(rc, "dedisperse")
+    return out, rowoff
+
+
+def dedisperse_point(x: np.ndarray, delay_row: np.ndarray, k: int, t: int) -> int:
+    """One output sample of one trial straight from the raw uint8 filterbank (decimation folded in)."""
+    x = np.ascontiguousarray(x, dtype=np.uint8)
+    delay_row = np.ascontiguousarray(delay_row, dtype=np.int32)
+    out = ctypes.c_int32(0)
+    _check(lib().orc_dedisperse_point_u8(_ptr(x), x.shape[0], x.shape[1], _ptr(delay_row), k, t,
+                                         ctypes.addressof(out)), "dedisperse_point")
+    return int(out.value)
+
+
+# ---- C. statistics, boxcar, best width ------------------------------------------------------------
+def stats(x: np.ndarray) -> Tuple[int, int]:
+    x = np.ascontiguousarray(x, dtype=np.int32)
+    s, q = ctypes.c_int64(0), ctypes.c_uint64(0)
+    _check(lib().orc_stats(_ptr(x), x.size, ctypes.addressof(s), ctypes.addressof(q)), "stats")
+    return int(s.value), int(q.value)
+
+
+def mean_sigma(n: int, s: int, q: int) -> Tuple[float, float]:
+    mu, sg = ctypes.c_double(0), ctypes.c_double(0)
+    _check(lib().orc_mean_sigma(n, s, q, ctypes.addressof(mu), ctypes.addressof(sg)), "mean_sigma")
+    return float(mu.value), float(sg.value)
+
+
+def boxcar_snr(x: np.ndarray, w: int) -> np.ndarray:
+    x = np.ascontiguousarray(x, dtype=np.int32)
+    out = np.zeros(max(0, x.size - w + 1), dtype=np.float64)
+    _check(lib().orc_boxcar_snr(_ptr(x), x.size, w, _ptr(out)), "boxcar_snr")
+    return out
+
+
+def best_width(x: np.ndarray, widths: Sequence[int]) -> Tuple[np.ndarray, np.ndarray]:
+    x = np.ascontiguousarray(x, dtype=np.int32)
+    wa = np.asarray(widths, dtype=np.int32)
+    nb = max(0, x.size - int(wa[0]) + 1)
+    b = np.zeros(nb, dtype=np.float64)
+    bw = np.zeros(nb, dtype=np.int32)
+    _check(lib().orc_best_width(_ptr(x), x.size, _ptr(wa), wa.size, _ptr(b), _ptr(bw)), "best_width")
+    return b, bw
+
+
+def snr_at(x: np.ndarray, w: int, t: int) -> float:
+    x = np.ascontiguousarray(x, dtype=np.int32)
+    out = ctypes.c_double(0)
+    _check(lib().orc_snr_at(_ptr(x), x.size, w, t, ctypes.addressof(out)), "snr_at")
+    return float(out.value)
+
+
+@dataclass
+class PlaneSearch:
+    sum: np.ndarray       # int64  [ntrial]
+    sumsq: np.ndarray     # uint64 [ntrial]
+    count: np.ndarray     # int64  [ntrial]
+    candoff: np.ndarray   # int64  [ntrial+1]
+    t: np.ndarray         # int32  [ncand]  (increasing within a trial)
+    w: np.ndarray         # int32  [ncand]
+    snr: np.ndarray       # float64 [ncand]
+
+
+def search_plane(dmt: np.ndarray, rowoff: np.ndarray, nout_: np.ndarray, widths: Sequence[int],
+                 threshold: float, want_candidates: bool = True) -> PlaneSearch:
+    dmt = np.ascontiguousarray(dmt, dtype=np.int32)
+    rowoff = np.ascontiguousarray(rowoff, dtype=np.int64)
+    nout_ = np.ascontiguousarray(nout_, dtype=np.int32)
+    wa = np.asarray(widths, dtype=np.int32)
+    nt = nout_.size
+    s = np.zeros(nt, dtype=np.int64)
+    q = np.zeros(nt, dtype=np.uint64)
+    cnt = np.zeros(nt, dtype=np.int64)
+    _check(lib().orc_search_plane(_ptr(dmt), nt, _ptr(rowoff), _ptr(nout_), _ptr(wa), wa.size, threshold,
+                                  _ptr(s), _ptr(q), _ptr(cnt), None, None, None, None), "search_plane(count)")
+    candoff = np.zeros(nt + 1, dtype=np.int64)
+    np.cumsum(cnt, out=candoff[1:])
+    n = int(candoff[-1])
+    ct = np.zeros(n, dtype=np.int32)
+    cw = np.zeros(n, dtype=np.int32)
+    cs = np.zeros(n, dtype=np.float64)
+    if want_candidates and n > 0:
+        _check(lib().orc_search_plane(_ptr(dmt), nt, _ptr(rowoff), _ptr(nout_), _ptr(wa), wa.size, threshold,
+                                      _ptr(s), _ptr(q), _ptr(cnt), _ptr(candoff), _ptr(ct), _ptr(cw), _ptr(cs)),
+               "search_plane(fill)")
+    return PlaneSearch(s, q, cnt, candoff, ct, cw, cs)
+
+
+# ---- whole path over a plan (one beam) ----------------------------------------------------------------
+@dataclass
+class RangeResult:
+    dm: np.ndarray        # float64 [ndm]
+    decim: int
+    delay: np.ndarray     # int32 [ndm][nchan]
+    nout: np.ndarray      # int32 [ndm]
+    series: Optional[np.ndarray]   # decimated input (uint16) or None for k == 1
+    dmt: np.ndarray       # int32 packed rows
+    rowoff: np.ndarray    # int64 [ndm+1]
+    search: Optional[PlaneSearch]
+
+
+def run_path(fb: np.ndarray, fch1: float, foff: float, tsamp: float,
+             ranges: Sequence[Tuple[float, float, int, int]], widths: Sequence[int], threshold: float,
+             do_search: bool = True) -> List[RangeResult]:
+    """delay table -> decimate -> dedisperse -> single-pulse search, range by range, for one beam."""
+    fb = np.ascontiguousarray(fb, dtype=np.uint8)
+    nchan, nsamp = fb.shape
+    out = []
+    for (dm_lo, dm_step, ndm, k) in ranges:
+        dly = delay_table(fch1, foff, nchan, tsamp, dm_lo, dm_step, ndm, k)
+        no = nout(dly, nsamp, k)
+        y = None if k == 1 else decimate(fb, k)
+        dmt, rowoff = dedisperse(fb if k == 1 else y, dly, no)
+        sr = search_plane(dmt, rowoff[:-1], no, widths, threshold) if do_search else None
+        dms = dm_lo + np.arange(ndm, dtype=np.float64) * dm_step
+        out.append(RangeResult(dms, k, dly, no, y, dmt, rowoff, sr))
+    return out
