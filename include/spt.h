@@ -1,0 +1,192 @@
+/*
+ * spt.h -- C ABI of libspt: the data-parallel hot path of the SPOTLIGHT real-time FRB search
+ * (arxiv/paper_2606_27262) for NVIDIA B200 (sm_100a).
+ *
+ *   host-side delay plan  ->  time decimation  ->  brute-force incoherent dedispersion (DM transform)
+ *   ->  boxcar single-pulse search  ->  candidate readback
+ *
+ * What each call computes is fixed by the paper (PAPER.md line numbers below) and, where the paper is
+ * silent, by the readings listed in DESIGN.md section 3 (same letters as SURVEY.md section 8(c)).
+ *
+ * Conventions
+ *   - plain pointers and sizes only; every pointer argument says HOST or DEVICE.
+ *   - every call returns SPT_OK (0) or a negative spt_status; nothing throws, aborts or prints.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - spt_dedisperse / spt_single_pulse_search only ENQUEUE work on that stream; spt_candidates_*,
+ *     spt_trial_stats and the *_host calls synchronise it.  One plan is used by one thread at a time.
+ *   - the caller owns the filterbank and DM-transform device buffers; the library owns everything
+ *     reachable from the plan (tables, decimated series, statistics, candidate list) until spt_plan_destroy.
+ *   - there is no CPU fallback: a call that needs the GPU fails with SPT_ERR_CUDA when none is usable.
+ */
+#ifndef SPT_H_
+#define SPT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    SPT_OK = 0,
+    SPT_ERR_INVALID = -1,     /* null pointer, non-positive size, widths not strictly increasing, nbeam > max_beams ... */
+    SPT_ERR_UNSUPPORTED = -2, /* foff >= 0 (band must be highest frequency first), decimation not a
+                                 power of two or > 64, sums that would not fit the integer types (see spt_plan_create) */
+    SPT_ERR_NOMEM = -3,       /* host or device allocation failed */
+    SPT_ERR_CUDA = -4,        /* CUDA runtime error or no usable device; text via spt_last_error() */
+    SPT_ERR_SHAPE = -5,       /* caller buffer too small / index out of range */
+    SPT_ERR_STATE = -6        /* call order: e.g. search before any dedisperse, stats before a search */
+} spt_status;
+
+typedef struct spt_plan spt_plan; /* opaque, library owned */
+
+/* One DM sub-range of the dedispersion plan ("the DM range is divided into sub-ranges, each
+ * with its own DM step"): trials DM_i = dm_lo + i*dm_step, i in [0, ndm), searched on the input decimated in
+ * time by `decim` (1 = full resolution; BASELINE.json north_star (3): "a time-decimation kernel for the
+ * high-DM ranges").  Global trial index = concatenation of the ranges in the order given. */
+typedef struct {
+    double dm_lo;   /* pc cm^-3 */
+    double dm_step; /* pc cm^-3, > 0 */
+    int32_t ndm;    /* >= 1 */
+    int32_t decim;  /* 1, 2, 4, ..., 64 */
+} spt_dm_range;
+
+/* One single-pulse candidate (boxcar matched filter, "all candidates above a threshold ... are
+ * taken to the next stage").  t and width are in samples OF THE TRIAL'S OWN (decimated) rate. */
+typedef struct {
+    int32_t beam;
+    int32_t trial; /* global trial index */
+    int32_t t;     /* start sample of the boxcar */
+    int32_t width; /* boxcar width that maximises S/N at t */
+    float snr;
+} spt_candidate;
+
+/* -------------------------------------------------------------------------------------------------------
+ * spt_plan_create -- a1 of SURVEY.md section 8(a): trial list, delay table, output geometry.  Host only: needs
+ * no GPU (device buffers are created on first use).
+ *
+ *   f_c   = fch1_mhz + c*foff_mhz, c in [0, nchan); channel 0 is the highest frequency and the reference
+ *           ("highest frequency in the observation band"); foff_mhz < 0 is required.
+ *   delay[d][c] = floor( 4.148808e3 * DM_d * (f_c^-2 - f_0^-2) / (tsamp_s * decim) + 0.5 )      int32
+ *           (Eq. 1-2; constant and "rounded to integer samples" per BASELINE.json north_star (2);
+ *           evaluated in IEEE double, no FMA contraction)
+ *   nout[d]     = max(0, floor(nsamp/decim) - delay[d][nchan-1])   valid output samples of trial d
+ *   offset[d]   = start of row d inside one beam's DM transform, in int32 elements; rows are padded to a multiple
+ *                 of 32 elements so that every row starts 128-byte aligned (padding is never written or read).
+ *
+ * widths: boxcar widths in samples of each trial's own rate, strictly increasing, >= 1 ("multiple
+ * trial widths").  max_beams bounds nbeam of later calls.  cand_capacity = records the device candidate list
+ * can hold (overflow is reported, not an error).
+ * Unsupported (SPT_ERR_UNSUPPORTED): foff >= 0; decim not a power of two <= 64; nchan*255*decim >= 2^31 (int32
+ * DM transform); widths[last]*nchan*255*decim >= 2^32 (boxcar sums are formed modulo 2^32).
+ * ----------------------------------------------------------------------------------------------------- */
+int spt_plan_create(double fch1_mhz, double foff_mhz, int32_t nchan, double tsamp_s, int64_t nsamp,
+                    const spt_dm_range* ranges /*HOST*/, int32_t nranges,
+                    const int32_t* widths /*HOST*/, int32_t nwidths,
+                    int32_t max_beams, int64_t cand_capacity, spt_plan** out /*HOST*/);
+int spt_plan_destroy(spt_plan* plan);
+
+/* Sizing: number of trials over all ranges; int32 elements of ONE beam's DM transform (sum of padded rows). */
+int spt_plan_info(const spt_plan* plan, int32_t* ntrials, int64_t* dmt_elems_per_beam);
+/* Per-trial metadata (any out pointer may be NULL). */
+int spt_plan_trial(const spt_plan* plan, int32_t trial, double* dm, int32_t* range, int32_t* decim,
+                   int32_t* nout, int64_t* offset);
+/* The delay-table row of one trial, host_out[nchan] (HOST) -- for the bit-exact delay-table parity. */
+int spt_plan_delays(const spt_plan* plan, int32_t trial, int32_t* host_out);
+
+/* Kernel-selection knobs, for A/B measurements and tests; must be set before the first spt_dedisperse.
+ *   "dedisp_kernel": 0 = tiled shared-memory kernel (default, the product), 1 = one-thread-per-output kernel
+ *                    reading global memory (bring-up / cross-check kernel, same results)
+ *   "group":         channels per pre-summed group G of the tiled kernel: 1, 2, 4 (default) or 8
+ *   "dm_tile":       trials per block tile (32 or 64; default 64)
+ *   "profile":       1 = bracket every kernel launch with CUDA events on the caller's stream (see
+ *                    spt_plan_kernel_times); may be switched at any time
+ * Unknown names / values -> SPT_ERR_INVALID. */
+int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value);
+
+/* Host-side view of the tables the tiled kernel runs on, for tests and reports; builds them
+ * if needed, needs no GPU.  Per range: DM tiles, stages, channel groups and pre-summed variants over all tiles, time
+ * tiles, and the largest shared-memory footprint (32-bit words) of a stage.  Any out pointer may be NULL. */
+int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int64_t* nstages, int64_t* ngroups,
+                         int64_t* nvariants, int64_t* ntiles_t, int64_t* max_stage_words);
+/* The delay row of one trial as the tiled kernel will apply it, reconstructed from those tables alone:
+ * host_out[nchan] (HOST).  Must equal spt_plan_delays for every trial (checked by the CPU tests). */
+int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out);
+
+/* -------------------------------------------------------------------------------------------------------
+ * spt_dedisperse -- a2 + a3: time decimation of the ranges with decim > 1, then the DM transform
+ *   y_k[b][c][j]  = sum_{m<k} x[b][c][k*j+m]                  uint16, j < floor(nsamp/k)   (decimation: a sum)
+ *   out[b][d][t]  = sum_c y_k[b][c][t + delay[d][c]]          int32,  t in [0, nout[d])
+ * ("shifting each channel ... by the appropriate time delay" and summing; the output is
+ * the DM transform, one row per trial.)
+ *   d_fb : DEVICE, uint8 [nbeam][nchan][nsamp], time contiguous, channel 0 = fch1 (highest frequency).
+ *   d_dmt: DEVICE, int32, at least nbeam*dmt_elems_per_beam elements, 128-byte aligned; beam b's row d starts at
+ *          b*dmt_elems_per_beam + offset[d].  Every element t < nout[d] of every row is written.
+ * Enqueues on cuda_stream and returns.
+ * ----------------------------------------------------------------------------------------------------- */
+int spt_dedisperse(spt_plan* plan, const uint8_t* d_fb, int32_t nbeam, int32_t* d_dmt, void* cuda_stream);
+
+/* DEVICE pointer to the decimated series made by the last spt_dedisperse for range `range` (decim > 1):
+ * uint16 [nbeam][nchan][nsamp_k].  Library owned; valid until the next spt_dedisperse / destroy.
+ * For a range with decim == 1 returns *d_ptr = NULL and nsamp_k = nsamp. */
+int spt_decimated(const spt_plan* plan, int32_t range, const uint16_t** d_ptr, int64_t* nsamp_k);
+/* Row stride (elements) of that series: rows are padded to a multiple of 16 elements; beam stride = nchan*row_stride. */
+int spt_decimated_stride(const spt_plan* plan, int32_t range, int64_t* row_stride);
+/* Copy of one beam of that series without the row padding: host_out (HOST) uint16 [nchan][nsamp_k].  Synchronises. */
+int spt_decimated_read(spt_plan* plan, int32_t range, int32_t beam, uint16_t* host_out);
+
+/* -------------------------------------------------------------------------------------------------------
+ * spt_single_pulse_search -- a4 (readings C1-C5, D1 of DESIGN.md): per (beam, trial) with N = nout > 0
+ *   Sx = sum x, Sxx = sum x^2 (exact integers);  mu = Sx/N;  sigma = sqrt((N*Sxx - Sx^2)/N^2)
+ *   S_w[t]   = sum_{j<w} x[t+j]                              t in [0, N-w]
+ *   snr_w[t] = (N*S_w[t] - w*Sx) / (N*sigma*sqrt(w))         (= (S_w - w*mu)/(sigma*sqrt(w)))
+ *   best[t]  = max over widths w <= N-t, scanned in increasing w with strict '>' ; t in [0, N-widths[0]]
+ *   a candidate {beam, trial, t, argmax width, best} is appended for every t with best[t] >= threshold.
+ * sigma == 0 or N < 2: no candidates.  The list and the statistics of the previous search are discarded.
+ * Order of the list is arbitrary.  Enqueues on cuda_stream and returns.
+ * ----------------------------------------------------------------------------------------------------- */
+int spt_single_pulse_search(spt_plan* plan, const int32_t* d_dmt /*DEVICE*/, int32_t nbeam, float threshold,
+                            void* cuda_stream);
+
+/* Exact statistics of one (beam, trial) from the last search (synchronises).  n = nout. */
+int spt_trial_stats(spt_plan* plan, int32_t beam, int32_t trial, int64_t* n, int64_t* sum, uint64_t* sumsq);
+/* All of them at once: host arrays [nbeam*ntrials] (beam major), any may be NULL. */
+int spt_trial_stats_all(spt_plan* plan, int32_t nbeam, int64_t* sum /*HOST*/, uint64_t* sumsq /*HOST*/);
+
+/* a5 Candidate readback (both synchronise the stream of the last search).
+ * total = exact number of candidates found (may exceed capacity); overflowed = 1 when records were dropped. */
+int spt_candidates_count(spt_plan* plan, int64_t* total, int32_t* overflowed);
+/* Copies min(total, capacity, cap) records to host_out (HOST); nwritten gets that number. */
+int spt_candidates_read(spt_plan* plan, spt_candidate* host_out, int64_t cap, int64_t* nwritten);
+
+/* -------------------------------------------------------------------------------------------------------
+ * spt_search_host -- the whole path from HOST memory: H2D copy of h_fb (uint8 [nbeam][nchan][nsamp]; pinned
+ * memory makes the copy asynchronous), spt_dedisperse + spt_single_pulse_search into a library-owned DM
+ * transform, then the candidate count back to the host.  Synchronous.  Candidates are then read with
+ * spt_candidates_read.  h_dmt (HOST, may be NULL): when given, receives the nbeam*dmt_elems_per_beam int32 DM transform.
+ * ----------------------------------------------------------------------------------------------------- */
+int spt_search_host(spt_plan* plan, const uint8_t* h_fb, int32_t nbeam, float threshold, int32_t* h_dmt,
+                    int64_t* ncand, int32_t* overflowed);
+
+/* With option "profile" = 1: device time (ms) of each kernel launched by the LAST spt_dedisperse and the LAST
+ * spt_single_pulse_search, in launch order; kinds: 1 = decimate, 2 = dedisperse, 3 = single-pulse search; `range` is the
+ * DM range the launch served (-1 for the search).  Synchronises.  Arrays (HOST) hold `cap` entries; n = entries written. */
+int spt_plan_kernel_times(spt_plan* plan, int32_t cap, int32_t* kind, int32_t* range, double* ms, int32_t* n);
+
+/* Number of kernel launches the library has enqueued through this plan since creation (bench bookkeeping). */
+int spt_plan_launches(const spt_plan* plan, int64_t* launches);
+
+/* Roofline probes: time `reps` launches of a register-only 32-bit integer-add loop
+ * (kind 0: IADD3 chain on the ALU pipe, kind 1: IMAD chain on the FMA pipe, kind 2: both interleaved) or of a
+ * conflict-free shared-memory load loop (kind 3: LDS.32, kind 4: LDS.128) on the current device and report warp
+ * instructions per second.  Synchronous; uses its own stream. */
+int spt_probe(int32_t kind, int32_t reps, double* warp_instr_per_s, double* elapsed_ms);
+
+const char* spt_strerror(int code);
+/* Text of the last CUDA error seen by this thread's calls ("" if none). */
+const char* spt_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPT_H_ */

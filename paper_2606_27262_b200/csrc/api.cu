@@ -1,0 +1,610 @@
+// api.cu -- the C ABI of libspt (include/spt.h): argument checking, device state, launch sequencing.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+
+#include "internal.h"
+#include "kernels.h"
+
+namespace spt {
+
+static thread_local std::string g_last_error;
+
+static int cuda_fail(cudaError_t e, const char* what) {
+    g_last_error = std::string(what) + ": " + cudaGetErrorString(e);
+    cudaGetLastError();  // clear the sticky-less error state
+    return e == cudaErrorMemoryAllocation ? SPT_ERR_NOMEM : SPT_ERR_CUDA;
+}
+#define SPT_CUDA(call)                                             \
+    do {                                                           \
+        cudaError_t e_ = (call);                                   \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);        \
+    } while (0)
+
+struct RangeDev {
+    int32_t* delay = nullptr;       // only for the naive kernel
+    TileDesc* tiles = nullptr;
+    StageDesc* stages = nullptr;
+    GroupDesc* groups = nullptr;
+    int16_t* var_shift = nullptr;
+    uint16_t* trial_off = nullptr;
+    uint16_t* series = nullptr;     // decimated input [max_beams][nchan][stride_k] (decim > 1)
+};
+
+struct DeviceState {
+    std::vector<RangeDev> r;
+    int32_t* nout = nullptr;        // [ntrials]
+    int64_t* offset = nullptr;      // [ntrials]
+    int64_t* sum = nullptr;         // [max_beams][ntrials]
+    unsigned long long* sumsq = nullptr;
+    spt_candidate* cand = nullptr;
+    unsigned long long* count = nullptr;
+    uint8_t* fb_pad = nullptr;      // aligned copy of an input whose rows are not 16-byte multiples
+    int64_t fb_pad_stride = 0;
+    uint8_t* h_fb = nullptr;        // spt_search_host: device copy of the host filterbank
+    int32_t* h_dmt = nullptr;       // spt_search_host: library-owned DM transform
+    cudaStream_t own_stream = nullptr;
+    cudaStream_t last_stream = nullptr;
+    int32_t nbeam_dedisp = 0, nbeam_search = 0;
+    bool searched = false;
+    // option "profile": events around every launch of the last dedisperse [0] / search [1]
+    struct Timed { int32_t kind, range; cudaEvent_t e0, e1; };
+    std::vector<Timed> timed[2];
+    std::vector<cudaEvent_t> event_pool;
+};
+
+static cudaEvent_t get_event(DeviceState* d) {
+    cudaEvent_t e = nullptr;
+    if (!d->event_pool.empty()) { e = d->event_pool.back(); d->event_pool.pop_back(); }
+    else cudaEventCreate(&e);
+    return e;
+}
+static void timed_clear(DeviceState* d, int slot) {
+    for (auto& t : d->timed[slot]) { d->event_pool.push_back(t.e0); d->event_pool.push_back(t.e1); }
+    d->timed[slot].clear();
+}
+struct ScopedTimer {  // records e0 at construction and e1 at destruction when profiling is on
+    DeviceState* d; cudaStream_t st; int slot; bool on;
+    ScopedTimer(Plan* p, cudaStream_t s, int slot_, int kind, int range) : d(p->dev), st(s), slot(slot_), on(p->opt_profile != 0) {
+        if (!on) return;
+        DeviceState::Timed t{kind, range, get_event(d), get_event(d)};
+        cudaEventRecord(t.e0, st);
+        d->timed[slot].push_back(t);
+    }
+    ~ScopedTimer() { if (on) cudaEventRecord(d->timed[slot].back().e1, st); }
+};
+
+template <typename T>
+static int upload(T** dst, const std::vector<T>& src) {
+    *dst = nullptr;
+    if (src.empty()) return SPT_OK;
+    SPT_CUDA(cudaMalloc((void**)dst, src.size() * sizeof(T)));
+    SPT_CUDA(cudaMemcpy(*dst, src.data(), src.size() * sizeof(T), cudaMemcpyHostToDevice));
+    return SPT_OK;
+}
+
+static void free_device(Plan* p) {
+    DeviceState* d = p->dev;
+    if (!d) return;
+    for (RangeDev& r : d->r) {
+        cudaFree(r.delay); cudaFree(r.tiles); cudaFree(r.stages); cudaFree(r.groups);
+        cudaFree(r.var_shift); cudaFree(r.trial_off); cudaFree(r.series);
+    }
+    cudaFree(d->nout); cudaFree(d->offset); cudaFree(d->sum); cudaFree(d->sumsq);
+    cudaFree(d->cand); cudaFree(d->count); cudaFree(d->fb_pad); cudaFree(d->h_fb); cudaFree(d->h_dmt);
+    if (d->own_stream) cudaStreamDestroy(d->own_stream);
+    timed_clear(d, 0); timed_clear(d, 1);
+    for (cudaEvent_t e : d->event_pool) cudaEventDestroy(e);
+    delete d;
+    p->dev = nullptr;
+}
+
+static int ensure_device(Plan* p) {
+    if (p->dev) return SPT_OK;
+    int ndev = 0;
+    cudaError_t e = cudaGetDeviceCount(&ndev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDeviceCount");
+    if (ndev < 1) { g_last_error = "no CUDA device"; return SPT_ERR_CUDA; }
+    if (p->opt_kernel == 0 && !p->tiling_built) {
+        const int rc = build_tiling(*p);
+        if (rc != SPT_OK) return rc;
+    }
+    DeviceState* d = new (std::nothrow) DeviceState();
+    if (!d) return SPT_ERR_NOMEM;
+    p->dev = d;
+    d->r.resize(p->ranges.size());
+    std::vector<int32_t> nout_all;
+    std::vector<int64_t> off_all;
+    int rc = SPT_OK;
+    for (size_t i = 0; i < p->ranges.size() && rc == SPT_OK; ++i) {
+        const RangePlan& rp = p->ranges[i];
+        RangeDev& rd = d->r[i];
+        nout_all.insert(nout_all.end(), rp.nout.begin(), rp.nout.end());
+        off_all.insert(off_all.end(), rp.offset.begin(), rp.offset.end());
+        if (p->opt_kernel == 1) rc = upload(&rd.delay, rp.delay);
+        else {
+            if ((rc = upload(&rd.tiles, rp.tiles)) != SPT_OK) break;
+            if ((rc = upload(&rd.stages, rp.stages)) != SPT_OK) break;
+            if ((rc = upload(&rd.groups, rp.groups)) != SPT_OK) break;
+            if ((rc = upload(&rd.var_shift, rp.var_shift)) != SPT_OK) break;
+            if ((rc = upload(&rd.trial_off, rp.trial_off)) != SPT_OK) break;
+        }
+        if (rc == SPT_OK && rp.decim > 1) {
+            const size_t bytes = (size_t)p->max_beams * p->nchan * rp.stride_k * sizeof(uint16_t);
+            cudaError_t ce = cudaMalloc((void**)&rd.series, bytes);
+            if (ce == cudaSuccess) ce = cudaMemset(rd.series, 0, bytes);
+            if (ce != cudaSuccess) rc = cuda_fail(ce, "series alloc");
+        }
+    }
+    if (rc == SPT_OK) rc = upload(&d->nout, nout_all);
+    if (rc == SPT_OK) rc = upload(&d->offset, off_all);
+    if (rc == SPT_OK) {
+        const size_t n = (size_t)p->max_beams * p->ntrials;
+        cudaError_t ce = cudaMalloc((void**)&d->sum, n * 8);
+        if (ce == cudaSuccess) ce = cudaMalloc((void**)&d->sumsq, n * 8);
+        if (ce == cudaSuccess) ce = cudaMalloc((void**)&d->count, 8);
+        if (ce == cudaSuccess) ce = cudaMemset(d->count, 0, 8);
+        if (ce == cudaSuccess && p->cand_capacity > 0)
+            ce = cudaMalloc((void**)&d->cand, (size_t)p->cand_capacity * sizeof(spt_candidate));
+        if (ce == cudaSuccess) ce = cudaStreamCreateWithFlags(&d->own_stream, cudaStreamNonBlocking);
+        if (ce != cudaSuccess) rc = cuda_fail(ce, "plan buffers");
+    }
+    if (rc != SPT_OK) free_device(p);
+    return rc;
+}
+
+static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d_dmt, cudaStream_t st) {
+    DeviceState* d = p->dev;
+    const uint8_t* in = d_fb;
+    int64_t in_stride = p->nsamp;
+    if ((p->nsamp & 15) != 0 || (reinterpret_cast<uintptr_t>(d_fb) & 15) != 0) {
+        // vector loads need 16-byte aligned rows: stage through a padded copy (zero pad)
+        const int64_t pitch = (p->nsamp + 15) / 16 * 16;
+        if (!d->fb_pad) {
+            const size_t bytes = (size_t)p->max_beams * p->nchan * pitch;
+            SPT_CUDA(cudaMalloc((void**)&d->fb_pad, bytes));
+            SPT_CUDA(cudaMemset(d->fb_pad, 0, bytes));
+            d->fb_pad_stride = pitch;
+        }
+        SPT_CUDA(cudaMemcpy2DAsync(d->fb_pad, (size_t)pitch, d_fb, (size_t)p->nsamp, (size_t)p->nsamp,
+                                   (size_t)nbeam * p->nchan, cudaMemcpyDeviceToDevice, st));
+        in = d->fb_pad;
+        in_stride = pitch;
+    }
+    timed_clear(d, 0);
+    // a2: decimated series of every range that needs one
+    for (size_t i = 0; i < p->ranges.size(); ++i) {
+        const RangePlan& rp = p->ranges[i];
+        if (rp.decim == 1 || rp.nsamp_k <= 0) continue;
+        ScopedTimer tm(p, st, 0, 1, (int)i);
+        launch_decimate(in, in_stride, (int64_t)p->nchan * in_stride, d->r[i].series, rp.stride_k,
+                        (int64_t)p->nchan * rp.stride_k, p->nchan, nbeam, rp.nsamp_k, rp.decim, st);
+        p->launches++;
+    }
+    // a3: DM transform, range by range
+    for (size_t i = 0; i < p->ranges.size(); ++i) {
+        const RangePlan& rp = p->ranges[i];
+        if (rp.max_nout <= 0) continue;
+        const RangeDev& rd = d->r[i];
+        const bool u16 = rp.decim > 1;
+        const void* src = u16 ? (const void*)rd.series : (const void*)in;
+        const int64_t rs = u16 ? rp.stride_k : in_stride;
+        const int32_t* nout = d->nout + rp.trial0;
+        const int64_t* off = d->offset + rp.trial0;
+        ScopedTimer tm(p, st, 0, 2, (int)i);
+        if (p->opt_kernel == 1) {
+            if (u16) launch_dedisp_naive<uint16_t>((const uint16_t*)src, rs, (int64_t)p->nchan * rs, rd.delay, nout, off,
+                                                   p->nchan, rp.ndm, nbeam, rp.max_nout, d_dmt, p->dmt_elems, st);
+            else launch_dedisp_naive<uint8_t>((const uint8_t*)src, rs, (int64_t)p->nchan * rs, rd.delay, nout, off,
+                                              p->nchan, rp.ndm, nbeam, rp.max_nout, d_dmt, p->dmt_elems, st);
+        } else {
+            const int rc = launch_dedisp_tiled(u16, p->opt_dm_tile, p->opt_group, src, rs, (int64_t)p->nchan * rs, d_dmt,
+                                               p->dmt_elems, rd.tiles, rd.stages, rd.groups, rd.var_shift, rd.trial_off,
+                                               nout, off, (int32_t)rp.tiles.size(), rp.ntile_t, nbeam, st);
+            if (rc != 0) { g_last_error = "dedisp_tiled: launch configuration rejected"; return SPT_ERR_CUDA; }
+        }
+        p->launches++;
+    }
+    SPT_CUDA(cudaGetLastError());
+    d->last_stream = st;
+    d->nbeam_dedisp = nbeam;
+    return SPT_OK;
+}
+
+static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float threshold, cudaStream_t st) {
+    DeviceState* d = p->dev;
+    SPT_CUDA(cudaMemsetAsync(d->count, 0, 8, st));
+    SpsArgs a{};
+    a.dmt = d_dmt;
+    a.beam_stride = p->dmt_elems;
+    a.nout = d->nout;
+    a.offset = d->offset;
+    a.ntrials = p->ntrials;
+    a.nw = (int32_t)p->widths.size();
+    for (int i = 0; i < a.nw; ++i) a.widths[i] = p->widths[i];
+    a.threshold = (double)threshold;
+    a.sum = d->sum;
+    a.sumsq = d->sumsq;
+    a.cand = d->cand;
+    a.count = d->count;
+    a.capacity = p->cand_capacity;
+    timed_clear(d, 1);
+    {
+        ScopedTimer tm(p, st, 1, 3, -1);
+        launch_sps(a, nbeam, st);
+    }
+    p->launches++;
+    SPT_CUDA(cudaGetLastError());
+    d->last_stream = st;
+    d->nbeam_search = nbeam;
+    d->searched = true;
+    return SPT_OK;
+}
+
+}  // namespace spt
+
+using namespace spt;
+
+struct spt_plan {
+    Plan p;
+};
+
+extern "C" {
+
+int spt_plan_create(double fch1_mhz, double foff_mhz, int32_t nchan, double tsamp_s, int64_t nsamp,
+                    const spt_dm_range* ranges, int32_t nranges, const int32_t* widths, int32_t nwidths,
+                    int32_t max_beams, int64_t cand_capacity, spt_plan** out) {
+    if (!out) return SPT_ERR_INVALID;
+    *out = nullptr;
+    if (!ranges || !widths || nranges < 1 || nwidths < 1 || nwidths > kMaxWidths || nchan < 1 || nsamp < 1 ||
+        !(tsamp_s > 0.0) || !(fch1_mhz > 0.0) || max_beams < 1 || cand_capacity < 0)
+        return SPT_ERR_INVALID;
+    if (!(foff_mhz < 0.0)) return SPT_ERR_UNSUPPORTED;                       // band must be flipped
+    if (!(fch1_mhz + (double)(nchan - 1) * foff_mhz > 0.0)) return SPT_ERR_INVALID;
+    for (int32_t i = 0; i < nwidths; ++i)
+        if (widths[i] < 1 || (i > 0 && widths[i] <= widths[i - 1])) return SPT_ERR_INVALID;
+    int maxdec = 1;
+    for (int32_t r = 0; r < nranges; ++r) {
+        const spt_dm_range& g = ranges[r];
+        if (g.ndm < 1 || !(g.dm_step > 0.0) || !(g.dm_lo >= 0.0) || g.decim < 1) return SPT_ERR_INVALID;
+        if ((g.decim & (g.decim - 1)) != 0 || g.decim > 64) return SPT_ERR_UNSUPPORTED;
+        if (g.decim > maxdec) maxdec = g.decim;
+    }
+    if ((double)nchan * 255.0 * maxdec >= 2147483648.0) return SPT_ERR_UNSUPPORTED;
+    if ((double)widths[nwidths - 1] * nchan * 255.0 * maxdec >= 4294967296.0) return SPT_ERR_UNSUPPORTED;
+    if (widths[nwidths - 1] > 4096 - 32) return SPT_ERR_UNSUPPORTED;
+    if (nsamp >= (1ll << 31)) return SPT_ERR_UNSUPPORTED;
+    spt_plan* h = new (std::nothrow) spt_plan();
+    if (!h) return SPT_ERR_NOMEM;
+    Plan& p = h->p;
+    p.fch1 = fch1_mhz; p.foff = foff_mhz; p.tsamp = tsamp_s; p.nchan = nchan; p.nsamp = nsamp;
+    p.max_beams = max_beams; p.cand_capacity = cand_capacity;
+    p.widths.assign(widths, widths + nwidths);
+    int rc;
+    try {
+        rc = build_plan(p, ranges, nranges);
+    } catch (const std::bad_alloc&) {
+        rc = SPT_ERR_NOMEM;
+    }
+    if (rc != SPT_OK) { delete h; return rc; }
+    *out = h;
+    return SPT_OK;
+}
+
+int spt_plan_destroy(spt_plan* plan) {
+    if (!plan) return SPT_ERR_INVALID;
+    free_device(&plan->p);
+    delete plan;
+    return SPT_OK;
+}
+
+int spt_plan_info(const spt_plan* plan, int32_t* ntrials, int64_t* dmt_elems_per_beam) {
+    if (!plan) return SPT_ERR_INVALID;
+    if (ntrials) *ntrials = plan->p.ntrials;
+    if (dmt_elems_per_beam) *dmt_elems_per_beam = plan->p.dmt_elems;
+    return SPT_OK;
+}
+
+int spt_plan_trial(const spt_plan* plan, int32_t trial, double* dm, int32_t* range, int32_t* decim, int32_t* nout,
+                   int64_t* offset) {
+    if (!plan) return SPT_ERR_INVALID;
+    int32_t loc = 0;
+    const RangePlan* rp = range_of_trial(plan->p, trial, &loc);
+    if (!rp) return SPT_ERR_SHAPE;
+    if (dm) *dm = rp->dm_lo + (double)loc * rp->dm_step;
+    if (range) *range = (int32_t)(rp - plan->p.ranges.data());
+    if (decim) *decim = rp->decim;
+    if (nout) *nout = rp->nout[loc];
+    if (offset) *offset = rp->offset[loc];
+    return SPT_OK;
+}
+
+int spt_plan_delays(const spt_plan* plan, int32_t trial, int32_t* host_out) {
+    if (!plan || !host_out) return SPT_ERR_INVALID;
+    int32_t loc = 0;
+    const RangePlan* rp = range_of_trial(plan->p, trial, &loc);
+    if (!rp) return SPT_ERR_SHAPE;
+    std::memcpy(host_out, &rp->delay[(size_t)loc * plan->p.nchan], sizeof(int32_t) * plan->p.nchan);
+    return SPT_OK;
+}
+
+int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value) {
+    if (!plan || !name) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (!std::strcmp(name, "profile")) {
+        if (value != 0 && value != 1) return SPT_ERR_INVALID;
+        p.opt_profile = (int32_t)value;
+        return SPT_OK;
+    }
+    if (p.dev) return SPT_ERR_STATE;
+    if (!std::strcmp(name, "dedisp_kernel")) {
+        if (value != 0 && value != 1) return SPT_ERR_INVALID;
+        p.opt_kernel = (int32_t)value;
+    } else if (!std::strcmp(name, "group")) {
+        if (value != 1 && value != 2 && value != 4 && value != 8) return SPT_ERR_INVALID;
+        p.opt_group = (int32_t)value; p.tiling_built = false;
+    } else if (!std::strcmp(name, "dm_tile")) {
+        if (value != 32 && value != 64) return SPT_ERR_INVALID;
+        p.opt_dm_tile = (int32_t)value; p.tiling_built = false;
+    } else {
+        return SPT_ERR_INVALID;
+    }
+    return SPT_OK;
+}
+
+static int ensure_tiling(Plan& p) {
+    if (p.tiling_built) return SPT_OK;
+    try {
+        return build_tiling(p);
+    } catch (const std::bad_alloc&) {
+        return SPT_ERR_NOMEM;
+    }
+}
+
+int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int64_t* nstages, int64_t* ngroups,
+                         int64_t* nvariants, int64_t* ntiles_t, int64_t* max_stage_words) {
+    if (!plan) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (range < 0 || range >= (int32_t)p.ranges.size()) return SPT_ERR_SHAPE;
+    const int rc = ensure_tiling(p);
+    if (rc != SPT_OK) return rc;
+    const RangePlan& rp = p.ranges[range];
+    if (ntiles_dm) *ntiles_dm = (int64_t)rp.tiles.size();
+    if (nstages) *nstages = (int64_t)rp.stages.size();
+    if (ngroups) *ngroups = (int64_t)rp.groups.size();
+    if (nvariants) *nvariants = (int64_t)(rp.var_shift.size() / kMaxG);
+    if (ntiles_t) *ntiles_t = rp.ntile_t;
+    if (max_stage_words) {
+        int64_t m = 0;
+        for (const StageDesc& s : rp.stages) m = std::max<int64_t>(m, ((s.vwords + 3) & ~3) + s.ewords);
+        *max_stage_words = m + kTabWords + kDescWords;
+    }
+    return SPT_OK;
+}
+
+int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
+    if (!plan || !host_out) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    int32_t loc = 0;
+    const RangePlan* rp = range_of_trial(p, trial, &loc);
+    if (!rp) return SPT_ERR_SHAPE;
+    const int rc = ensure_tiling(p);
+    if (rc != SPT_OK) return rc;
+    const int DT = p.opt_dm_tile;
+    const TileDesc& td = rp->tiles[loc / DT];
+    const int dl = loc - td.trial0;
+    for (int32_t c = 0; c < p.nchan; ++c) host_out[c] = INT32_MIN;
+    for (int s = td.stage0; s < td.stage0 + td.nstage; ++s) {
+        const StageDesc& sd = rp->stages[s];
+        for (int g = sd.grp0; g < sd.grp0 + sd.ngrp; ++g) {
+            const GroupDesc& gd = rp->groups[g];
+            const int32_t rel = (int32_t)rp->trial_off[(size_t)g * DT + dl] - gd.vbase;  // r*vlen + b
+            const int32_t r = rel / gd.vlen, b = rel - r * gd.vlen;
+            if (r < 0 || r >= gd.nvar) return SPT_ERR_STATE;
+            const int16_t* sh = &rp->var_shift[(size_t)(gd.var0 + r) * kMaxG];
+            // the gather reads P_r[q + b] = sum_j E_j[q + b + sh_j], and E_j[e] is sample t0 + wlo + e of channel chan0+j
+            for (int j = 0; j < gd.nch; ++j) host_out[gd.chan0 + j] = gd.wlo + b + sh[j];
+        }
+    }
+    return SPT_OK;
+}
+
+int spt_dedisperse(spt_plan* plan, const uint8_t* d_fb, int32_t nbeam, int32_t* d_dmt, void* cuda_stream) {
+    if (!plan || !d_fb || !d_dmt || nbeam < 1) return SPT_ERR_INVALID;
+    if (nbeam > plan->p.max_beams) return SPT_ERR_INVALID;
+    if ((reinterpret_cast<uintptr_t>(d_dmt) & 127) != 0) return SPT_ERR_INVALID;
+    int rc;
+    try {
+        rc = ensure_device(&plan->p);
+    } catch (const std::bad_alloc&) {
+        rc = SPT_ERR_NOMEM;
+    }
+    if (rc != SPT_OK) return rc;
+    return do_dedisperse(&plan->p, d_fb, nbeam, d_dmt, (cudaStream_t)cuda_stream);
+}
+
+int spt_decimated(const spt_plan* plan, int32_t range, const uint16_t** d_ptr, int64_t* nsamp_k) {
+    if (!plan || !d_ptr) return SPT_ERR_INVALID;
+    const Plan& p = plan->p;
+    if (range < 0 || range >= (int32_t)p.ranges.size()) return SPT_ERR_SHAPE;
+    const RangePlan& rp = p.ranges[range];
+    if (nsamp_k) *nsamp_k = rp.nsamp_k;
+    if (rp.decim == 1) { *d_ptr = nullptr; return SPT_OK; }
+    if (!p.dev || p.dev->nbeam_dedisp == 0) return SPT_ERR_STATE;
+    *d_ptr = p.dev->r[range].series;
+    return SPT_OK;
+}
+
+int spt_decimated_stride(const spt_plan* plan, int32_t range, int64_t* row_stride) {
+    if (!plan || !row_stride) return SPT_ERR_INVALID;
+    const Plan& p = plan->p;
+    if (range < 0 || range >= (int32_t)p.ranges.size()) return SPT_ERR_SHAPE;
+    *row_stride = p.ranges[range].stride_k;
+    return SPT_OK;
+}
+
+int spt_decimated_read(spt_plan* plan, int32_t range, int32_t beam, uint16_t* host_out) {
+    if (!plan || !host_out) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (range < 0 || range >= (int32_t)p.ranges.size()) return SPT_ERR_SHAPE;
+    const RangePlan& rp = p.ranges[range];
+    if (rp.decim == 1) return SPT_ERR_INVALID;
+    if (!p.dev || p.dev->nbeam_dedisp == 0) return SPT_ERR_STATE;
+    if (beam < 0 || beam >= p.dev->nbeam_dedisp) return SPT_ERR_SHAPE;
+    SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
+    if (rp.nsamp_k <= 0) return SPT_OK;
+    const uint16_t* src = p.dev->r[range].series + (size_t)beam * p.nchan * rp.stride_k;
+    SPT_CUDA(cudaMemcpy2D(host_out, (size_t)rp.nsamp_k * 2, src, (size_t)rp.stride_k * 2, (size_t)rp.nsamp_k * 2,
+                          (size_t)p.nchan, cudaMemcpyDeviceToHost));
+    return SPT_OK;
+}
+
+int spt_single_pulse_search(spt_plan* plan, const int32_t* d_dmt, int32_t nbeam, float threshold, void* cuda_stream) {
+    if (!plan || !d_dmt || nbeam < 1 || nbeam > plan->p.max_beams || !(threshold == threshold)) return SPT_ERR_INVALID;
+    int rc;
+    try {
+        rc = ensure_device(&plan->p);
+    } catch (const std::bad_alloc&) {
+        rc = SPT_ERR_NOMEM;
+    }
+    if (rc != SPT_OK) return rc;
+    return do_search(&plan->p, d_dmt, nbeam, threshold, (cudaStream_t)cuda_stream);
+}
+
+int spt_trial_stats(spt_plan* plan, int32_t beam, int32_t trial, int64_t* n, int64_t* sum, uint64_t* sumsq) {
+    if (!plan) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (!p.dev || !p.dev->searched) return SPT_ERR_STATE;
+    if (beam < 0 || beam >= p.dev->nbeam_search || trial < 0 || trial >= p.ntrials) return SPT_ERR_SHAPE;
+    SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
+    int32_t loc = 0;
+    const RangePlan* rp = range_of_trial(p, trial, &loc);
+    if (n) *n = rp->nout[loc];
+    const size_t idx = (size_t)beam * p.ntrials + trial;
+    if (sum) SPT_CUDA(cudaMemcpy(sum, p.dev->sum + idx, 8, cudaMemcpyDeviceToHost));
+    if (sumsq) SPT_CUDA(cudaMemcpy(sumsq, p.dev->sumsq + idx, 8, cudaMemcpyDeviceToHost));
+    return SPT_OK;
+}
+
+int spt_trial_stats_all(spt_plan* plan, int32_t nbeam, int64_t* sum, uint64_t* sumsq) {
+    if (!plan) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (!p.dev || !p.dev->searched) return SPT_ERR_STATE;
+    if (nbeam < 1 || nbeam > p.dev->nbeam_search) return SPT_ERR_SHAPE;
+    SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
+    const size_t bytes = (size_t)nbeam * p.ntrials * 8;
+    if (sum) SPT_CUDA(cudaMemcpy(sum, p.dev->sum, bytes, cudaMemcpyDeviceToHost));
+    if (sumsq) SPT_CUDA(cudaMemcpy(sumsq, p.dev->sumsq, bytes, cudaMemcpyDeviceToHost));
+    return SPT_OK;
+}
+
+int spt_candidates_count(spt_plan* plan, int64_t* total, int32_t* overflowed) {
+    if (!plan) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (!p.dev || !p.dev->searched) return SPT_ERR_STATE;
+    SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
+    unsigned long long c = 0;
+    SPT_CUDA(cudaMemcpy(&c, p.dev->count, 8, cudaMemcpyDeviceToHost));
+    if (total) *total = (int64_t)c;
+    if (overflowed) *overflowed = (int64_t)c > p.cand_capacity ? 1 : 0;
+    return SPT_OK;
+}
+
+int spt_candidates_read(spt_plan* plan, spt_candidate* host_out, int64_t cap, int64_t* nwritten) {
+    if (!plan || (!host_out && cap > 0) || cap < 0) return SPT_ERR_INVALID;
+    int64_t total = 0;
+    const int rc = spt_candidates_count(plan, &total, nullptr);
+    if (rc != SPT_OK) return rc;
+    int64_t n = total;
+    if (n > plan->p.cand_capacity) n = plan->p.cand_capacity;
+    if (n > cap) n = cap;
+    if (n > 0) SPT_CUDA(cudaMemcpy(host_out, plan->p.dev->cand, (size_t)n * sizeof(spt_candidate), cudaMemcpyDeviceToHost));
+    if (nwritten) *nwritten = n;
+    return SPT_OK;
+}
+
+int spt_search_host(spt_plan* plan, const uint8_t* h_fb, int32_t nbeam, float threshold, int32_t* h_dmt, int64_t* ncand,
+                    int32_t* overflowed) {
+    if (!plan || !h_fb || nbeam < 1 || nbeam > plan->p.max_beams) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    int rc;
+    try {
+        rc = ensure_device(&p);
+    } catch (const std::bad_alloc&) {
+        rc = SPT_ERR_NOMEM;
+    }
+    if (rc != SPT_OK) return rc;
+    DeviceState* d = p.dev;
+    const size_t fb_bytes = (size_t)p.nchan * p.nsamp;
+    if (!d->h_fb) SPT_CUDA(cudaMalloc((void**)&d->h_fb, fb_bytes * p.max_beams));
+    if (!d->h_dmt) SPT_CUDA(cudaMalloc((void**)&d->h_dmt, (size_t)p.dmt_elems * 4 * p.max_beams + 128));
+    cudaStream_t st = d->own_stream;
+    SPT_CUDA(cudaMemcpyAsync(d->h_fb, h_fb, fb_bytes * nbeam, cudaMemcpyHostToDevice, st));
+    if ((rc = do_dedisperse(&p, d->h_fb, nbeam, d->h_dmt, st)) != SPT_OK) return rc;
+    if ((rc = do_search(&p, d->h_dmt, nbeam, threshold, st)) != SPT_OK) return rc;
+    if (h_dmt) SPT_CUDA(cudaMemcpyAsync(h_dmt, d->h_dmt, (size_t)p.dmt_elems * 4 * nbeam, cudaMemcpyDeviceToHost, st));
+    int64_t total = 0;
+    int32_t ovf = 0;
+    if ((rc = spt_candidates_count(plan, &total, &ovf)) != SPT_OK) return rc;
+    if (ncand) *ncand = total;
+    if (overflowed) *overflowed = ovf;
+    return SPT_OK;
+}
+
+int spt_plan_kernel_times(spt_plan* plan, int32_t cap, int32_t* kind, int32_t* range, double* ms, int32_t* n) {
+    if (!plan || !n || cap < 0) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    *n = 0;
+    if (!p.dev) return SPT_ERR_STATE;
+    if (p.dev->last_stream || p.dev->nbeam_dedisp) SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
+    for (int slot = 0; slot < 2; ++slot)
+        for (auto& t : p.dev->timed[slot]) {
+            if (*n >= cap) return SPT_OK;
+            float f = 0.f;
+            SPT_CUDA(cudaEventElapsedTime(&f, t.e0, t.e1));
+            if (kind) kind[*n] = t.kind;
+            if (range) range[*n] = t.range;
+            if (ms) ms[*n] = (double)f;
+            ++*n;
+        }
+    return SPT_OK;
+}
+
+int spt_plan_launches(const spt_plan* plan, int64_t* launches) {
+    if (!plan || !launches) return SPT_ERR_INVALID;
+    *launches = plan->p.launches;
+    return SPT_OK;
+}
+
+int spt_probe(int32_t kind, int32_t reps, double* warp_instr_per_s, double* elapsed_ms) {
+    if (kind < 0 || kind > 4) return SPT_ERR_INVALID;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        g_last_error = "no CUDA device";
+        return SPT_ERR_CUDA;
+    }
+    if (run_probe(kind, reps, warp_instr_per_s, elapsed_ms) != 0) { g_last_error = "probe failed"; return SPT_ERR_CUDA; }
+    return SPT_OK;
+}
+
+const char* spt_strerror(int code) {
+    switch (code) {
+        case SPT_OK: return "ok";
+        case SPT_ERR_INVALID: return "invalid argument";
+        case SPT_ERR_UNSUPPORTED: return "unsupported configuration";
+        case SPT_ERR_NOMEM: return "out of memory";
+        case SPT_ERR_CUDA: return "CUDA error";
+        case SPT_ERR_SHAPE: return "buffer too small or index out of range";
+        case SPT_ERR_STATE: return "call out of order";
+        default: return "unknown error";
+    }
+}
+
+const char* spt_last_error(void) { return g_last_error.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,44 @@
+// kernels.h -- launchers of the CUDA kernels (dedisperse.cu, sps.cu, probe.cu).  Not part of the ABI.
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include "internal.h"
+
+namespace spt {
+
+void launch_decimate(const uint8_t* x, int64_t in_row_stride, int64_t in_beam_stride, uint16_t* y,
+                     int64_t out_row_stride, int64_t out_beam_stride, int32_t nchan, int32_t nbeam, int64_t nsamp_k,
+                     int32_t k, cudaStream_t st);
+
+template <typename T>
+void launch_dedisp_naive(const T* y, int64_t row_stride, int64_t beam_stride, const int32_t* d_delay,
+                         const int32_t* d_nout, const int64_t* d_offset, int32_t nchan, int32_t ndm, int32_t nbeam,
+                         int32_t max_nout, int32_t* out, int64_t out_beam_stride, cudaStream_t st);
+
+int launch_dedisp_tiled(bool is_u16, int DT, int G, const void* in, int64_t row_stride, int64_t beam_stride,
+                        int32_t* out, int64_t out_beam_stride, const TileDesc* tiles, const StageDesc* stages,
+                        const GroupDesc* groups, const int16_t* var_shift, const uint16_t* trial_off,
+                        const int32_t* nout, const int64_t* offset, int32_t ntile_dm, int32_t ntile_t, int32_t nbeam,
+                        cudaStream_t st);
+
+struct SpsArgs {
+    const int32_t* dmt;
+    int64_t beam_stride;            // int32 elements per beam
+    const int32_t* nout;            // [ntrials] global trial index
+    const int64_t* offset;          // [ntrials]
+    int32_t ntrials;
+    int32_t nw;
+    int32_t widths[kMaxWidths];
+    double threshold;
+    int64_t* sum;                   // [nbeam][ntrials]
+    unsigned long long* sumsq;      // [nbeam][ntrials]
+    spt_candidate* cand;
+    unsigned long long* count;      // exact number found (may exceed capacity)
+    long long capacity;
+};
+void launch_sps(const SpsArgs& a, int32_t nbeam, cudaStream_t st);
+
+int run_probe(int kind, int reps, double* warp_instr_per_s, double* elapsed_ms);
+
+}  // namespace spt

@@ -25,3 +25,21 @@ def synth():
     from paper_2606_27262_b200 import synth as s
     s.build()
     return s
+
+
+@pytest.fixture(scope="session")
+def api():
+    """The ctypes binding over libspt.so, built in-tree with nvcc (cross-compiles without a GPU)."""
+    from paper_2606_27262_b200 import build
+    build.build()
+    from paper_2606_27262_b200 import api as a
+    a.lib()
+    return a
+
+
+@pytest.fixture(scope="session")
+def cuda():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("this test needs a CUDA device (run with -m 'not gpu' on a CPU box)")
+    return torch

@@ -1,0 +1,120 @@
+"""Shared comparison code of the parity tests: CUDA path (through the C ABI) vs the oracle.
+
+The rules are those of BASELINE.json north_star / DESIGN.md section 4: bit-exact delay tables, decimated series,
+int32 DM transform and integer statistics; |dSNR| <= 1e-3; candidate lists identical except for events whose oracle
+S/N lies within 1e-3 of the threshold (and widths that are tied within 1e-3).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+SNR_TOL = 1e-3
+
+
+def make_plan(api, w, nbeam=None, cand_capacity=1 << 22, options=None, ranges=None, widths=None, nsamp=None):
+    return api.Plan(w.fch1, w.foff, w.nchan, w.tsamp, nsamp or w.nsamp, ranges or w.ranges, widths or w.widths,
+                    max_beams=nbeam or w.nbeam, cand_capacity=cand_capacity, options=options)
+
+
+def check_plan_against_oracle(orc, plan, w, ranges=None, stride=1):
+    """Trial list, delay rows, nout and row offsets, bit-exact."""
+    ranges = ranges or w.ranges
+    dm, rg, dec, nout, off = plan.trial_table()
+    d = 0
+    expect_off = 0
+    for ri, (lo, step, ndm, k) in enumerate(ranges):
+        dly = orc.delay_table(w.fch1, w.foff, w.nchan, w.tsamp, lo, step, ndm, k)
+        no = orc.nout(dly, plan.nsamp, k)
+        for i in range(ndm):
+            assert rg[d] == ri and dec[d] == k
+            assert dm[d] == lo + float(i) * step
+            assert nout[d] == no[i], (d, nout[d], no[i])
+            assert off[d] == expect_off
+            expect_off += (int(no[i]) + 31) // 32 * 32
+            if i % stride == 0 or i == ndm - 1:
+                assert np.array_equal(plan.delays(d), dly[i]), ("delay row", d)
+            d += 1
+    assert d == plan.ntrials and expect_off == plan.dmt_elems_per_beam
+
+
+def rows_of(plan, dmt_host, beam=0):
+    """Yield (trial, row view) of one beam of a host copy of the DM transform."""
+    _, _, _, nout, off = plan.trial_table()
+    base = dmt_host[beam]
+    for d in range(plan.ntrials):
+        yield d, base[off[d]: off[d] + nout[d]]
+
+
+def check_dmt_against_oracle(plan, dmt_host, oracle_ranges, beam=0):
+    """Every valid element of every row equals the oracle's, bit for bit."""
+    _, _, _, nout, off = plan.trial_table()
+    d = 0
+    for rr in oracle_ranges:
+        for i in range(len(rr.nout)):
+            got = dmt_host[beam][off[d]: off[d] + nout[d]]
+            exp = rr.dmt[rr.rowoff[i]: rr.rowoff[i + 1]]
+            assert nout[d] == rr.nout[i]
+            if not np.array_equal(got, exp):
+                bad = np.flatnonzero(got != exp)
+                raise AssertionError(f"DM transform mismatch: trial {d} (range row {i}), {bad.size} of {exp.size} samples, "
+                                     f"first at t={bad[0]}: got {got[bad[0]]} expected {exp[bad[0]]}")
+            d += 1
+    assert d == plan.ntrials
+
+
+def check_stats_against_oracle(plan, oracle_ranges, beam=0, nbeam=1):
+    s, q = plan.trial_stats_all(nbeam)
+    d = 0
+    for rr in oracle_ranges:
+        for i in range(len(rr.nout)):
+            assert int(s[beam, d]) == int(rr.search.sum[i]), ("sum", d)
+            assert int(q[beam, d]) == int(rr.search.sumsq[i]), ("sumsq", d)
+            d += 1
+
+
+def check_candidates_against_oracle(orc, plan, cands, oracle_ranges, widths, threshold, beam=0):
+    """cands: structured array from spt_candidates_read (all beams).  Returns a dict of counts for the report."""
+    mine = cands[cands["beam"] == beam]
+    order = np.lexsort((mine["t"], mine["trial"]))
+    mine = mine[order]
+    # unique key (trial, t)
+    key = mine["trial"].astype(np.int64) << 32 | mine["t"].astype(np.int64)
+    assert np.unique(key).size == key.size, "duplicate (trial, t) in the candidate list"
+    starts = np.searchsorted(mine["trial"], np.arange(plan.ntrials + 1))
+    stats = dict(oracle=0, gpu=int(mine.size), matched=0, near_threshold_only_oracle=0, near_threshold_only_gpu=0,
+                 width_near_ties=0, max_dsnr=0.0)
+    d = 0
+    for rr in oracle_ranges:
+        sr = rr.search
+        for i in range(len(rr.nout)):
+            o_t = sr.t[sr.candoff[i]: sr.candoff[i + 1]]
+            o_w = sr.w[sr.candoff[i]: sr.candoff[i + 1]]
+            o_s = sr.snr[sr.candoff[i]: sr.candoff[i + 1]]
+            g = mine[starts[d]: starts[d + 1]]
+            stats["oracle"] += int(o_t.size)
+            if o_t.size or g.size:
+                row = rr.dmt[rr.rowoff[i]: rr.rowoff[i + 1]]
+                common, io, ig = np.intersect1d(o_t, g["t"], assume_unique=True, return_indices=True)
+                ds = np.abs(o_s[io] - g["snr"][ig].astype(np.float64))
+                if ds.size:
+                    stats["max_dsnr"] = max(stats["max_dsnr"], float(ds.max()))
+                    assert ds.max() <= SNR_TOL, f"trial {d}: |dSNR| = {ds.max()}"
+                wbad = np.flatnonzero(o_w[io] != g["width"][ig])
+                for j in wbad:  # allowed only for a near tie between widths (rule D2 iv)
+                    alt = orc.snr_at(row, int(g["width"][ig[j]]), int(common[j]))
+                    assert abs(alt - o_s[io[j]]) <= SNR_TOL, f"trial {d} t {common[j]}: width {g['width'][ig[j]]} vs {o_w[io[j]]}"
+                    stats["width_near_ties"] += 1
+                stats["matched"] += int(common.size)
+                only_o = np.setdiff1d(np.arange(o_t.size), io)
+                for j in only_o:
+                    assert abs(o_s[j] - threshold) <= SNR_TOL, f"trial {d} t {o_t[j]}: oracle-only candidate snr {o_s[j]}"
+                    stats["near_threshold_only_oracle"] += 1
+                only_g = np.setdiff1d(np.arange(g.size), ig)
+                if only_g.size:
+                    best, _ = orc.best_width(row, widths)
+                    for j in only_g:
+                        b = best[int(g["t"][j])]
+                        assert abs(b - threshold) <= SNR_TOL, f"trial {d} t {g['t'][j]}: GPU-only candidate, oracle best {b}"
+                        stats["near_threshold_only_gpu"] += 1
+            d += 1
+    return stats

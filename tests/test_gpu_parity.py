@@ -1,0 +1,216 @@
+"""Parity of the CUDA path (through the C ABI) with the oracle, element by element, on seeded synthetic inputs.
+
+Bar (BASELINE.json north_star): bit-exact delay tables, decimated series, int32 DM transform and integer statistics;
+|dSNR| <= 1e-3; identical candidate lists except for events within 1e-3 of the threshold.
+"""
+import numpy as np
+import pytest
+
+from helpers import (check_candidates_against_oracle, check_dmt_against_oracle, check_plan_against_oracle,
+                     check_stats_against_oracle, make_plan)
+
+pytestmark = pytest.mark.gpu
+
+TSAMP = 1.31072e-3
+
+
+class Shape:
+    """A free-form workload (same attribute names as synth.Workload) for the odd-shape cases."""
+
+    def __init__(self, fch1, foff, nchan, nsamp, ranges, widths, threshold, nbeam=1, tsamp=TSAMP):
+        self.fch1, self.foff, self.nchan, self.nsamp, self.ranges = fch1, foff, nchan, nsamp, ranges
+        self.widths, self.threshold, self.nbeam, self.tsamp = widths, threshold, nbeam, tsamp
+
+
+def run_gpu(cuda, api, w, fb_host, options=None, search=True, cand_capacity=1 << 22):
+    """fb_host: uint8 [nbeam][nchan][nsamp].  Returns (plan, dmt host array [nbeam][elems], candidates or None)."""
+    plan = make_plan(api, w, nbeam=fb_host.shape[0], cand_capacity=cand_capacity, options=options)
+    d_fb = cuda.from_numpy(fb_host).cuda()
+    d_dmt = cuda.full((fb_host.shape[0], plan.dmt_elems_per_beam), -7, dtype=cuda.int32, device="cuda")
+    plan.dedisperse(d_fb, d_dmt)
+    cands = None
+    if search:
+        plan.single_pulse_search(d_dmt, w.threshold)
+        total, ovf = plan.candidates_count()
+        assert not ovf, f"candidate list overflowed ({total})"
+        cands = plan.candidates_read()
+        assert cands.size == total
+    cuda.cuda.synchronize()
+    return plan, d_dmt.cpu().numpy(), cands
+
+
+def oracle_path(orc, w, fb, search=True):
+    return orc.run_path(fb, w.fch1, w.foff, w.tsamp, w.ranges, w.widths, w.threshold, do_search=search)
+
+
+# ---- config 1 (Tiny), every kernel variant --------------------------------------------------------------------
+@pytest.mark.parametrize("options", [
+    {"dedisp_kernel": 1},
+    {"group": 1}, {"group": 2}, {"group": 4}, {"group": 8}, {"group": 4, "dm_tile": 32}, {"group": 8, "dm_tile": 32},
+])
+def test_cfg1_dm_transform_bit_exact(cuda, api, orc, synth, options):
+    w = synth.workload(1)
+    fb = synth.generate(w)
+    ref = oracle_path(orc, w, fb, search=False)
+    plan, dmt, _ = run_gpu(cuda, api, w, fb[None], options=options, search=False)
+    check_plan_against_oracle(orc, plan, w)
+    check_dmt_against_oracle(plan, dmt, ref)
+    # row padding is never written
+    _, _, _, nout, off = plan.trial_table()
+    for d in range(plan.ntrials - 1):
+        assert np.all(dmt[0][off[d] + nout[d]: off[d + 1]] == -7)
+
+
+def test_cfg1_search_and_recovery(cuda, api, orc, synth):
+    w = synth.workload(1)
+    fb = synth.generate(w)
+    ref = oracle_path(orc, w, fb)
+    plan, dmt, cands = run_gpu(cuda, api, w, fb[None])
+    check_dmt_against_oracle(plan, dmt, ref)
+    check_stats_against_oracle(plan, ref)
+    st = check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+    assert st["oracle"] > 0 and st["matched"] >= st["oracle"] - st["near_threshold_only_oracle"]
+    # the injected burst (DM 50 = trial 50, t 1000, width 4, S/N 24) is the top candidate of the CUDA path too
+    top = cands[np.argmax(cands["snr"])]
+    assert abs(int(top["trial"]) - 50) <= 1 and abs(int(top["t"]) - 1000) <= 2 and top["width"] in (2, 4, 8)
+    assert abs(float(top["snr"]) - 24.0) <= 3.0
+    n, s, q = plan.trial_stats(0, 50)
+    assert (n, s, q) == (int(ref[0].nout[50]), int(ref[0].search.sum[50]), int(ref[0].search.sumsq[50]))
+
+
+# ---- several ranges with decimation, several tiles and a ragged tail ---------------------------------------------
+def mini3(synth, seed, nsamp=65536, nchan=1024):
+    """Config-3-like: three ranges (decimation 1, 2, 4), one dispersed burst inside each, a zero-DM spike."""
+    import math
+    w = synth.Workload("mini3", 0, 1, nchan, nsamp, 500.0, -200.0 / nchan, TSAMP, 128.0, 10.0,
+                       [(0.0, 0.2, 150, 1), (480.0, 0.5, 70, 2), (1900.0, 1.0, 101, 4)],
+                       [1, 2, 4, 8, 16, 32, 64, 128, 256, 512], 6.0, seed)
+    amp = lambda snr, wid: snr * w.std / math.sqrt(nchan * wid)
+    w.bursts = [[synth.Burst(dm=15.1, t0=20000, width=4, snr=30.0, amp=amp(30.0, 4)),
+                 synth.Burst(dm=497.3, t0=9000, width=8, snr=40.0, amp=amp(40.0, 8)),
+                 synth.Burst(dm=1950.0, t0=3000, width=16, snr=50.0, amp=amp(50.0, 16))]]
+    w.spikes = [(30000, 3, 4.0)]
+    return w
+
+
+@pytest.mark.parametrize("options", [{"group": 4}, {"group": 8}, {"group": 2, "dm_tile": 32}, {"dedisp_kernel": 1}])
+def test_multirange_decimated_bit_exact(cuda, api, orc, synth, options):
+    w = mini3(synth, 11)
+    fb = synth.generate(w)
+    ref = oracle_path(orc, w, fb, search=False)
+    plan, dmt, _ = run_gpu(cuda, api, w, fb[None], options=options, search=False)
+    check_plan_against_oracle(orc, plan, w, stride=7)
+    check_dmt_against_oracle(plan, dmt, ref)
+    for ri, rr in enumerate(ref):                      # decimated series, bit-exact
+        got = plan.decimated_read(ri)
+        if rr.decim == 1:
+            assert got is None
+        else:
+            assert got.dtype == np.uint16 and np.array_equal(got, rr.series)
+
+
+def test_multirange_search(cuda, api, orc, synth):
+    w = mini3(synth, 12)
+    fb = synth.generate(w)
+    ref = oracle_path(orc, w, fb)
+    per_range = [int(r.search.candoff[-1]) for r in ref]
+    assert all(n > 0 for n in per_range), per_range     # every range (decimation 1, 2, 4) has detections
+    plan, dmt, cands = run_gpu(cuda, api, w, fb[None], cand_capacity=sum(per_range) + 4096)
+    check_dmt_against_oracle(plan, dmt, ref)
+    check_stats_against_oracle(plan, ref)
+    st = check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+    assert st["oracle"] > 1000, st            # the append path is exercised
+    assert st["near_threshold_only_oracle"] + st["near_threshold_only_gpu"] <= max(5, st["oracle"] // 1000)
+
+
+# ---- odd shapes and degenerate inputs -------------------------------------------------------------------------
+@pytest.mark.parametrize("fill", ["uniform", "all255", "zero"])
+@pytest.mark.parametrize("options", [{"group": 4}, {"group": 8}, {"dedisp_kernel": 1}])
+def test_odd_shapes(cuda, api, orc, fill, options):
+    # 71 channels (not a multiple of any group size), 5003 samples (rows not 16-byte multiples), trial counts that
+    # are not multiples of the DM tile, decimation 8, a range whose last trials have no valid output at all
+    w = Shape(420.0, -1.0, 71, 5003, [(3.0, 0.7, 77, 1), (60.0, 1.1, 41, 2), (100.0, 2.0, 5, 8), (600.0, 150.0, 4, 1)],
+              [1, 3, 7, 20], 5.0)
+    rs = np.random.default_rng(5)
+    if fill == "uniform":
+        fb = rs.integers(0, 256, size=(w.nchan, w.nsamp), dtype=np.uint8)
+    elif fill == "all255":
+        fb = np.full((w.nchan, w.nsamp), 255, dtype=np.uint8)      # every 16-bit lane at its maximum
+    else:
+        fb = np.zeros((w.nchan, w.nsamp), dtype=np.uint8)          # sigma == 0: no candidates
+    ref = oracle_path(orc, w, fb)
+    plan, dmt, cands = run_gpu(cuda, api, w, fb[None], options=options)
+    check_plan_against_oracle(orc, plan, w)
+    _, _, _, nout, _ = plan.trial_table()
+    assert (nout == 0).any() and (nout > 0).any()
+    check_dmt_against_oracle(plan, dmt, ref)
+    check_stats_against_oracle(plan, ref)
+    st = check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+    if fill != "uniform":
+        assert st["gpu"] == 0 and st["oracle"] == 0
+    for ri, rr in enumerate(ref):
+        if rr.decim > 1:
+            assert np.array_equal(plan.decimated_read(ri), rr.series)
+
+
+def test_all255_wide_band_lane_limits(cuda, api, orc):
+    """4096 channels of 255 at decimation 4: int32 outputs reach 4096*255*4 and every packed lane flush is needed."""
+    w = Shape(500.0, -0.048828125, 4096, 4096, [(0.0, 0.2, 70, 1), (0.0, 1.0, 70, 4)], [1, 2, 1024], 6.0)
+    fb = np.full((w.nchan, w.nsamp), 255, dtype=np.uint8)
+    ref = oracle_path(orc, w, fb, search=False)
+    plan, dmt, _ = run_gpu(cuda, api, w, fb[None], search=False)
+    check_dmt_against_oracle(plan, dmt, ref)
+    assert dmt.max() == 4096 * 255 * 4
+
+
+# ---- config 2 at reduced length -----------------------------------------------------------------------------------
+def test_cfg2_reduced(cuda, api, orc, synth):
+    w = synth.workload(2, nsamp=16384)
+    fb = synth.generate(w)
+    ref = oracle_path(orc, w, fb)
+    plan, dmt, cands = run_gpu(cuda, api, w, fb[None])
+    check_plan_against_oracle(orc, plan, w, stride=41)
+    check_dmt_against_oracle(plan, dmt, ref)
+    check_stats_against_oracle(plan, ref)
+    check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+
+
+# ---- multibeam batch (config 4 shape, reduced) -----------------------------------------------------------------------
+def test_multibeam_batch(cuda, api, orc, synth):
+    w = synth.workload(4, nsamp=1 << 14, nbeam=3)
+    w.ranges = [(0.0, 0.2, 130, 1), (500.0, 0.5, 66, 2), (1000.0, 1.0, 40, 4)]
+    w.threshold = 6.0
+    fb = np.stack([synth.generate(w, beam=b) for b in range(w.nbeam)])
+    fb[1, :, 5000:5004] += 30
+    plan, dmt, cands = run_gpu(cuda, api, w, fb)
+    assert set(np.unique(cands["beam"])) <= {0, 1, 2}
+    for b in range(w.nbeam):
+        ref = oracle_path(orc, w, fb[b])
+        check_dmt_against_oracle(plan, dmt, ref, beam=b)
+        check_stats_against_oracle(plan, ref, beam=b, nbeam=w.nbeam)
+        check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold, beam=b)
+
+
+# ---- the host-buffer entry point ---------------------------------------------------------------------------------------
+def test_search_host_matches_device_path(cuda, api, orc, synth):
+    w = synth.workload(1)
+    fb = synth.generate(w)
+    ref = oracle_path(orc, w, fb)
+    plan = make_plan(api, w)
+    h_dmt = np.full((1, plan.dmt_elems_per_beam), -7, dtype=np.int32)
+    ncand, ovf = plan.search_host(fb[None], w.threshold, h_dmt)
+    assert not ovf
+    check_dmt_against_oracle(plan, h_dmt, ref)
+    cands = plan.candidates_read()
+    assert cands.size == ncand
+    check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+    assert plan.launches() >= 2
+
+
+def test_candidate_overflow_is_reported(cuda, api, synth):
+    w = synth.workload(1)
+    fb = synth.generate(w)
+    plan = make_plan(api, w, cand_capacity=3)
+    ncand, ovf = plan.search_host(fb[None], 2.0)
+    assert ovf and ncand > 3
+    assert plan.candidates_read().size == 3
