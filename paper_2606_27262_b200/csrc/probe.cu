@@ -64,22 +64,29 @@ __global__ void __launch_bounds__(kProbeThreads) probe_mixed(uint32_t* out, uint
 
 template <int VEC>
 __global__ void __launch_bounds__(kProbeThreads) probe_lds(uint32_t* out, uint32_t seed) {
-    __shared__ __align__(16) uint32_t buf[kProbeThreads * 4 + 64];
-    for (int i = threadIdx.x; i < kProbeThreads * 4 + 64; i += kProbeThreads) buf[i] = i ^ seed;
+    // 32 KB: the address moves every iteration so that no load can be merged with another
+    __shared__ __align__(16) uint32_t buf[8192];
+    for (int i = threadIdx.x; i < 8192; i += kProbeThreads) buf[i] = i ^ seed;
     __syncthreads();
     uint32_t acc = 0;
-    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(buf) + threadIdx.x * 4 * VEC;
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(buf);
     for (int it = 0; it < kProbeIters; ++it) {
+        if (VEC == 1) {
+            // lane-contiguous 128-byte rows (conflict free); 8 different rows per iteration
+            const uint32_t a0 = sbase + ((threadIdx.x & 31) << 2) + (((threadIdx.x >> 5) + it) & 15) * 2048;
 #pragma unroll
-        for (int i = 0; i < kIlp; ++i) {
-            if (VEC == 1) {
+            for (int i = 0; i < kIlp; ++i) {
                 uint32_t v;
-                asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(sbase + (uint32_t)((i & 3) * 16 * VEC)));
+                asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(a0 + (uint32_t)(i * 128)) : "memory");
                 acc ^= v;
-            } else {
+            }
+        } else {
+            const uint32_t a0 = sbase + ((threadIdx.x & 31) << 4) + (((threadIdx.x >> 5) + it) & 7) * 4096;
+#pragma unroll
+            for (int i = 0; i < kIlp; ++i) {
                 uint32_t v0, v1, v2, v3;
                 asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v0), "=r"(v1), "=r"(v2), "=r"(v3)
-                             : "r"(sbase + (uint32_t)((i & 3) * 16)));
+                             : "r"(a0 + (uint32_t)((i & 3) * 512) + (uint32_t)((i >> 2) * 2048)) : "memory");
                 acc ^= v0 ^ v1 ^ v2 ^ v3;
             }
         }
