@@ -28,10 +28,9 @@ static int cuda_fail(cudaError_t e, const char* what) {
 struct RangeDev {
     int32_t* delay = nullptr;       // only for the naive kernel
     TileDesc* tiles = nullptr;
-    StageDesc* stages = nullptr;
-    GroupDesc* groups = nullptr;
-    int16_t* var_shift = nullptr;
-    uint16_t* trial_off = nullptr;
+    StageIndex* sidx = nullptr;
+    RowDesc* rows = nullptr;
+    uint32_t* blob = nullptr;
     uint16_t* series = nullptr;     // decimated input [max_beams][nchan][stride_k] (decim > 1)
 };
 
@@ -91,8 +90,8 @@ static void free_device(Plan* p) {
     DeviceState* d = p->dev;
     if (!d) return;
     for (RangeDev& r : d->r) {
-        cudaFree(r.delay); cudaFree(r.tiles); cudaFree(r.stages); cudaFree(r.groups);
-        cudaFree(r.var_shift); cudaFree(r.trial_off); cudaFree(r.series);
+        cudaFree(r.delay); cudaFree(r.tiles); cudaFree(r.sidx); cudaFree(r.rows); cudaFree(r.blob);
+        cudaFree(r.series);
     }
     cudaFree(d->nout); cudaFree(d->offset); cudaFree(d->sum); cudaFree(d->sumsq);
     cudaFree(d->cand); cudaFree(d->count); cudaFree(d->fb_pad); cudaFree(d->h_fb); cudaFree(d->h_dmt);
@@ -128,10 +127,9 @@ static int ensure_device(Plan* p) {
         if (p->opt_kernel == 1) rc = upload(&rd.delay, rp.delay);
         else {
             if ((rc = upload(&rd.tiles, rp.tiles)) != SPT_OK) break;
-            if ((rc = upload(&rd.stages, rp.stages)) != SPT_OK) break;
-            if ((rc = upload(&rd.groups, rp.groups)) != SPT_OK) break;
-            if ((rc = upload(&rd.var_shift, rp.var_shift)) != SPT_OK) break;
-            if ((rc = upload(&rd.trial_off, rp.trial_off)) != SPT_OK) break;
+            if ((rc = upload(&rd.sidx, rp.sidx)) != SPT_OK) break;
+            if ((rc = upload(&rd.rows, rp.rows)) != SPT_OK) break;
+            if ((rc = upload(&rd.blob, rp.blob)) != SPT_OK) break;
         }
         if (rc == SPT_OK && rp.decim > 1) {
             const size_t bytes = (size_t)p->max_beams * p->nchan * rp.stride_k * sizeof(uint16_t);
@@ -202,9 +200,9 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
             else launch_dedisp_naive<uint8_t>((const uint8_t*)src, rs, (int64_t)p->nchan * rs, rd.delay, nout, off,
                                               p->nchan, rp.ndm, nbeam, rp.max_nout, d_dmt, p->dmt_elems, st);
         } else {
-            const int rc = launch_dedisp_tiled(u16, p->opt_dm_tile, p->opt_group, src, rs, (int64_t)p->nchan * rs, d_dmt,
-                                               p->dmt_elems, rd.tiles, rd.stages, rd.groups, rd.var_shift, rd.trial_off,
-                                               nout, off, (int32_t)rp.tiles.size(), rp.ntile_t, nbeam, st);
+            const int rc = launch_dedisp_tiled(u16, p->opt_dm_tile, src, rs, (int64_t)p->nchan * rs, d_dmt, p->dmt_elems,
+                                               rd.tiles, rd.sidx, rd.rows, rd.blob, rp.vcap_words, nout, off,
+                                               (int32_t)rp.tiles.size(), rp.ntile_t, nbeam, st);
             if (rc != 0) { g_last_error = "dedisp_tiled: launch configuration rejected"; return SPT_ERR_CUDA; }
         }
         p->launches++;
@@ -374,14 +372,23 @@ int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int6
     if (rc != SPT_OK) return rc;
     const RangePlan& rp = p.ranges[range];
     if (ntiles_dm) *ntiles_dm = (int64_t)rp.tiles.size();
-    if (nstages) *nstages = (int64_t)rp.stages.size();
-    if (ngroups) *ngroups = (int64_t)rp.groups.size();
-    if (nvariants) *nvariants = (int64_t)(rp.var_shift.size() / kMaxG);
+    if (nstages) *nstages = (int64_t)rp.sidx.size();
+    if (ngroups) *ngroups = rp.ngroups;
+    if (nvariants) *nvariants = rp.nvariants;
     if (ntiles_t) *ntiles_t = rp.ntile_t;
     if (max_stage_words) {
+        // largest shared-memory footprint of a stage: variant words + raw-row bytes, plus the fixed control area
+        const int es = rp.decim == 1 ? 1 : 2;
         int64_t m = 0;
-        for (const StageDesc& s : rp.stages) m = std::max<int64_t>(m, ((s.vwords + 3) & ~3) + s.ewords);
-        *max_stage_words = m + kTabWords + kDescWords;
+        for (const StageIndex& si : rp.sidx) {
+            const uint32_t* b = &rp.blob[si.blob_word0];
+            int64_t v = 0, r = 0;
+            for (uint32_t k = 0; k < b[0]; ++k) v += (int64_t)b[kBlobHdrWords + 4 * k + 1] * b[kBlobHdrWords + 4 * k + 3];
+            for (uint32_t k = 0; k < si.nrows; ++k) r += (int64_t)rp.rows[si.row0 + k].nelem * es;
+            if (v > rp.vcap_words || r > kSmemDataBytes - (int64_t)rp.vcap_words * 4) return SPT_ERR_STATE;
+            m = std::max(m, v + r / 4);
+        }
+        *max_stage_words = m + (kSmemCtrlBytes + 2 * kBlobBytes) / 4;
     }
     return SPT_OK;
 }
@@ -395,19 +402,44 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
     const int rc = ensure_tiling(p);
     if (rc != SPT_OK) return rc;
     const int DT = p.opt_dm_tile;
+    const int es = rp->decim == 1 ? 1 : 2;
     const TileDesc& td = rp->tiles[loc / DT];
     const int dl = loc - td.trial0;
     for (int32_t c = 0; c < p.nchan; ++c) host_out[c] = INT32_MIN;
     for (int s = td.stage0; s < td.stage0 + td.nstage; ++s) {
-        const StageDesc& sd = rp->stages[s];
-        for (int g = sd.grp0; g < sd.grp0 + sd.ngrp; ++g) {
-            const GroupDesc& gd = rp->groups[g];
-            const int32_t rel = (int32_t)rp->trial_off[(size_t)g * DT + dl] - gd.vbase;  // r*vlen + b
-            const int32_t r = rel / gd.vlen, b = rel - r * gd.vlen;
-            if (r < 0 || r >= gd.nvar) return SPT_ERR_STATE;
-            const int16_t* sh = &rp->var_shift[(size_t)(gd.var0 + r) * kMaxG];
-            // the gather reads P_r[q + b] = sum_j E_j[q + b + sh_j], and E_j[e] is sample t0 + wlo + e of channel chan0+j
-            for (int j = 0; j < gd.nch; ++j) host_out[gd.chan0 + j] = gd.wlo + b + sh[j];
+        const StageIndex& si = rp->sidx[s];
+        const uint32_t* b = &rp->blob[si.blob_word0];
+        const uint32_t ngrp = b[0];
+        const uint32_t* pairs = b + kBlobHdrWords + 4 * ngrp;
+        const uint32_t* toff = pairs + b[2];
+        for (uint32_t g = 0; g < ngrp; ++g) {
+            const uint32_t* gh = b + kBlobHdrWords + 4 * g;
+            const int32_t vbase = (int32_t)gh[0], vlen = (int32_t)gh[1], nvar = (int32_t)gh[3];
+            const uint32_t pair0 = gh[2] & 0xffffu, npairs = gh[2] >> 16;
+            const uint32_t tw = toff[(g * DT + dl) / 2];
+            const int32_t to = (int32_t)(((g * DT + dl) & 1) ? (tw >> 16) : (tw & 0xffffu));
+            const int32_t rel = to - vbase, r = rel / vlen, bb = rel - r * vlen;
+            if (r < 0 || r >= nvar) return SPT_ERR_STATE;
+            // the gather reads P_r[q + bb]; P_r[u] sums, per channel, the pair the variant takes: the base pair unless a
+            // delta pair of the same row has bit r set; a pair at byte offset `off` of row (soff, astart) is element
+            // t0 + astart + (off - soff)/es + u of that channel
+            int32_t cur_chan = -1;
+            for (uint32_t q = 0; q < npairs; ++q) {
+                const uint32_t d = pairs[pair0 + q];
+                const int32_t off = (int32_t)(d & 0x1ffffu);
+                const RowDesc* row = nullptr;
+                for (uint32_t k = 0; k < si.nrows; ++k) {
+                    const RowDesc& rr = rp->rows[si.row0 + k];
+                    if (off >= rr.soff && off < rr.soff + rr.nelem * es) { row = &rr; break; }
+                }
+                if (!row) return SPT_ERR_STATE;
+                const int32_t dly = row->astart + (off - row->soff) / es + bb;
+                if (d & kPairBaseBit) { cur_chan = row->chan; host_out[cur_chan] = dly; }
+                else {
+                    if (row->chan != cur_chan) return SPT_ERR_STATE;
+                    if ((d >> 20) & (1u << r)) host_out[cur_chan] = dly;
+                }
+            }
         }
     }
     return SPT_OK;

@@ -102,38 +102,61 @@ template void launch_dedisp_naive<uint16_t>(const uint16_t*, int64_t, int64_t, c
 // 16 bits of word q accumulate output t0+q, the high 16 bits output t0+kH+q.  Because both halves of a word
 // move together, a read at ANY sample offset is one aligned 32-bit shared-memory load (no byte realignment).
 //
-// Per stage (a run of channel groups that fits shared memory), see plan.cpp for the tables:
-//   A  expand : E_j[e]  = y[c0+j][t0+wlo+e] | y[c0+j][t0+wlo+e+kH] << 16          (global -> shared)
-//   B  presum : P_r[u]  = sum_j E_j[u + shift_r[j]]   for every variant r of every group  (shared -> shared)
-//   C  gather : acc[d][q] += P_{r(d)}[q + b(d)]       one LDS.32 + one IADD = 2*G algorithmic adds, packed
+// Per stage (a run of channel groups that fits shared memory; tables built by plan.cpp):
+//   T  TMA    : one elected warp issues cp.async.bulk copies of the stage's table blob and raw channel rows
+//               (global -> shared, completion on an mbarrier); they land while the previous stage is gathered
+//   B  presum : P_r[u] = sum_j y[c0+j][t0 + dmin + u + rho^r_j] | (same at +kH) << 16 for every variant r of every
+//               group, in one sweep over the group's (channel, shift) pairs: base pairs go to all variants, delta
+//               pairs replace the base for the variants in their mask (predicated adds)
+//   C  gather : acc[d][q] += P_{r(d)}[q + b(d)]       one LDS.32 + one add = 2*G algorithmic adds
 //   F  flush  : every <= 257/decim channels the 16-bit lanes are widened into the int32 DM transform (L2 RMW).
 // ---------------------------------------------------------------------------------------------------------------
 struct TiledArgs {
     const void* in;            // series of beam 0
-    int64_t row_stride;        // elements
+    int64_t row_stride;        // elements (multiple of 16)
     int64_t beam_stride;       // elements
     int32_t* out;
     int64_t out_beam_stride;
     const TileDesc* tiles;
-    const StageDesc* stages;
-    const GroupDesc* groups;
-    const int16_t* var_shift;
-    const uint16_t* trial_off;
+    const StageIndex* sidx;
+    const RowDesc* rows;
+    const uint32_t* blob;
     const int32_t* nout;       // range local
     const int64_t* offset;     // range local
-    int32_t ntile_dm, ntile_t, nbeam;
+    int32_t vcap_words, ntile_dm, ntile_t, nbeam;
 };
 
-__device__ __forceinline__ uint32_t ld_word_or_zero(const uint32_t* p, bool ok) { return ok ? __ldg(p) : 0u; }
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@!p bra WAIT_%=;\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-template <typename T, int DT, int G>
+template <typename T, int DT>
 __global__ void __launch_bounds__(kThreads, 1) dedisp_tiled_kernel(const TiledArgs a) {
-    constexpr int TPW = DT / (kThreads / 32);
-    static_assert(TPW >= 1, "DT must be a multiple of the warp count");
-    extern __shared__ __align__(16) uint32_t smem[];
-    uint16_t* s_tab = reinterpret_cast<uint16_t*>(smem);                    // [ngrp][DT]
-    GroupDesc* s_grp = reinterpret_cast<GroupDesc*>(smem + kTabWords);      // [ngrp]
-    uint32_t* s_data = smem + kTabWords + kDescWords;                       // variants, then expansion rows
+    constexpr int NW = kThreads / 32;
+    constexpr int TPW = DT / NW;
+    static_assert(TPW >= 1 && TPW * NW == DT, "DT must be a multiple of the warp count");
+    extern __shared__ __align__(128) uint8_t smem[];
+    const uint32_t bar = smem_u32(smem);
+    uint32_t* const s_var = reinterpret_cast<uint32_t*>(smem + kSmemCtrlBytes + 2 * kBlobBytes);
+    uint8_t* const s_rawb = reinterpret_cast<uint8_t*>(s_var + a.vcap_words);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     int bid = blockIdx.x;
@@ -145,6 +168,44 @@ __global__ void __launch_bounds__(kThreads, 1) dedisp_tiled_kernel(const TiledAr
     if (t0 >= a.nout[td.trial0]) return;  // nout is non-increasing in the trial index (delays grow with DM)
 
     const T* in = reinterpret_cast<const T*>(a.in) + (int64_t)beam * a.beam_stride;
+
+    // T: the elected warp arms the stage barrier with the byte count and issues the bulk copies
+    auto issue_stage = [&](int s) {
+        const StageIndex si = a.sidx[td.stage0 + s];
+        uint32_t bytes = 0;
+        for (uint32_t k = lane; k < si.nrows; k += 32) {
+            const RowDesc r = a.rows[si.row0 + k];
+            const int64_t room = a.row_stride - (t0 + r.astart);
+            const int64_t n = room < (int64_t)r.nelem ? (room > 0 ? room : 0) : (int64_t)r.nelem;
+            bytes += (uint32_t)n * (uint32_t)sizeof(T);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
+        if (lane == 0) {
+            fence_proxy_async();  // generic-proxy reads of the buffers (previous stage) before async-proxy writes
+            mbar_expect_tx(bar, bytes + si.blob_words * 4u);
+            bulk_g2s(smem_u32(smem + kSmemCtrlBytes + (s & 1) * kBlobBytes), a.blob + si.blob_word0, si.blob_words * 4u, bar);
+        }
+        __syncwarp();
+        for (uint32_t k = lane; k < si.nrows; k += 32) {
+            const RowDesc r = a.rows[si.row0 + k];
+            const int64_t pos = t0 + r.astart;
+            const int64_t room = a.row_stride - pos;
+            const int64_t n = room < (int64_t)r.nelem ? (room > 0 ? room : 0) : (int64_t)r.nelem;
+            if (n > 0)
+                bulk_g2s(smem_u32(s_rawb + r.soff), in + (int64_t)r.chan * a.row_stride + pos,
+                         (uint32_t)n * (uint32_t)sizeof(T), bar);
+        }
+    };
+
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        fence_proxy_async();
+    }
+    __syncthreads();
+    if (warp == 0) issue_stage(0);
+
     uint32_t acc[TPW][16];
 #pragma unroll
     for (int q = 0; q < TPW; ++q)
@@ -153,98 +214,68 @@ __global__ void __launch_bounds__(kThreads, 1) dedisp_tiled_kernel(const TiledAr
     bool first_flush = true;
 
     for (int s = 0; s < td.nstage; ++s) {
-        const StageDesc sd = a.stages[td.stage0 + s];
-        uint32_t* s_var = s_data;
-        uint32_t* s_exp = s_data + ((sd.vwords + 3) & ~3);
-        __syncthreads();  // everyone is done with the previous stage's tables and variants
-        // stage tables -> shared
+        mbar_wait(bar, (uint32_t)(s & 1));
+        const uint32_t* tb = reinterpret_cast<const uint32_t*>(smem + kSmemCtrlBytes + (s & 1) * kBlobBytes);
+        const int ngrp = (int)tb[0];
+        const bool flush = tb[1] != 0u;
+        const uint32_t* pairs = tb + kBlobHdrWords + 4 * ngrp;
+        const uint16_t* toff = reinterpret_cast<const uint16_t*>(pairs + tb[2]);
+
+        // ---- B: pre-sum every variant of every group ---------------------------------------------------------
         {
-            const uint32_t* gsrc = reinterpret_cast<const uint32_t*>(a.groups + sd.grp0);
-            uint32_t* gdst = reinterpret_cast<uint32_t*>(s_grp);
-            for (int i = tid; i < sd.ngrp * (int)(sizeof(GroupDesc) / 4); i += kThreads) gdst[i] = __ldg(gsrc + i);
-            const uint16_t* tsrc = a.trial_off + (int64_t)sd.grp0 * DT;
-            for (int i = tid; i < sd.ngrp * DT; i += kThreads) s_tab[i] = __ldg(tsrc + i);
-        }
-        // ---- A: expand raw samples into half-interleaved 16-bit words --------------------------------------
-        {
-            int idx = 0;
-            for (int g = 0; g < sd.ngrp; ++g) {
-              const GroupDesc gd = a.groups[sd.grp0 + g];
-              for (int j = 0; j < gd.nch; ++j, ++idx) {
-                if ((idx & (kThreads / 32 - 1)) != warp) continue;
-                const T* row = in + (int64_t)(gd.chan0 + j) * a.row_stride;
-                const int64_t p0 = t0 + gd.wlo;  // multiple of 4
-                uint32_t* E = s_exp + gd.ebase + j * gd.elen;
-                for (int e4 = lane; e4 < (gd.elen >> 2); e4 += 32) {
-                    const int64_t plo = p0 + 4 * e4, phi = plo + kH;
-                    uint4 w;
-                    if (sizeof(T) == 1) {
-                        const uint32_t lo = ld_word_or_zero(reinterpret_cast<const uint32_t*>(row + plo), plo < a.row_stride);
-                        const uint32_t hi = ld_word_or_zero(reinterpret_cast<const uint32_t*>(row + phi), phi < a.row_stride);
-                        const uint32_t lo_e = lo & 0x00FF00FFu, lo_o = __byte_perm(lo, 0u, 0x4341);
-                        const uint32_t hi_e = hi & 0x00FF00FFu, hi_o = __byte_perm(hi, 0u, 0x4341);
-                        w.x = __byte_perm(lo_e, hi_e, 0x5410);
-                        w.y = __byte_perm(lo_o, hi_o, 0x5410);
-                        w.z = __byte_perm(lo_e, hi_e, 0x7632);
-                        w.w = __byte_perm(lo_o, hi_o, 0x7632);
-                    } else {
-                        uint2 lo = make_uint2(0u, 0u), hi = make_uint2(0u, 0u);
-                        if (plo < a.row_stride) lo = __ldg(reinterpret_cast<const uint2*>(row + plo));
-                        if (phi < a.row_stride) hi = __ldg(reinterpret_cast<const uint2*>(row + phi));
-                        w.x = __byte_perm(lo.x, hi.x, 0x5410);
-                        w.y = __byte_perm(lo.x, hi.x, 0x7632);
-                        w.z = __byte_perm(lo.y, hi.y, 0x5410);
-                        w.w = __byte_perm(lo.y, hi.y, 0x7632);
-                    }
-                    *reinterpret_cast<uint4*>(E + 4 * e4) = w;
-                }
-              }
-            }
-        }
-        __syncthreads();
-        // ---- B: pre-sum every variant of every group -------------------------------------------------------
-        {
-            int idx = 0;
-            for (int g = 0; g < sd.ngrp; ++g) {
-                const GroupDesc gd = s_grp[g];
-                for (int r = 0; r < gd.nvar; ++r, ++idx) {
-                    if ((idx & (kThreads / 32 - 1)) != warp) continue;
-                    const int16_t* sh = a.var_shift + (int64_t)(gd.var0 + r) * kMaxG;
-                    const uint32_t* E0 = s_exp + gd.ebase;
-                    uint32_t* P = s_var + gd.vbase + r * gd.vlen;
-                    if (gd.nch == G) {
-                        const uint32_t* E[G];
+            int task = 0;
+            for (int g = 0; g < ngrp; ++g) {
+                const uint32_t* gh = tb + kBlobHdrWords + 4 * g;
+                const int vlen = (int)gh[1];
+                const int nchunk = (vlen + 63) >> 6;
+                for (int ch = 0; ch < nchunk; ++ch, ++task) {
+                    if ((task & (NW - 1)) != warp) continue;
+                    const int vbase = (int)gh[0], nvar = (int)gh[3];
+                    const uint32_t pair0 = gh[2] & 0xffffu, npairs = gh[2] >> 16;
+                    const int u0 = (ch << 6) + lane, u1 = u0 + 32;   // rows carry kRowSlack elements past vlen
+                    uint32_t av0[kMaxVar], av1[kMaxVar];
 #pragma unroll
-                        for (int j = 0; j < G; ++j) E[j] = E0 + j * gd.elen + (int)sh[j];
-                        for (int u = lane; u < gd.vlen; u += 32) {
-                            uint32_t sum = E[0][u];
+                    for (int r = 0; r < kMaxVar; ++r) { av0[r] = 0u; av1[r] = 0u; }
+                    uint32_t base0 = 0u, base1 = 0u, wb0 = 0u, wb1 = 0u;
+                    for (uint32_t q = 0; q < npairs; ++q) {
+                        const uint32_t d = pairs[pair0 + q];
+                        const T* row = reinterpret_cast<const T*>(s_rawb + (d & 0x1ffffu));
+                        const uint32_t w0 = __byte_perm((uint32_t)row[u0], (uint32_t)row[u0 + kH], 0x5410);
+                        const uint32_t w1 = __byte_perm((uint32_t)row[u1], (uint32_t)row[u1 + kH], 0x5410);
+                        if (d & kPairBaseBit) {
+                            wb0 = w0; wb1 = w1; base0 += w0; base1 += w1;
+                        } else {
+                            const uint32_t m = d >> 20, d0 = w0 - wb0, d1 = w1 - wb1;
 #pragma unroll
-                            for (int j = 1; j < G; ++j) sum += E[j][u];
-                            P[u] = sum;
-                        }
-                    } else {  // a group the plan had to shrink (few channels, many relative-delay vectors)
-                        for (int u = lane; u < gd.vlen; u += 32) {
-                            uint32_t sum = 0;
-                            for (int j = 0; j < gd.nch; ++j) sum += E0[j * gd.elen + (int)sh[j] + u];
-                            P[u] = sum;
+                            for (int r = 0; r < kMaxVar; ++r)
+                                if (m & (1u << r)) { av0[r] += d0; av1[r] += d1; }
                         }
                     }
+                    uint32_t* P = s_var + vbase;
+#pragma unroll
+                    for (int r = 0; r < kMaxVar; ++r)
+                        if (r < nvar) {
+                            if (u0 < vlen) P[r * vlen + u0] = base0 + av0[r];
+                            if (u1 < vlen) P[r * vlen + u1] = base1 + av1[r];
+                        }
                 }
             }
         }
-        __syncthreads();
+        __syncthreads();  // variants complete; raw rows and the other blob buffer are free
+        if (warp == 0 && s + 1 < td.nstage) issue_stage(s + 1);
+
         // ---- C: gather-accumulate ------------------------------------------------------------------------------
-        for (int g = 0; g < sd.ngrp; ++g) {
-            const uint16_t* to = s_tab + g * DT + warp * TPW;
+        for (int g = 0; g < ngrp; ++g) {
+            const uint16_t* to = toff + g * DT + warp * TPW;
 #pragma unroll
             for (int q = 0; q < TPW; ++q) {
-                const uint32_t* src = s_data + to[q] + lane;
+                const uint32_t* src = s_var + to[q] + lane;
 #pragma unroll
                 for (int j = 0; j < 16; ++j) acc[q][j] += src[32 * j];
             }
         }
         // ---- F: widen the 16-bit lanes into the int32 DM transform -------------------------------------------
-        if (sd.flush) {
+        if (flush) {
 #pragma unroll
             for (int q = 0; q < TPW; ++q) {
                 const int dl = warp * TPW + q;
@@ -265,38 +296,33 @@ __global__ void __launch_bounds__(kThreads, 1) dedisp_tiled_kernel(const TiledAr
             }
             first_flush = false;
         }
+        __syncthreads();  // everyone is done with this stage's variants
     }
 }
 
-template <typename T, int DT, int G>
+template <typename T, int DT>
 static int launch_tiled_inst(const TiledArgs& a, cudaStream_t st) {
     static bool attr_set = false;
-    auto kern = dedisp_tiled_kernel<T, DT, G>;
-    const int smem_bytes = kSmemWords * 4;
+    auto kern = dedisp_tiled_kernel<T, DT>;
     if (!attr_set) {
-        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes) != cudaSuccess) return -1;
+        if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes) != cudaSuccess) return -1;
         attr_set = true;
     }
     const int64_t nblocks = (int64_t)a.ntile_dm * a.ntile_t * a.nbeam;
     if (nblocks <= 0) return 0;
     if (nblocks > 0x7fffffffLL) return -1;
-    kern<<<(unsigned)nblocks, kThreads, smem_bytes, st>>>(a);
+    kern<<<(unsigned)nblocks, kThreads, kSmemBytes, st>>>(a);
     return 0;
 }
 
-int launch_dedisp_tiled(bool is_u16, int DT, int G, const void* in, int64_t row_stride, int64_t beam_stride,
-                        int32_t* out, int64_t out_beam_stride, const TileDesc* tiles, const StageDesc* stages,
-                        const GroupDesc* groups, const int16_t* var_shift, const uint16_t* trial_off,
-                        const int32_t* nout, const int64_t* offset, int32_t ntile_dm, int32_t ntile_t, int32_t nbeam,
-                        cudaStream_t st) {
-    TiledArgs a{in, row_stride, beam_stride, out, out_beam_stride, tiles, stages, groups, var_shift, trial_off,
-                nout, offset, ntile_dm, ntile_t, nbeam};
-#define SPT_CASE(DT_, G_)                                                              \
-    if (DT == DT_ && G == G_)                                                          \
-        return is_u16 ? launch_tiled_inst<uint16_t, DT_, G_>(a, st) : launch_tiled_inst<uint8_t, DT_, G_>(a, st);
-    SPT_CASE(64, 1) SPT_CASE(64, 2) SPT_CASE(64, 4) SPT_CASE(64, 8)
-    SPT_CASE(32, 1) SPT_CASE(32, 2) SPT_CASE(32, 4) SPT_CASE(32, 8)
-#undef SPT_CASE
+int launch_dedisp_tiled(bool is_u16, int DT, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
+                        int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
+                        const uint32_t* blob, int32_t vcap_words, const int32_t* nout, const int64_t* offset,
+                        int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, cudaStream_t st) {
+    TiledArgs a{in, row_stride, beam_stride, out, out_beam_stride, tiles, sidx, rows, blob, nout, offset,
+                vcap_words, ntile_dm, ntile_t, nbeam};
+    if (DT == 64) return is_u16 ? launch_tiled_inst<uint16_t, 64>(a, st) : launch_tiled_inst<uint8_t, 64>(a, st);
+    if (DT == 32) return is_u16 ? launch_tiled_inst<uint16_t, 32>(a, st) : launch_tiled_inst<uint8_t, 32>(a, st);
     return -1;
 }
 

@@ -24,34 +24,37 @@ constexpr int kH = 512;              // words per trial per tile
 constexpr int kTT = 2 * kH;          // output samples per tile
 constexpr int kThreads = 512;        // 16 warps
 constexpr int kMaxG = 8;             // channels per pre-summed group
-constexpr int kSmemWords = 56 * 1024;  // 224 KB of the 227 KB a block may opt in to
-constexpr int kMaxStageGroups = 32;  // groups per stage (bounds the per-stage tables kept in shared memory)
+constexpr int kMaxVar = 12;          // variants per group (bits of a pair mask)
 constexpr int kMaxDT = 64;           // trials per DM tile
-constexpr int kTabWords = kMaxStageGroups * kMaxDT / 2;                 // trial_off slice of a stage (uint16)
-constexpr int kDescWords = kMaxStageGroups * 10;                        // GroupDesc slice of a stage
-constexpr int kStageDataWords = kSmemWords - kTabWords - kDescWords;    // variants + expansion rows
+constexpr int kMaxStageGroups = 16;  // groups per stage
+constexpr int kBlobBytes = 4096;     // per-stage table blob (two buffers in shared memory)
+constexpr int kSmemBytes = 227 * 1024;                                   // what a block may opt in to on sm_100
+constexpr int kSmemCtrlBytes = 64;                                       // mbarrier + padding
+constexpr int kSmemDataBytes = kSmemBytes - kSmemCtrlBytes - 2 * kBlobBytes;  // variant region + raw-row region
+constexpr int kRowSlack = 64;        // elements readable past the last needed one of every raw row (presum tail)
 
-struct GroupDesc {          // one channel group of one (DM tile, stage); 40 bytes
-    int32_t chan0;          // first channel
-    int32_t nch;            // channels in the group (<= G; the last group of a band may be short)
-    int32_t wlo;            // window start relative to the tile's t0, in samples, multiple of 4
-    int32_t elen;           // words of each expanded channel row E_j[0 .. elen), multiple of 4
-    int32_t vlen;           // words of each variant row P_r[0 .. vlen)
-    int32_t nvar;           // variants R
-    int32_t var0;           // index of the first variant's shift list in var_shift (x kMaxG)
-    int32_t vbase;          // word offset of P_0 inside the stage's variant region
-    int32_t ebase;          // word offset of E_0 inside the stage's expansion region (multiple of 4)
-    int32_t pad_;
+// Per-stage blob, 32-bit words (copied to shared memory with one bulk copy):
+//   [0] ngrp  [1] flush  [2] npairs (all groups)  [3] reserved
+//   [4 ..)                 ngrp x { vbase, vlen, pair0 | npairs << 16, nvar }
+//   [4 + 4*ngrp ..)        pair descriptors: bits 0-16 byte offset of (row start + shift) inside the raw region,
+//                          bit 17 = base pair (taken by every variant unless a later delta pair of the same channel
+//                          claims it), bits 20-31 = mask of the variants that take this (delta) pair
+//   [.. ]                  trial_off: ngrp x DT uint16 = word offset of the trial's read start in the variant region
+constexpr int kBlobHdrWords = 4;
+constexpr uint32_t kPairBaseBit = 1u << 17;
+
+struct RowDesc {            // one raw channel row of a stage; 16 bytes
+    int32_t chan;
+    int32_t astart;         // first element copied, relative to the tile's t0 (multiple of 16)
+    int32_t nelem;          // elements to copy (multiple of 16)
+    int32_t soff;           // byte offset inside the raw region (multiple of 16)
 };
 
-struct StageDesc {          // 32 bytes
-    int32_t grp0;           // first GroupDesc
-    int32_t ngrp;
-    int32_t vwords;         // words of the variant region used by this stage
-    int32_t ewords;         // words of the expansion region used by this stage
-    int32_t flush;          // 1: packed accumulators must be flushed to int32 after this stage
-    int32_t nvar;           // variants over all groups of the stage
-    int32_t pad_[2];
+struct StageIndex {         // 16 bytes
+    uint32_t blob_word0;    // first word of the stage's blob
+    uint32_t blob_words;    // multiple of 4
+    uint32_t row0;          // first RowDesc
+    uint32_t nrows;
 };
 
 struct TileDesc {           // one DM tile of a range
@@ -73,11 +76,12 @@ struct RangePlan {
 
     // tiled-kernel tables (host copies; built by build_tiling)
     std::vector<TileDesc> tiles;
-    std::vector<StageDesc> stages;
-    std::vector<GroupDesc> groups;
-    std::vector<int16_t> var_shift;  // [nvariants][kMaxG] shift (>= 0) of channel j of variant r inside its E row
-    std::vector<uint16_t> trial_off; // [groups.size()][DT] word offset of trial's read start inside the variant region
+    std::vector<StageIndex> sidx;
+    std::vector<RowDesc> rows;
+    std::vector<uint32_t> blob;
+    int32_t vcap_words = 0;          // words of the variant region; the raw region follows it
     int32_t ntile_t = 0;             // time tiles
+    int64_t ngroups = 0, nvariants = 0, npairs = 0;   // totals, for reports
 };
 
 struct DeviceState;  // defined in api.cu

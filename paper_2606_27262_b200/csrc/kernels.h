@@ -16,11 +16,10 @@ void launch_dedisp_naive(const T* y, int64_t row_stride, int64_t beam_stride, co
                          const int32_t* d_nout, const int64_t* d_offset, int32_t nchan, int32_t ndm, int32_t nbeam,
                          int32_t max_nout, int32_t* out, int64_t out_beam_stride, cudaStream_t st);
 
-int launch_dedisp_tiled(bool is_u16, int DT, int G, const void* in, int64_t row_stride, int64_t beam_stride,
-                        int32_t* out, int64_t out_beam_stride, const TileDesc* tiles, const StageDesc* stages,
-                        const GroupDesc* groups, const int16_t* var_shift, const uint16_t* trial_off,
-                        const int32_t* nout, const int64_t* offset, int32_t ntile_dm, int32_t ntile_t, int32_t nbeam,
-                        cudaStream_t st);
+int launch_dedisp_tiled(bool is_u16, int DT, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
+                        int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
+                        const uint32_t* blob, int32_t vcap_words, const int32_t* nout, const int64_t* offset,
+                        int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, cudaStream_t st);
 
 struct SpsArgs {
     const int32_t* dmt;

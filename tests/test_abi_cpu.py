@@ -102,7 +102,7 @@ def test_tiling_tables_reproduce_the_delay_table(api, synth, group, dm_tile):
             assert np.array_equal(p.tiling_delays(d), p.delays(d)), (cfg, d)
         for r in range(len(w.ranges)):
             info = p.tiling_info(r)
-            assert info["max_stage_words"] <= 56 * 1024
+            assert info["max_stage_words"] <= 227 * 1024 // 4
             assert info["ngroups"] >= info["ntiles_dm"] * ((w.nchan + group - 1) // group)
 
 
