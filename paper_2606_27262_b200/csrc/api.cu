@@ -383,7 +383,8 @@ int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int6
         for (const StageIndex& si : rp.sidx) {
             const uint32_t* b = &rp.blob[si.blob_word0];
             int64_t v = 0, r = 0;
-            for (uint32_t k = 0; k < b[0]; ++k) v += (int64_t)b[kBlobHdrWords + 4 * k + 1] * b[kBlobHdrWords + 4 * k + 3];
+            for (uint32_t k = 0; k < b[0]; ++k)
+                v += (int64_t)b[kBlobHdrWords + 4 * k + 1] * (b[kBlobHdrWords + 4 * k + 2] >> 8);
             for (uint32_t k = 0; k < si.nrows; ++k) r += (int64_t)rp.rows[si.row0 + k].nelem * es;
             if (v > rp.vcap_words || r > kSmemDataBytes - (int64_t)rp.vcap_words * 4) return SPT_ERR_STATE;
             m = std::max(m, v + r / 4);
@@ -410,36 +411,39 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
         const StageIndex& si = rp->sidx[s];
         const uint32_t* b = &rp->blob[si.blob_word0];
         const uint32_t ngrp = b[0];
-        const uint32_t* pairs = b + kBlobHdrWords + 4 * ngrp;
-        const uint32_t* toff = pairs + b[2];
+        const uint16_t* toff = reinterpret_cast<const uint16_t*>(b + b[3]);
         for (uint32_t g = 0; g < ngrp; ++g) {
             const uint32_t* gh = b + kBlobHdrWords + 4 * g;
-            const int32_t vbase = (int32_t)gh[0], vlen = (int32_t)gh[1], nvar = (int32_t)gh[3];
-            const uint32_t pair0 = gh[2] & 0xffffu, npairs = gh[2] >> 16;
-            const uint32_t tw = toff[(g * DT + dl) / 2];
-            const int32_t to = (int32_t)(((g * DT + dl) & 1) ? (tw >> 16) : (tw & 0xffffu));
+            const int32_t vbase = (int32_t)gh[0], vlen = (int32_t)gh[1];
+            const int32_t nch = (int32_t)(gh[2] & 0xffu), nvar = (int32_t)(gh[2] >> 8);
+            const uint32_t* cd = b + (gh[3] & 0xffffu);
+            const uint32_t* vd = b + (gh[3] >> 16);
+            const int32_t to = (int32_t)toff[g * DT + dl];
             const int32_t rel = to - vbase, r = rel / vlen, bb = rel - r * vlen;
-            if (r < 0 || r >= nvar) return SPT_ERR_STATE;
-            // the gather reads P_r[q + bb]; P_r[u] sums, per channel, the pair the variant takes: the base pair unless a
-            // delta pair of the same row has bit r set; a pair at byte offset `off` of row (soff, astart) is element
-            // t0 + astart + (off - soff)/es + u of that channel
-            int32_t cur_chan = -1;
-            for (uint32_t q = 0; q < npairs; ++q) {
-                const uint32_t d = pairs[pair0 + q];
-                const int32_t off = (int32_t)(d & 0x1ffffu);
-                const RowDesc* row = nullptr;
-                for (uint32_t k = 0; k < si.nrows; ++k) {
-                    const RowDesc& rr = rp->rows[si.row0 + k];
-                    if (off >= rr.soff && off < rr.soff + rr.nelem * es) { row = &rr; break; }
+            if (r < 0 || r >= nvar || (int32_t)vd[2 * r] != vbase + r * vlen) return SPT_ERR_STATE;
+            // the gather reads P_r[q + bb]; P_r[u] takes, of the channel at position q of the prefix order, the sample
+            // at its base shift + u, or one later when the variant has it on the alternate shift
+            const uint32_t k = vd[2 * r + 1] & 0xffu, plus = (vd[2 * r + 1] >> 8) & 0xffu, minus = vd[2 * r + 1] >> 16;
+            for (int pass = 0; pass < 2; ++pass)       // pass 0: base shifts; pass 1: one sample later per delta taken
+                for (int32_t q = 0; q < nch; ++q) {
+                    const int32_t byte = (int32_t)((cd[q] & 0xffffffu) * 4u) +
+                                         (es == 1 ? (int32_t)((cd[q] >> 24) & 3u) : 2 * (int32_t)((cd[q] >> 24) & 3u));
+                    const RowDesc* row = nullptr;
+                    for (uint32_t i = 0; i < si.nrows; ++i) {
+                        const RowDesc& rr = rp->rows[si.row0 + i];
+                        if (byte >= rr.soff && byte < rr.soff + rr.nelem * es) { row = &rr; break; }
+                    }
+                    if (!row) return SPT_ERR_STATE;
+                    const bool taken = (((uint32_t)q < k) && !((minus >> q) & 1u)) || ((plus >> q) & 1u);
+                    if (pass == 0 && (cd[q] & kEntryAddBase)) {
+                        if (host_out[row->chan] != INT32_MIN) return SPT_ERR_STATE;   // every channel exactly once
+                        host_out[row->chan] = row->astart + (byte - row->soff) / es + bb;
+                    }
+                    if (pass == 1 && taken) {
+                        if (host_out[row->chan] == INT32_MIN) return SPT_ERR_STATE;
+                        host_out[row->chan] += 1;
+                    }
                 }
-                if (!row) return SPT_ERR_STATE;
-                const int32_t dly = row->astart + (off - row->soff) / es + bb;
-                if (d & kPairBaseBit) { cur_chan = row->chan; host_out[cur_chan] = dly; }
-                else {
-                    if (row->chan != cur_chan) return SPT_ERR_STATE;
-                    if ((d >> 20) & (1u << r)) host_out[cur_chan] = dly;
-                }
-            }
         }
     }
     return SPT_OK;

@@ -97,17 +97,18 @@ template void launch_dedisp_naive<uint16_t>(const uint16_t*, int64_t, int64_t, c
                                             cudaStream_t);
 
 // ---------------------------------------------------------------------------------------------------------------
-// a3, the product kernel.  One block = DT trials x TT = 2*kH output samples of one beam; 16 warps, TPW = DT/16
-// trials per warp; lane l of a warp owns the packed words q = l + 32*j (j < 16) of each of its trials: the low
-// 16 bits of word q accumulate output t0+q, the high 16 bits output t0+kH+q.  Because both halves of a word
-// move together, a read at ANY sample offset is one aligned 32-bit shared-memory load (no byte realignment).
+// a3, the product kernel.  One block = DT trials x TT = 2*kH output samples of one beam; 8 warps, TPW = DT/8 trials
+// per warp, two blocks per SM; lane l of a warp owns the packed words q = l + 32*j (j < kH/32) of each of its
+// trials: the low 16 bits of word q accumulate output t0+q, the high 16 bits output t0+kH+q.  Because both halves
+// of a word move together, a read at ANY sample offset is one aligned 32-bit shared-memory load.
 //
 // Per stage (a run of channel groups that fits shared memory; tables built by plan.cpp):
 //   T  TMA    : one elected warp issues cp.async.bulk copies of the stage's table blob and raw channel rows
 //               (global -> shared, completion on an mbarrier); they land while the previous stage is gathered
-//   B  presum : P_r[u] = sum_j y[c0+j][t0 + dmin + u + rho^r_j] | (same at +kH) << 16 for every variant r of every
-//               group, in one sweep over the group's (channel, shift) pairs: base pairs go to all variants, delta
-//               pairs replace the base for the variants in their mask (predicated adds)
+//   B  presum : P_r[u] = sum_j y[c0+j][t0 + dmin + u + s_j + tau^r_j] | (same at +kH) << 16 for every variant r of
+//               every group.  A lane makes 4 consecutive u from aligned 32-bit words of the raw rows: per channel the
+//               five samples u..u+4 as packed words w0..w4, base += w_i, delta_i = w_{i+1} - w_i (the alternate shift
+//               is one sample later), then walks the prefix chain: variant k = base + delta of the first k channels.
 //   C  gather : acc[d][q] += P_{r(d)}[q + b(d)]       one LDS.32 + one add = 2*G algorithmic adds
 //   F  flush  : every <= 257/decim channels the 16-bit lanes are widened into the int32 DM transform (L2 RMW).
 // ---------------------------------------------------------------------------------------------------------------
@@ -148,10 +149,100 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
+// The five packed words w_i = y[u0+i] | y[u0+i+kH] << 16, i = 0..4, of one channel at its base shift.
+// cd: bits 0-23 word index (raw region) of the word holding the u = 0 sample, bits 24-25 its position in the word.
+template <typename T>
+__device__ __forceinline__ void load_channel(const uint32_t* __restrict__ s_raw, uint32_t cd, int u0, uint32_t (&w)[5]) {
+    const uint32_t a0 = (cd >> 24) & 3u;
+    if (sizeof(T) == 1) {
+        const uint32_t* pw = s_raw + (cd & 0xffffffu) + (u0 >> 2);
+        const uint32_t aL = pw[0], bL = pw[1], aH = pw[kH / 4], bH = pw[kH / 4 + 1];
+        const uint32_t sh = a0 * 8u;
+        const uint32_t Lw = __funnelshift_r(aL, bL, sh), Hw = __funnelshift_r(aH, bH, sh);   // samples 0..3
+        const uint32_t Le = Lw & 0x00FF00FFu, Lo = __byte_perm(Lw, 0u, 0x4341);
+        const uint32_t He = Hw & 0x00FF00FFu, Ho = __byte_perm(Hw, 0u, 0x4341);
+        w[0] = __byte_perm(Le, He, 0x5410);
+        w[1] = __byte_perm(Lo, Ho, 0x5410);
+        w[2] = __byte_perm(Le, He, 0x7632);
+        w[3] = __byte_perm(Lo, Ho, 0x7632);
+        const uint32_t sel = a0 | (a0 << 4) | ((a0 + 4u) << 8) | ((a0 + 4u) << 12);         // sample 4 = byte a0 of b
+        w[4] = __byte_perm(bL, bH, sel) & 0x00FF00FFu;
+    } else {
+        const uint32_t* pw = s_raw + (cd & 0xffffffu) + (u0 >> 1);
+        const uint32_t x0L = pw[0], x1L = pw[1], x2L = pw[2];
+        const uint32_t x0H = pw[kH / 2], x1H = pw[kH / 2 + 1], x2H = pw[kH / 2 + 2];
+        if (a0 == 0u) {
+            w[0] = __byte_perm(x0L, x0H, 0x5410); w[1] = __byte_perm(x0L, x0H, 0x7632);
+            w[2] = __byte_perm(x1L, x1H, 0x5410); w[3] = __byte_perm(x1L, x1H, 0x7632);
+            w[4] = __byte_perm(x2L, x2H, 0x5410);
+        } else {
+            w[0] = __byte_perm(x0L, x0H, 0x7632); w[1] = __byte_perm(x1L, x1H, 0x5410);
+            w[2] = __byte_perm(x1L, x1H, 0x7632); w[3] = __byte_perm(x2L, x2H, 0x5410);
+            w[4] = __byte_perm(x2L, x2H, 0x7632);
+        }
+    }
+}
+
+// B: one warp task = kChunkU variant words (4 per lane) of every variant of one group.
+template <typename T>
+__device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uint32_t task, uint32_t* __restrict__ s_var,
+                                            const uint32_t* __restrict__ s_raw, int lane) {
+    const uint32_t* gh = tb + kBlobHdrWords + 4 * (task & 0xffu);
+    const int vlen = (int)gh[1];
+    const int u0 = (int)(task >> 8) * kChunkU + lane * 4;
+    if (u0 >= vlen) return;                       // vlen is a multiple of 4; no warp-wide operation below
+    const int nch = (int)(gh[2] & 0xffu);
+    const uint32_t* cd = tb + (gh[3] & 0xffffu);
+    const uint32_t* vd = tb + (gh[3] >> 16);
+    uint32_t cur[4] = {0u, 0u, 0u, 0u};
+    uint32_t dl[kMaxG][4];
+#pragma unroll
+    for (int q = 0; q < kMaxG; ++q) {
+        if (q < nch) {
+            uint32_t w[5];
+            load_channel<T>(s_raw, cd[q], u0, w);
+#pragma unroll
+            for (int i = 0; i < 4; ++i) dl[q][i] = w[i + 1] - w[i];
+            if (cd[q] & kEntryAddBase) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) cur[i] += w[i];
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) dl[q][i] = 0u;
+        }
+    }
+    // prefix chain: after step k, cur = all channels at their base shift except the first k of the order
+    uint32_t dst = vd[0], code = vd[1];
+#pragma unroll
+    for (int k = 0; k <= kMaxG; ++k) {
+        if (k > 0) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) cur[i] += dl[k - 1][i];
+        }
+        while ((code & 0xffu) == (uint32_t)k) {
+            uint4 o = make_uint4(cur[0], cur[1], cur[2], cur[3]);
+            const uint32_t fix = code >> 8;
+            if (fix != 0u) {                      // a variant off the chain (rare)
+#pragma unroll
+                for (int q = 0; q < kMaxG; ++q) {
+                    if (fix & (1u << q)) { o.x += dl[q][0]; o.y += dl[q][1]; o.z += dl[q][2]; o.w += dl[q][3]; }
+                    if (fix & (0x100u << q)) { o.x -= dl[q][0]; o.y -= dl[q][1]; o.z -= dl[q][2]; o.w -= dl[q][3]; }
+                }
+            }
+            *reinterpret_cast<uint4*>(s_var + dst + u0) = o;
+            vd += 2;
+            dst = vd[0]; code = vd[1];
+        }
+        if ((code & 0xffu) == 255u) break;        // the sentinel entry
+    }
+}
+
 template <typename T, int DT>
-__global__ void __launch_bounds__(kThreads, 1) dedisp_tiled_kernel(const TiledArgs a) {
+__global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledArgs a) {
     constexpr int NW = kThreads / 32;
     constexpr int TPW = DT / NW;
+    constexpr int NJ = kH / 32;
     static_assert(TPW >= 1 && TPW * NW == DT, "DT must be a multiple of the warp count");
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t bar = smem_u32(smem);
@@ -206,11 +297,11 @@ __global__ void __launch_bounds__(kThreads, 1) dedisp_tiled_kernel(const TiledAr
     __syncthreads();
     if (warp == 0) issue_stage(0);
 
-    uint32_t acc[TPW][16];
+    uint32_t acc[TPW][NJ];
 #pragma unroll
     for (int q = 0; q < TPW; ++q)
 #pragma unroll
-        for (int j = 0; j < 16; ++j) acc[q][j] = 0u;
+        for (int j = 0; j < NJ; ++j) acc[q][j] = 0u;
     bool first_flush = true;
 
     for (int s = 0; s < td.nstage; ++s) {
@@ -218,49 +309,12 @@ __global__ void __launch_bounds__(kThreads, 1) dedisp_tiled_kernel(const TiledAr
         const uint32_t* tb = reinterpret_cast<const uint32_t*>(smem + kSmemCtrlBytes + (s & 1) * kBlobBytes);
         const int ngrp = (int)tb[0];
         const bool flush = tb[1] != 0u;
-        const uint32_t* pairs = tb + kBlobHdrWords + 4 * ngrp;
-        const uint16_t* toff = reinterpret_cast<const uint16_t*>(pairs + tb[2]);
+        const int ntask = (int)tb[2];
+        const uint16_t* toff = reinterpret_cast<const uint16_t*>(tb + tb[3]);
 
         // ---- B: pre-sum every variant of every group ---------------------------------------------------------
-        {
-            int task = 0;
-            for (int g = 0; g < ngrp; ++g) {
-                const uint32_t* gh = tb + kBlobHdrWords + 4 * g;
-                const int vlen = (int)gh[1];
-                const int nchunk = (vlen + 63) >> 6;
-                for (int ch = 0; ch < nchunk; ++ch, ++task) {
-                    if ((task & (NW - 1)) != warp) continue;
-                    const int vbase = (int)gh[0], nvar = (int)gh[3];
-                    const uint32_t pair0 = gh[2] & 0xffffu, npairs = gh[2] >> 16;
-                    const int u0 = (ch << 6) + lane, u1 = u0 + 32;   // rows carry kRowSlack elements past vlen
-                    uint32_t av0[kMaxVar], av1[kMaxVar];
-#pragma unroll
-                    for (int r = 0; r < kMaxVar; ++r) { av0[r] = 0u; av1[r] = 0u; }
-                    uint32_t base0 = 0u, base1 = 0u, wb0 = 0u, wb1 = 0u;
-                    for (uint32_t q = 0; q < npairs; ++q) {
-                        const uint32_t d = pairs[pair0 + q];
-                        const T* row = reinterpret_cast<const T*>(s_rawb + (d & 0x1ffffu));
-                        const uint32_t w0 = __byte_perm((uint32_t)row[u0], (uint32_t)row[u0 + kH], 0x5410);
-                        const uint32_t w1 = __byte_perm((uint32_t)row[u1], (uint32_t)row[u1 + kH], 0x5410);
-                        if (d & kPairBaseBit) {
-                            wb0 = w0; wb1 = w1; base0 += w0; base1 += w1;
-                        } else {
-                            const uint32_t m = d >> 20, d0 = w0 - wb0, d1 = w1 - wb1;
-#pragma unroll
-                            for (int r = 0; r < kMaxVar; ++r)
-                                if (m & (1u << r)) { av0[r] += d0; av1[r] += d1; }
-                        }
-                    }
-                    uint32_t* P = s_var + vbase;
-#pragma unroll
-                    for (int r = 0; r < kMaxVar; ++r)
-                        if (r < nvar) {
-                            if (u0 < vlen) P[r * vlen + u0] = base0 + av0[r];
-                            if (u1 < vlen) P[r * vlen + u1] = base1 + av1[r];
-                        }
-                }
-            }
-        }
+        for (int tk = warp; tk < ntask; tk += NW)
+            presum_task<T>(tb, tb[kBlobHdrWords + 4 * ngrp + tk], s_var, reinterpret_cast<const uint32_t*>(s_rawb), lane);
         __syncthreads();  // variants complete; raw rows and the other blob buffer are free
         if (warp == 0 && s + 1 < td.nstage) issue_stage(s + 1);
 
@@ -271,7 +325,7 @@ __global__ void __launch_bounds__(kThreads, 1) dedisp_tiled_kernel(const TiledAr
             for (int q = 0; q < TPW; ++q) {
                 const uint32_t* src = s_var + to[q] + lane;
 #pragma unroll
-                for (int j = 0; j < 16; ++j) acc[q][j] += src[32 * j];
+                for (int j = 0; j < NJ; ++j) acc[q][j] += src[32 * j];
             }
         }
         // ---- F: widen the 16-bit lanes into the int32 DM transform -------------------------------------------
@@ -284,7 +338,7 @@ __global__ void __launch_bounds__(kThreads, 1) dedisp_tiled_kernel(const TiledAr
                     const int64_t n = a.nout[d];
                     int32_t* row = a.out + (int64_t)beam * a.out_beam_stride + a.offset[d] + t0;
 #pragma unroll
-                    for (int j = 0; j < 16; ++j) {
+                    for (int j = 0; j < NJ; ++j) {
                         const int i = lane + 32 * j;
                         const int32_t lo = (int32_t)(acc[q][j] & 0xFFFFu), hi = (int32_t)(acc[q][j] >> 16);
                         if (t0 + i < n) row[i] = first_flush ? lo : row[i] + lo;
@@ -292,7 +346,7 @@ __global__ void __launch_bounds__(kThreads, 1) dedisp_tiled_kernel(const TiledAr
                     }
                 }
 #pragma unroll
-                for (int j = 0; j < 16; ++j) acc[q][j] = 0u;
+                for (int j = 0; j < NJ; ++j) acc[q][j] = 0u;
             }
             first_flush = false;
         }

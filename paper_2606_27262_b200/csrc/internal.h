@@ -17,31 +17,38 @@ constexpr double kDispersionConstantS = 4.148808e3;
 constexpr int kRowAlignElems = 32;  // DM-transform rows start 128-byte aligned
 constexpr int kMaxWidths = 32;
 
-// ---- tiled dedispersion kernel geometry ---------------------------------------------
-// A block owns DT trials x TT = 2*H output samples.  Packed 16-bit accumulator word q of a trial holds the
-// outputs t0+q (low half) and t0+H+q (high half).
-constexpr int kH = 512;              // words per trial per tile
+// ---- tiled dedispersion kernel geometry ------------------------------------------------
+// A block owns DT trials x TT = 2*H output samples; two blocks are resident per SM.  Packed 16-bit accumulator
+// word q of a trial holds the outputs t0+q (low half) and t0+H+q (high half).
+constexpr int kH = 256;              // words per trial per tile
 constexpr int kTT = 2 * kH;          // output samples per tile
-constexpr int kThreads = 512;        // 16 warps
+constexpr int kThreads = 256;        // 8 warps
 constexpr int kMaxG = 8;             // channels per pre-summed group
-constexpr int kMaxVar = 12;          // variants per group (bits of a pair mask)
+constexpr int kMaxVar = 16;          // variants per group
 constexpr int kMaxDT = 64;           // trials per DM tile
-constexpr int kMaxStageGroups = 16;  // groups per stage
-constexpr int kBlobBytes = 4096;     // per-stage table blob (two buffers in shared memory)
-constexpr int kSmemBytes = 227 * 1024;                                   // what a block may opt in to on sm_100
+constexpr int kMaxStageGroups = 8;   // groups per stage
+constexpr int kChunkU = 128;         // variant words one warp builds per pre-sum task (4 per lane)
+constexpr int kBlobBytes = 3072;     // per-stage table blob (two buffers in shared memory)
+constexpr int kSmemBytes = 113 * 1024;                                   // two blocks per SM (228 KB incl. 1 KB each reserved)
 constexpr int kSmemCtrlBytes = 64;                                       // mbarrier + padding
 constexpr int kSmemDataBytes = kSmemBytes - kSmemCtrlBytes - 2 * kBlobBytes;  // variant region + raw-row region
-constexpr int kRowSlack = 64;        // elements readable past the last needed one of every raw row (presum tail)
 
 // Per-stage blob, 32-bit words (copied to shared memory with one bulk copy):
-//   [0] ngrp  [1] flush  [2] npairs (all groups)  [3] reserved
-//   [4 ..)                 ngrp x { vbase, vlen, pair0 | npairs << 16, nvar }
-//   [4 + 4*ngrp ..)        pair descriptors: bits 0-16 byte offset of (row start + shift) inside the raw region,
-//                          bit 17 = base pair (taken by every variant unless a later delta pair of the same channel
-//                          claims it), bits 20-31 = mask of the variants that take this (delta) pair
-//   [.. ]                  trial_off: ngrp x DT uint16 = word offset of the trial's read start in the variant region
+//   [0] ngrp  [1] flush  [2] ntask  [3] word offset of the trial_off table
+//   [4 ..)        ngrp x { vbase, vlen, nent | nvar << 8, cdesc_off | vdesc_off << 16 }      (offsets inside the blob)
+//   task table    ntask x { group | chunk << 8 }: warp task = kChunkU variant words of every variant of one group
+//   cdesc         per group, nent <= kMaxG entries in PREFIX ORDER (most-often-taken delta first); an entry is a channel
+//                 at one of its shifts: bits 0-23 word index inside the raw region of the 32-bit word that holds the
+//                 entry's sample at u = 0, bits 24-25 position of that sample inside the word, bit 26 = the entry is
+//                 the channel's smallest shift and adds it to the base sum.  The entry's delta (sample one later
+//                 minus sample) moves its channel one sample later.
+//   vdesc         per group, nvar + 1 entries of 2 words, sorted by k: { word offset of the variant in the variant
+//                 region, k | plus << 8 | minus << 16 }: the variant is the base sum plus the deltas of the first k
+//                 entries, corrected by the entries in plus (delta taken too) and minus (not taken after all); the
+//                 extra entry has k = 255
+//   trial_off     ngrp x DT uint16 = word offset of the trial's read start in the variant region
 constexpr int kBlobHdrWords = 4;
-constexpr uint32_t kPairBaseBit = 1u << 17;
+constexpr uint32_t kEntryAddBase = 1u << 26;
 
 struct RowDesc {            // one raw channel row of a stage; 16 bytes
     int32_t chan;
@@ -81,7 +88,7 @@ struct RangePlan {
     std::vector<uint32_t> blob;
     int32_t vcap_words = 0;          // words of the variant region; the raw region follows it
     int32_t ntile_t = 0;             // time tiles
-    int64_t ngroups = 0, nvariants = 0, npairs = 0;   // totals, for reports
+    int64_t ngroups = 0, nvariants = 0, ncorrected = 0;   // totals, for reports (ncorrected: variants off the prefix chain)
 };
 
 struct DeviceState;  // defined in api.cu
@@ -98,7 +105,7 @@ struct Plan {
     int64_t dmt_elems = 0;           // per beam
     // options
     int32_t opt_kernel = 0;          // 0 tiled, 1 naive
-    int32_t opt_group = 4;
+    int32_t opt_group = 8;
     int32_t opt_dm_tile = 64;
     int32_t opt_profile = 0;
     bool tiling_built = false;

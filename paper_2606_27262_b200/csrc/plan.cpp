@@ -73,31 +73,45 @@ const RangePlan* range_of_trial(const Plan& p, int32_t trial, int32_t* local) {
 }
 
 // -------------------------------------------------------------------------------------------------------------
-// Factorisation of the delay table for the tiled kernel.
+// Factorisation of the delay table for the tiled kernel (DESIGN.md section 5.3).
 //
-// For a DM tile (DT consecutive trials) and a group of G adjacent channels c0..c0+G-1 write
-//     delay[d][c0+j] = dmin + b(d) + rho_j(d),      dmin = min_d delay[d][c0],  b(d) >= 0,  rho_0 = 0.
-// Over the DT trials the vector rho(d) takes only a handful of distinct values ("variants": each rho_j toggles
-// between floor and ceil of the slowly varying true relative delay), so
-//     out[d][t] = sum_groups P_{r(d)}[ t - t0 + b(d) ],     P_r[u] = sum_j y[c0+j][t0 + dmin + u + rho^r_j]
-// is the SAME integer sum as the definition, with every P_r built once per tile and shared by the trials.
-// The kernel builds all P_r of a group in one sweep over the (channel, shift) pairs the variants use: the most
-// used shift of a channel is its "base" pair (added for every variant), every other shift a "delta" pair that
-// replaces the base for the variants in its mask.
+// For a DM tile (DT consecutive trials) and a group of up to 8 adjacent channels c0..c0+n-1 write
+//     delay[d][c0+j] = dmin + b(d) + s_j + tau_j(d),      dmin = min_d delay[d][c0],  b(d) >= 0,  s_0 = tau_0 = 0,
+// where s_j is the smallest delay of channel j relative to channel c0 over the tile and tau_j(d) is 0 or 1 (a group
+// is halved until that holds: the true relative delay drifts by less than a sample over a tile of close trials, so
+// its rounded value toggles between two neighbours).  The bit vectors tau(d) take only a few distinct values over the
+// tile ("variants"), so
+//     out[d][t] = sum_groups P_{r(d)}[ t - t0 + b(d) ],     P_r[u] = sum_j y[c0+j][t0 + dmin + u + s_j + tau^r_j]
+// is the SAME integer sum as the definition, with every P_r built once per tile and shared by its trials.
+// tau_j(d) = [theta(d) >= threshold_j] up to the slow drift, so ordered by how often they are 1 the channels form a
+// chain: most variants are "the first k channels of the order take the alternate shift".  The kernel walks that chain
+// with one vector add per step; a variant off the chain carries correction masks.
 // -------------------------------------------------------------------------------------------------------------
 namespace {
 
+struct PendingVariant { int k; uint32_t plus, minus, bits; };
+
+struct PendingEntry { int j, level; bool addbase; int ones; };   // one pre-sum entry: channel offset j at shift s_j + level
+
 struct PendingGroup {
-    int32_t chan0, nch, dmin, vlen, nvar;
-    std::vector<std::vector<int16_t>> vars;   // [nvar][nch] rho
+    int32_t chan0, nch, dmin, vlen, nvar, nent;
+    std::vector<PendingEntry> ent;            // prefix order (most often taken delta first)
+    std::vector<int16_t> smin, smax;          // [nch] by channel offset j
+    std::vector<PendingVariant> vars;         // sorted by k
     std::vector<int> var_of;                  // [ntrial]
     std::vector<int32_t> b;                   // [ntrial]
-    std::vector<RowDesc> rows;                // [nch], soff relative to the group's first row
-    int32_t raw_bytes, vwords, npairs;
+    std::vector<RowDesc> rows;                // [nch] by channel offset j, soff relative to the group's first row
+    int32_t raw_bytes, vwords, ncorrected;
 };
+
+inline int popcount32(uint32_t x) { return __builtin_popcount(x); }
 
 }  // namespace
 
+// Entries of a group: every channel has one entry at its smallest relative delay s_j (it adds the channel to the
+// base sum); a channel whose relative delay reaches s_j + L over the tile has L entries, at s_j .. s_j+L-1, and the
+// delta of the entry at level l (sample one later minus sample) moves the channel from s_j+l to s_j+l+1: bit
+// "tau_j > l".  Bits sorted by how often they are set form the prefix chain.
 static bool make_group(const Plan& p, const RangePlan& rp, int32_t d0, int32_t ntrial, int32_t c0, int G, int es,
                        PendingGroup& g) {
     g.chan0 = c0;
@@ -107,51 +121,87 @@ static bool make_group(const Plan& p, const RangePlan& rp, int32_t d0, int32_t n
         dmin = std::min(dmin, v); dmax = std::max(dmax, v);
     }
     g.dmin = dmin;
-    g.vlen = kH + (dmax - dmin);
+    g.vlen = (int32_t)round_up(kH + (dmax - dmin), 4);
     g.b.resize(ntrial);
     for (int i = 0; i < ntrial; ++i) g.b[i] = rp.delay[(size_t)(d0 + i) * p.nchan + c0] - dmin;
     g.var_of.assign(ntrial, 0);
-    // distinct relative-delay vectors of the tile's trials; the group is halved until they are few (widely spaced
-    // channels at high DM have a different vector for every trial: nothing to share)
-    for (int gsize = std::min(G, p.nchan - c0);; gsize >>= 1) {
-        std::map<std::vector<int16_t>, int> seen;
-        g.vars.clear();
+    // the group shrinks until its entries fit the kernel's registers and the variants are few (widely spaced
+    // channels at high DM have a different relative delay for every trial: nothing to share)
+    for (int gsize = std::min(G, p.nchan - c0);; --gsize) {
         g.nch = gsize;
+        g.smin.assign(gsize, 0);
+        g.smax.assign(gsize, 0);
+        int nent = 0;
+        bool ok = true;
+        for (int j = 0; j < gsize && ok; ++j) {
+            int lo = INT32_MAX, hi = INT32_MIN;
+            for (int i = 0; i < ntrial; ++i) {
+                const int32_t* row = &rp.delay[(size_t)(d0 + i) * p.nchan + c0];
+                const int s = row[j] - row[0];
+                lo = std::min(lo, s); hi = std::max(hi, s);
+            }
+            if (lo < 0 || hi > 30000) return false;
+            g.smin[j] = (int16_t)lo; g.smax[j] = (int16_t)hi;
+            nent += std::max(1, hi - lo);
+            if (nent > kMaxG) ok = false;
+        }
+        if (!ok) continue;   // gsize == 1 always passes: channel c0 relative to itself
+        g.ent.clear();
+        for (int j = 0; j < gsize; ++j)
+            for (int l = 0; l < std::max(1, g.smax[j] - g.smin[j]); ++l) g.ent.push_back({j, l, l == 0, 0});
         for (int i = 0; i < ntrial; ++i) {
             const int32_t* row = &rp.delay[(size_t)(d0 + i) * p.nchan + c0];
-            std::vector<int16_t> rho(gsize, 0);
-            for (int j = 0; j < gsize; ++j) {
-                const int s = row[j] - row[0];
-                if (s > 30000) return false;
-                rho[j] = (int16_t)s;
-            }
-            auto it = seen.find(rho);
-            if (it == seen.end()) {
-                it = seen.emplace(rho, (int)g.vars.size()).first;
-                g.vars.push_back(rho);
-            }
-            g.var_of[i] = it->second;
+            for (PendingEntry& e : g.ent)
+                if (row[e.j] - row[0] - g.smin[e.j] > e.level) e.ones++;
         }
-        if (gsize == 1 || (int)g.vars.size() <= kMaxVar) break;
+        std::stable_sort(g.ent.begin(), g.ent.end(), [](const PendingEntry& a, const PendingEntry& b) { return a.ones > b.ones; });
+        int ntog = 0;
+        for (const PendingEntry& e : g.ent) ntog += e.ones > 0;
+        // distinct variants, as bit masks over the positions of the prefix order
+        std::map<uint32_t, int> seen;
+        std::vector<uint32_t> bits_of_trial(ntrial);
+        for (int i = 0; i < ntrial; ++i) {
+            const int32_t* row = &rp.delay[(size_t)(d0 + i) * p.nchan + c0];
+            uint32_t m = 0;
+            for (int q = 0; q < (int)g.ent.size(); ++q)
+                if (row[g.ent[q].j] - row[0] - g.smin[g.ent[q].j] > g.ent[q].level) m |= 1u << q;
+            bits_of_trial[i] = m;
+            seen.emplace(m, 0);
+        }
+        if ((int)seen.size() > kMaxVar) continue;   // gsize == 1 has exactly one variant
+        g.vars.clear();
+        for (auto& kv : seen) {
+            PendingVariant v{0, 0, 0, kv.first};
+            int best = 1 << 30;
+            for (int k = 0; k <= ntog; ++k) {
+                const uint32_t pre = (1u << k) - 1u;
+                const int cost = popcount32(kv.first ^ pre);
+                if (cost < best) { best = cost; v.k = k; v.plus = kv.first & ~pre; v.minus = pre & ~kv.first; }
+            }
+            g.vars.push_back(v);
+        }
+        std::stable_sort(g.vars.begin(), g.vars.end(), [](const PendingVariant& a, const PendingVariant& b) { return a.k < b.k; });
+        g.ncorrected = 0;
+        for (size_t r = 0; r < g.vars.size(); ++r) {
+            seen[g.vars[r].bits] = (int)r;
+            g.ncorrected += (g.vars[r].plus | g.vars[r].minus) != 0;
+        }
+        for (int i = 0; i < ntrial; ++i) g.var_of[i] = seen[bits_of_trial[i]];
+        break;
     }
+    g.nent = (int32_t)g.ent.size();
     g.nvar = (int32_t)g.vars.size();
     g.vwords = g.nvar * g.vlen;
     g.rows.resize(g.nch);
     g.raw_bytes = 0;
-    g.npairs = 0;
     for (int j = 0; j < g.nch; ++j) {
-        int rmin = INT32_MAX, rmax = 0;
-        std::vector<int> shifts;
-        for (auto& v : g.vars) {
-            rmin = std::min<int>(rmin, v[j]); rmax = std::max<int>(rmax, v[j]);
-            if (std::find(shifts.begin(), shifts.end(), (int)v[j]) == shifts.end()) shifts.push_back(v[j]);
-        }
-        g.npairs += (int32_t)shifts.size();
         RowDesc& r = g.rows[j];
         r.chan = c0 + j;
-        r.astart = (dmin + rmin) & ~15;
-        const int32_t last = dmin + rmax + (g.vlen - 1) + kH;   // last element any valid output can need
-        r.nelem = (int32_t)((last + 1 + kRowSlack - r.astart + 15) / 16 * 16);
+        r.astart = (dmin + g.smin[j]) & ~15;
+        // last element a pre-sum task touches: u = vlen-1 at the largest shift in the high half, plus the words
+        // its aligned 32-bit loads reach past it
+        const int32_t last = dmin + std::max<int>(g.smax[j], g.smin[j] + 1) + g.vlen + kH + 8;
+        r.nelem = (int32_t)round_up(last - r.astart, 16);
         r.soff = g.raw_bytes;
         g.raw_bytes += r.nelem * es;
     }
@@ -162,7 +212,7 @@ int build_tiling(Plan& p) {
     const int G = p.opt_group, DT = p.opt_dm_tile;
     for (RangePlan& rp : p.ranges) {
         rp.tiles.clear(); rp.sidx.clear(); rp.rows.clear(); rp.blob.clear();
-        rp.ngroups = rp.nvariants = rp.npairs = 0;
+        rp.ngroups = rp.nvariants = rp.ncorrected = 0;
         rp.ntile_t = (int32_t)((rp.max_nout + kTT - 1) / kTT);
         const int es = rp.decim == 1 ? 1 : 2;
         // 16-bit lanes hold sums of at most floor(65535 / (255*decim)) channel samples
@@ -184,7 +234,7 @@ int build_tiling(Plan& p) {
             v = std::min<int64_t>(v, 65535 * 4);
             rp.vcap_words = (int32_t)(v / 16 * 4);
         }
-        const int64_t rcap_bytes = std::min<int64_t>(kSmemDataBytes - (int64_t)rp.vcap_words * 4, 1 << 17);
+        const int64_t rcap_bytes = kSmemDataBytes - (int64_t)rp.vcap_words * 4;
 
         for (int32_t d0 = 0; d0 < rp.ndm; d0 += DT) {
             TileDesc td;
@@ -192,10 +242,16 @@ int build_tiling(Plan& p) {
             td.ntrial = std::min(DT, rp.ndm - d0);
             td.stage0 = (int32_t)rp.sidx.size();
             std::vector<PendingGroup> open;
-            int64_t open_v = 0, open_r = 0, open_pairs = 0;
+            int64_t open_v = 0, open_r = 0;
             int since_flush = 0;
-            auto blob_words_of = [&](size_t ngrp, int64_t npairs) {
-                return (int64_t)kBlobHdrWords + 4 * (int64_t)ngrp + npairs + (int64_t)ngrp * DT / 2;
+            auto blob_words_of = [&](const std::vector<PendingGroup>& gs, const PendingGroup* extra) {
+                int64_t w = kBlobHdrWords;
+                auto one = [&](const PendingGroup& g) {
+                    w += 4 + (g.vlen + kChunkU - 1) / kChunkU + g.nent + 2 * (g.nvar + 1) + DT / 2;
+                };
+                for (const PendingGroup& g : gs) one(g);
+                if (extra) one(*extra);
+                return w;
             };
             auto close_stage = [&](bool flush) {
                 if (open.empty()) {
@@ -209,48 +265,58 @@ int build_tiling(Plan& p) {
                 si.blob_word0 = (uint32_t)rp.blob.size();
                 si.row0 = (uint32_t)rp.rows.size();
                 const size_t ngrp = open.size();
-                std::vector<uint32_t> hdr(kBlobHdrWords + 4 * ngrp), pairs;
+                std::vector<uint32_t> hdr(kBlobHdrWords + 4 * ngrp), tasks, cdesc, vdesc;
                 std::vector<uint16_t> toff;
                 int32_t vbase = 0, rbase = 0;
+                for (size_t k = 0; k < ngrp; ++k)
+                    for (int ch = 0; ch < (open[k].vlen + kChunkU - 1) / kChunkU; ++ch)
+                        tasks.push_back((uint32_t)k | ((uint32_t)ch << 8));
+                const uint32_t cdesc0 = (uint32_t)(hdr.size() + tasks.size());
                 for (size_t k = 0; k < ngrp; ++k) {
                     PendingGroup& g = open[k];
-                    const uint32_t pair0 = (uint32_t)pairs.size();
+                    const uint32_t my_cdesc = cdesc0 + (uint32_t)cdesc.size();
                     for (int j = 0; j < g.nch; ++j) {
                         RowDesc r = g.rows[j];
                         r.soff += rbase;
                         rp.rows.push_back(r);
-                        // shifts of this channel, most used first (= base pair)
-                        std::vector<std::pair<int, int>> cnt;  // (shift, variants using it)
-                        for (auto& v : g.vars) {
-                            auto it = std::find_if(cnt.begin(), cnt.end(), [&](auto& x) { return x.first == v[j]; });
-                            if (it == cnt.end()) cnt.push_back({v[j], 1}); else it->second++;
-                        }
-                        std::stable_sort(cnt.begin(), cnt.end(), [](auto& a, auto& b) { return a.second > b.second; });
-                        for (size_t q = 0; q < cnt.size(); ++q) {
-                            const int s = cnt[q].first;
-                            const uint32_t off = (uint32_t)(r.soff + (g.dmin + s - r.astart) * es);
-                            uint32_t mask = 0;
-                            if (q > 0)
-                                for (int v = 0; v < g.nvar; ++v) if (g.vars[v][j] == s) mask |= 1u << v;
-                            pairs.push_back(off | (q == 0 ? kPairBaseBit : 0u) | (mask << 20));
-                        }
+                    }
+                    for (const PendingEntry& en : g.ent) {
+                        const RowDesc& r = g.rows[en.j];
+                        const int32_t e0 = g.dmin + g.smin[en.j] + en.level - r.astart;   // element of the entry's u = 0 sample
+                        const uint32_t byte = (uint32_t)(rbase + r.soff + e0 * es);
+                        cdesc.push_back((byte >> 2) | ((es == 1 ? (byte & 3u) : (uint32_t)(e0 & 1)) << 24) |
+                                        (en.addbase ? kEntryAddBase : 0u));
                     }
                     hdr[kBlobHdrWords + 4 * k + 0] = (uint32_t)vbase;
                     hdr[kBlobHdrWords + 4 * k + 1] = (uint32_t)g.vlen;
-                    hdr[kBlobHdrWords + 4 * k + 2] = pair0 | ((uint32_t)(pairs.size() - pair0) << 16);
-                    hdr[kBlobHdrWords + 4 * k + 3] = (uint32_t)g.nvar;
+                    hdr[kBlobHdrWords + 4 * k + 2] = (uint32_t)g.nent | ((uint32_t)g.nvar << 8);
+                    hdr[kBlobHdrWords + 4 * k + 3] = my_cdesc;                     // vdesc offset patched below
                     for (int i = 0; i < DT; ++i) {
                         const int ii = std::min(i, td.ntrial - 1);  // unused trial slots alias the last valid trial
                         toff.push_back((uint16_t)(vbase + g.var_of[ii] * g.vlen + g.b[ii]));
                     }
                     vbase += g.vwords;
                     rbase += g.raw_bytes;
-                    rp.ngroups++; rp.nvariants += g.nvar;
+                    rp.ngroups++; rp.nvariants += g.nvar; rp.ncorrected += g.ncorrected;
                 }
-                rp.npairs += (int64_t)pairs.size();
-                hdr[0] = (uint32_t)ngrp; hdr[1] = flush ? 1u : 0u; hdr[2] = (uint32_t)pairs.size(); hdr[3] = 0;
+                const uint32_t vdesc0 = cdesc0 + (uint32_t)cdesc.size();
+                vbase = 0;
+                for (size_t k = 0; k < ngrp; ++k) {
+                    PendingGroup& g = open[k];
+                    hdr[kBlobHdrWords + 4 * k + 3] |= (vdesc0 + (uint32_t)vdesc.size()) << 16;
+                    for (int r = 0; r < g.nvar; ++r) {
+                        vdesc.push_back((uint32_t)(vbase + r * g.vlen));
+                        vdesc.push_back((uint32_t)g.vars[r].k | (g.vars[r].plus << 8) | (g.vars[r].minus << 16));
+                    }
+                    vdesc.push_back(0); vdesc.push_back(255u);
+                    vbase += g.vwords;
+                }
+                hdr[0] = (uint32_t)ngrp; hdr[1] = flush ? 1u : 0u; hdr[2] = (uint32_t)tasks.size();
+                hdr[3] = vdesc0 + (uint32_t)vdesc.size();
                 rp.blob.insert(rp.blob.end(), hdr.begin(), hdr.end());
-                rp.blob.insert(rp.blob.end(), pairs.begin(), pairs.end());
+                rp.blob.insert(rp.blob.end(), tasks.begin(), tasks.end());
+                rp.blob.insert(rp.blob.end(), cdesc.begin(), cdesc.end());
+                rp.blob.insert(rp.blob.end(), vdesc.begin(), vdesc.end());
                 for (size_t i = 0; i < toff.size(); i += 2)
                     rp.blob.push_back((uint32_t)toff[i] | ((uint32_t)(i + 1 < toff.size() ? toff[i + 1] : 0) << 16));
                 while ((rp.blob.size() - si.blob_word0) % 4) rp.blob.push_back(0);
@@ -259,21 +325,19 @@ int build_tiling(Plan& p) {
                 rp.sidx.push_back(si);
                 if (flush) since_flush = 0;
                 open.clear();
-                open_v = open_r = open_pairs = 0;
+                open_v = open_r = 0;
             };
             for (int32_t c = 0; c < p.nchan;) {
                 PendingGroup g;
                 if (!make_group(p, rp, d0, td.ntrial, c, G, es, g)) return SPT_ERR_UNSUPPORTED;
                 c += g.nch;
-                if (g.vwords > rp.vcap_words || g.raw_bytes > rcap_bytes ||
-                    blob_words_of(1, g.npairs) * 4 > kBlobBytes)
+                if (g.vwords > rp.vcap_words || g.raw_bytes > rcap_bytes || blob_words_of({}, &g) * 4 > kBlobBytes)
                     return SPT_ERR_UNSUPPORTED;  // one group must fit a stage
                 if (since_flush + g.nch > lane_channels) close_stage(true);
                 else if (open_v + g.vwords > rp.vcap_words || open_r + g.raw_bytes > rcap_bytes ||
-                         (int)open.size() >= kMaxStageGroups ||
-                         blob_words_of(open.size() + 1, open_pairs + g.npairs) * 4 > kBlobBytes)
+                         (int)open.size() >= kMaxStageGroups || blob_words_of(open, &g) * 4 > kBlobBytes)
                     close_stage(false);
-                open_v += g.vwords; open_r += g.raw_bytes; open_pairs += g.npairs;
+                open_v += g.vwords; open_r += g.raw_bytes;
                 since_flush += g.nch;
                 open.push_back(std::move(g));
             }
