@@ -384,7 +384,7 @@ int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int6
             const uint32_t* b = &rp.blob[si.blob_word0];
             int64_t v = 0, r = 0;
             for (uint32_t k = 0; k < b[0]; ++k)
-                v += (int64_t)b[kBlobHdrWords + 4 * k + 1] * (b[kBlobHdrWords + 4 * k + 2] >> 8);
+                v += (int64_t)b[kBlobHdrWords + 4 * k + 1] * (b[kBlobHdrWords + 4 * k + 2] >> 24);
             for (uint32_t k = 0; k < si.nrows; ++k) r += (int64_t)rp.rows[si.row0 + k].nelem * es;
             if (v > rp.vcap_words || r > kSmemDataBytes - (int64_t)rp.vcap_words * 4) return SPT_ERR_STATE;
             m = std::max(m, v + r / 4);
@@ -415,26 +415,31 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
         for (uint32_t g = 0; g < ngrp; ++g) {
             const uint32_t* gh = b + kBlobHdrWords + 4 * g;
             const int32_t vbase = (int32_t)gh[0], vlen = (int32_t)gh[1];
-            const int32_t nch = (int32_t)(gh[2] & 0xffu), nvar = (int32_t)(gh[2] >> 8);
+            const int32_t nch = (int32_t)(gh[2] & 0xffu), ntog = (int32_t)((gh[2] >> 8) & 0xffu);
+            const int32_t ncorr = (int32_t)((gh[2] >> 16) & 0xffu), nvar = (int32_t)(gh[2] >> 24);
             const uint32_t* cd = b + (gh[3] & 0xffffu);
             const uint32_t* vd = b + (gh[3] >> 16);
             const int32_t to = (int32_t)toff[g * DT + dl];
             const int32_t rel = to - vbase, r = rel / vlen, bb = rel - r * vlen;
-            if (r < 0 || r >= nvar || (int32_t)vd[2 * r] != vbase + r * vlen) return SPT_ERR_STATE;
-            // the gather reads P_r[q + bb]; P_r[u] takes, of the channel at position q of the prefix order, the sample
-            // at its base shift + u, or one later when the variant has it on the alternate shift
-            const uint32_t k = vd[2 * r + 1] & 0xffu, plus = (vd[2 * r + 1] >> 8) & 0xffu, minus = vd[2 * r + 1] >> 16;
+            if (r < 0 || r >= nvar) return SPT_ERR_STATE;
+            // the gather reads P_r[q + bb]; P_r[u] takes, of the entry at position q, the sample at its shift + u, or
+            // one later when the variant takes the entry's delta.  Which deltas: from the chain word or the mask.
+            uint32_t bits = 0xffffffffu;
+            for (int32_t k = 0; k <= ntog; ++k)
+                if (vd[k] == (uint32_t)(vbase + r * vlen)) bits = (1u << k) - 1u;
+            for (int32_t c = 0; c < ncorr; ++c)
+                if (vd[ntog + 1 + 2 * c] == (uint32_t)(vbase + r * vlen)) bits = ((1u << ntog) - 1u) & ~vd[ntog + 2 + 2 * c];
+            if (bits == 0xffffffffu) return SPT_ERR_STATE;
             for (int pass = 0; pass < 2; ++pass)       // pass 0: base shifts; pass 1: one sample later per delta taken
                 for (int32_t q = 0; q < nch; ++q) {
-                    const int32_t byte = (int32_t)((cd[q] & 0xffffffu) * 4u) +
-                                         (es == 1 ? (int32_t)((cd[q] >> 24) & 3u) : 2 * (int32_t)((cd[q] >> 24) & 3u));
+                    const int32_t byte = (int32_t)(cd[q] & 0x3ffffu) + (int32_t)((cd[q] >> 24) & 3u) * es;
                     const RowDesc* row = nullptr;
                     for (uint32_t i = 0; i < si.nrows; ++i) {
                         const RowDesc& rr = rp->rows[si.row0 + i];
                         if (byte >= rr.soff && byte < rr.soff + rr.nelem * es) { row = &rr; break; }
                     }
                     if (!row) return SPT_ERR_STATE;
-                    const bool taken = (((uint32_t)q < k) && !((minus >> q) & 1u)) || ((plus >> q) & 1u);
+                    const bool taken = (bits >> q) & 1u;
                     if (pass == 0 && (cd[q] & kEntryAddBase)) {
                         if (host_out[row->chan] != INT32_MIN) return SPT_ERR_STATE;   // every channel exactly once
                         host_out[row->chan] = row->astart + (byte - row->soff) / es + bb;

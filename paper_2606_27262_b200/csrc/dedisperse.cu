@@ -149,14 +149,22 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
-// The five packed words w_i = y[u0+i] | y[u0+i+kH] << 16, i = 0..4, of one channel at its base shift.
-// cd: bits 0-23 word index (raw region) of the word holding the u = 0 sample, bits 24-25 its position in the word.
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+    uint32_t v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
+    asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
+}
+
+// The five packed words w_i = y[u0+i] | y[u0+i+kH] << 16, i = 0..4, of one entry (a channel at one of its shifts).
+// addr: shared-memory byte address of the aligned 32-bit word holding the lane's first sample; a0: position of that
+// sample inside the word.
 template <typename T>
-__device__ __forceinline__ void load_channel(const uint32_t* __restrict__ s_raw, uint32_t cd, int u0, uint32_t (&w)[5]) {
-    const uint32_t a0 = (cd >> 24) & 3u;
+__device__ __forceinline__ void load_entry(uint32_t addr, uint32_t a0, uint32_t (&w)[5]) {
     if (sizeof(T) == 1) {
-        const uint32_t* pw = s_raw + (cd & 0xffffffu) + (u0 >> 2);
-        const uint32_t aL = pw[0], bL = pw[1], aH = pw[kH / 4], bH = pw[kH / 4 + 1];
+        const uint32_t aL = lds32(addr), bL = lds32(addr + 4), aH = lds32(addr + kH), bH = lds32(addr + kH + 4);
         const uint32_t sh = a0 * 8u;
         const uint32_t Lw = __funnelshift_r(aL, bL, sh), Hw = __funnelshift_r(aH, bH, sh);   // samples 0..3
         const uint32_t Le = Lw & 0x00FF00FFu, Lo = __byte_perm(Lw, 0u, 0x4341);
@@ -165,45 +173,46 @@ __device__ __forceinline__ void load_channel(const uint32_t* __restrict__ s_raw,
         w[1] = __byte_perm(Lo, Ho, 0x5410);
         w[2] = __byte_perm(Le, He, 0x7632);
         w[3] = __byte_perm(Lo, Ho, 0x7632);
-        const uint32_t sel = a0 | (a0 << 4) | ((a0 + 4u) << 8) | ((a0 + 4u) << 12);         // sample 4 = byte a0 of b
-        w[4] = __byte_perm(bL, bH, sel) & 0x00FF00FFu;
+        w[4] = __byte_perm(bL, bH, a0 * 0x1111u + 0x4400u) & 0x00FF00FFu;                    // sample 4 = byte a0 of b
     } else {
-        const uint32_t* pw = s_raw + (cd & 0xffffffu) + (u0 >> 1);
-        const uint32_t x0L = pw[0], x1L = pw[1], x2L = pw[2];
-        const uint32_t x0H = pw[kH / 2], x1H = pw[kH / 2 + 1], x2H = pw[kH / 2 + 2];
-        if (a0 == 0u) {
-            w[0] = __byte_perm(x0L, x0H, 0x5410); w[1] = __byte_perm(x0L, x0H, 0x7632);
-            w[2] = __byte_perm(x1L, x1H, 0x5410); w[3] = __byte_perm(x1L, x1H, 0x7632);
-            w[4] = __byte_perm(x2L, x2H, 0x5410);
-        } else {
-            w[0] = __byte_perm(x0L, x0H, 0x7632); w[1] = __byte_perm(x1L, x1H, 0x5410);
-            w[2] = __byte_perm(x1L, x1H, 0x7632); w[3] = __byte_perm(x2L, x2H, 0x5410);
-            w[4] = __byte_perm(x2L, x2H, 0x7632);
-        }
+        const uint32_t x0L = lds32(addr), x1L = lds32(addr + 4), x2L = lds32(addr + 8);
+        const uint32_t x0H = lds32(addr + 2 * kH), x1H = lds32(addr + 2 * kH + 4), x2H = lds32(addr + 2 * kH + 8);
+        const uint32_t s_even = a0 ? 0x7632u : 0x5410u, s_odd = a0 ? 0x5410u : 0x7632u;
+        w[0] = __byte_perm(x0L, x0H, s_even);
+        w[1] = __byte_perm(a0 ? x1L : x0L, a0 ? x1H : x0H, s_odd);
+        w[2] = __byte_perm(x1L, x1H, s_even);
+        w[3] = __byte_perm(a0 ? x2L : x1L, a0 ? x2H : x1H, s_odd);
+        w[4] = __byte_perm(x2L, x2H, s_even);
     }
 }
 
-// B: one warp task = kChunkU variant words (4 per lane) of every variant of one group.
+// B: one warp task = kChunkU variant words (4 per lane) of every variant of one group.  All control flow is warp
+// uniform: a lane past the end of the variants works on the last four words and does not store.
 template <typename T>
-__device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uint32_t task, uint32_t* __restrict__ s_var,
-                                            const uint32_t* __restrict__ s_raw, int lane) {
+__device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uint32_t task, uint32_t var_addr,
+                                            uint32_t raw_addr, int lane) {
     const uint32_t* gh = tb + kBlobHdrWords + 4 * (task & 0xffu);
     const int vlen = (int)gh[1];
-    const int u0 = (int)(task >> 8) * kChunkU + lane * 4;
-    if (u0 >= vlen) return;                       // vlen is a multiple of 4; no warp-wide operation below
-    const int nch = (int)(gh[2] & 0xffu);
+    const uint32_t meta = gh[2];
+    const int nent = (int)(meta & 0xffu), ntog = (int)((meta >> 8) & 0xffu), ncorr = (int)((meta >> 16) & 0xffu);
     const uint32_t* cd = tb + (gh[3] & 0xffffu);
     const uint32_t* vd = tb + (gh[3] >> 16);
+    int u0 = (int)(task >> 8) * kChunkU + lane * 4;
+    const bool active = u0 < vlen;                // vlen is a multiple of 4
+    u0 = active ? u0 : vlen - 4;
+    const uint32_t rbase = raw_addr + (uint32_t)u0 * (uint32_t)sizeof(T);
+    const uint32_t vbase = var_addr + (uint32_t)u0 * 4u;
     uint32_t cur[4] = {0u, 0u, 0u, 0u};
     uint32_t dl[kMaxG][4];
 #pragma unroll
     for (int q = 0; q < kMaxG; ++q) {
-        if (q < nch) {
+        if (q < nent) {
+            const uint32_t c = cd[q];
             uint32_t w[5];
-            load_channel<T>(s_raw, cd[q], u0, w);
+            load_entry<T>(rbase + (c & 0x3ffffu), (c >> 24) & 3u, w);
 #pragma unroll
             for (int i = 0; i < 4; ++i) dl[q][i] = w[i + 1] - w[i];
-            if (cd[q] & kEntryAddBase) {
+            if (c & kEntryAddBase) {
 #pragma unroll
                 for (int i = 0; i < 4; ++i) cur[i] += w[i];
             }
@@ -212,29 +221,29 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
             for (int i = 0; i < 4; ++i) dl[q][i] = 0u;
         }
     }
-    // prefix chain: after step k, cur = all channels at their base shift except the first k of the order
-    uint32_t dst = vd[0], code = vd[1];
+    // prefix chain: after step k, cur = base sum + deltas of the first k entries
 #pragma unroll
     for (int k = 0; k <= kMaxG; ++k) {
-        if (k > 0) {
+        if (k <= ntog) {
+            if (k > 0) {
 #pragma unroll
-            for (int i = 0; i < 4; ++i) cur[i] += dl[k - 1][i];
-        }
-        while ((code & 0xffu) == (uint32_t)k) {
-            uint4 o = make_uint4(cur[0], cur[1], cur[2], cur[3]);
-            const uint32_t fix = code >> 8;
-            if (fix != 0u) {                      // a variant off the chain (rare)
-#pragma unroll
-                for (int q = 0; q < kMaxG; ++q) {
-                    if (fix & (1u << q)) { o.x += dl[q][0]; o.y += dl[q][1]; o.z += dl[q][2]; o.w += dl[q][3]; }
-                    if (fix & (0x100u << q)) { o.x -= dl[q][0]; o.y -= dl[q][1]; o.z -= dl[q][2]; o.w -= dl[q][3]; }
-                }
+                for (int i = 0; i < 4; ++i) cur[i] += dl[k - 1][i];
             }
-            *reinterpret_cast<uint4*>(s_var + dst + u0) = o;
-            vd += 2;
-            dst = vd[0]; code = vd[1];
+            const uint32_t dst = vd[k];
+            if (dst != 0xffffffffu && active) sts128(vbase + dst * 4u, cur[0], cur[1], cur[2], cur[3]);
         }
-        if ((code & 0xffu) == 255u) break;        // the sentinel entry
+    }
+    // variants off the chain (few): all deltas, minus those the variant does not take
+    for (int c = 0; c < ncorr; ++c) {
+        const uint32_t dst = vd[ntog + 1 + 2 * c], mask = vd[ntog + 2 + 2 * c];
+        uint32_t o[4] = {cur[0], cur[1], cur[2], cur[3]};
+#pragma unroll
+        for (int q = 0; q < kMaxG; ++q)
+            if (mask & (1u << q)) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) o[i] -= dl[q][i];
+            }
+        if (active) sts128(vbase + dst * 4u, o[0], o[1], o[2], o[3]);
     }
 }
 
@@ -246,8 +255,12 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     static_assert(TPW >= 1 && TPW * NW == DT, "DT must be a multiple of the warp count");
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t bar = smem_u32(smem);
+    // control area: mbarrier, then per trial of the tile {row pointer, nout} for the flush
+    int32_t** const s_rowp = reinterpret_cast<int32_t**>(smem + 64);
+    int32_t* const s_nout = reinterpret_cast<int32_t*>(smem + 64 + kMaxDT * 8);
     uint32_t* const s_var = reinterpret_cast<uint32_t*>(smem + kSmemCtrlBytes + 2 * kBlobBytes);
     uint8_t* const s_rawb = reinterpret_cast<uint8_t*>(s_var + a.vcap_words);
+    const uint32_t var_addr = smem_u32(s_var), raw_addr = smem_u32(s_rawb);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     int bid = blockIdx.x;
@@ -294,6 +307,11 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_proxy_async();
     }
+    if (tid < DT) {
+        const int d = td.trial0 + (tid < td.ntrial ? tid : td.ntrial - 1);
+        s_rowp[tid] = a.out + (int64_t)beam * a.out_beam_stride + a.offset[d] + t0;
+        s_nout[tid] = tid < td.ntrial ? (int32_t)min((int64_t)kTT, max((int64_t)0, (int64_t)a.nout[d] - t0)) : 0;  // valid outputs of the tile
+    }
     __syncthreads();
     if (warp == 0) issue_stage(0);
 
@@ -314,18 +332,30 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
 
         // ---- B: pre-sum every variant of every group ---------------------------------------------------------
         for (int tk = warp; tk < ntask; tk += NW)
-            presum_task<T>(tb, tb[kBlobHdrWords + 4 * ngrp + tk], s_var, reinterpret_cast<const uint32_t*>(s_rawb), lane);
+            presum_task<T>(tb, tb[kBlobHdrWords + 4 * ngrp + tk], var_addr, raw_addr, lane);
         __syncthreads();  // variants complete; raw rows and the other blob buffer are free
         if (warp == 0 && s + 1 < td.nstage) issue_stage(s + 1);
 
         // ---- C: gather-accumulate ------------------------------------------------------------------------------
-        for (int g = 0; g < ngrp; ++g) {
-            const uint16_t* to = toff + g * DT + warp * TPW;
+        {
+            const uint32_t lane_addr = var_addr + (uint32_t)lane * 4u;
+            const uint16_t* to = toff + warp * TPW;
+            for (int g = 0; g < ngrp; ++g, to += DT) {
+                uint32_t off[TPW];
+                if (TPW == 8) {
+                    const uint4 o4 = *reinterpret_cast<const uint4*>(to);
+                    off[0] = o4.x & 0xffffu; off[1] = o4.x >> 16; off[2] = o4.y & 0xffffu; off[3] = o4.y >> 16;
+                    off[4 % TPW] = o4.z & 0xffffu; off[5 % TPW] = o4.z >> 16; off[6 % TPW] = o4.w & 0xffffu; off[7 % TPW] = o4.w >> 16;
+                } else {
 #pragma unroll
-            for (int q = 0; q < TPW; ++q) {
-                const uint32_t* src = s_var + to[q] + lane;
+                    for (int q = 0; q < TPW; ++q) off[q] = to[q];
+                }
 #pragma unroll
-                for (int j = 0; j < NJ; ++j) acc[q][j] += src[32 * j];
+                for (int q = 0; q < TPW; ++q) {
+                    const uint32_t src = lane_addr + off[q] * 4u;
+#pragma unroll
+                    for (int j = 0; j < NJ; ++j) acc[q][j] += lds32(src + 128u * j);
+                }
             }
         }
         // ---- F: widen the 16-bit lanes into the int32 DM transform -------------------------------------------
@@ -333,20 +363,21 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
 #pragma unroll
             for (int q = 0; q < TPW; ++q) {
                 const int dl = warp * TPW + q;
-                if (dl < td.ntrial) {
-                    const int d = td.trial0 + dl;
-                    const int64_t n = a.nout[d];
-                    int32_t* row = a.out + (int64_t)beam * a.out_beam_stride + a.offset[d] + t0;
+                int32_t* row = s_rowp[dl];
+                const int n = s_nout[dl];
 #pragma unroll
-                    for (int j = 0; j < NJ; ++j) {
-                        const int i = lane + 32 * j;
-                        const int32_t lo = (int32_t)(acc[q][j] & 0xFFFFu), hi = (int32_t)(acc[q][j] >> 16);
-                        if (t0 + i < n) row[i] = first_flush ? lo : row[i] + lo;
-                        if (t0 + i + kH < n) row[i + kH] = first_flush ? hi : row[i + kH] + hi;
+                for (int j = 0; j < NJ; ++j) {
+                    const int i = lane + 32 * j;
+                    const int32_t lo = (int32_t)(acc[q][j] & 0xFFFFu), hi = (int32_t)(acc[q][j] >> 16);
+                    if (first_flush) {
+                        if (i < n) row[i] = lo;
+                        if (i + kH < n) row[i + kH] = hi;
+                    } else {
+                        if (i < n) atomicAdd(row + i, lo);          // result unused: a fire-and-forget RED in L2
+                        if (i + kH < n) atomicAdd(row + i + kH, hi);
                     }
+                    acc[q][j] = 0u;
                 }
-#pragma unroll
-                for (int j = 0; j < NJ; ++j) acc[q][j] = 0u;
             }
             first_flush = false;
         }

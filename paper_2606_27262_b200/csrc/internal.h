@@ -30,22 +30,22 @@ constexpr int kMaxStageGroups = 8;   // groups per stage
 constexpr int kChunkU = 128;         // variant words one warp builds per pre-sum task (4 per lane)
 constexpr int kBlobBytes = 3072;     // per-stage table blob (two buffers in shared memory)
 constexpr int kSmemBytes = 113 * 1024;                                   // two blocks per SM (228 KB incl. 1 KB each reserved)
-constexpr int kSmemCtrlBytes = 64;                                       // mbarrier + padding
+constexpr int kSmemCtrlBytes = 64 + kMaxDT * 16;                         // mbarrier, per-trial {row pointer, nout}
 constexpr int kSmemDataBytes = kSmemBytes - kSmemCtrlBytes - 2 * kBlobBytes;  // variant region + raw-row region
 
 // Per-stage blob, 32-bit words (copied to shared memory with one bulk copy):
 //   [0] ngrp  [1] flush  [2] ntask  [3] word offset of the trial_off table
-//   [4 ..)        ngrp x { vbase, vlen, nent | nvar << 8, cdesc_off | vdesc_off << 16 }      (offsets inside the blob)
+//   [4 ..)        ngrp x { vbase, vlen, nent | ntog << 8 | ncorr << 16 | nvar << 24, cdesc_off | vdesc_off << 16 }
+//                 (offsets inside the blob)
 //   task table    ntask x { group | chunk << 8 }: warp task = kChunkU variant words of every variant of one group
-//   cdesc         per group, nent <= kMaxG entries in PREFIX ORDER (most-often-taken delta first); an entry is a channel
-//                 at one of its shifts: bits 0-23 word index inside the raw region of the 32-bit word that holds the
-//                 entry's sample at u = 0, bits 24-25 position of that sample inside the word, bit 26 = the entry is
-//                 the channel's smallest shift and adds it to the base sum.  The entry's delta (sample one later
-//                 minus sample) moves its channel one sample later.
-//   vdesc         per group, nvar + 1 entries of 2 words, sorted by k: { word offset of the variant in the variant
-//                 region, k | plus << 8 | minus << 16 }: the variant is the base sum plus the deltas of the first k
-//                 entries, corrected by the entries in plus (delta taken too) and minus (not taken after all); the
-//                 extra entry has k = 255
+//   cdesc         per group, nent <= kMaxG entries in PREFIX ORDER (most-often-taken delta first; the first ntog have
+//                 a delta that some trial takes); an entry is a channel at one of its shifts: bits 0-17 byte offset
+//                 inside the raw region of the aligned 32-bit word that holds the entry's sample at u = 0, bits 24-25
+//                 position of that sample inside the word, bit 26 = the entry is the channel's smallest shift and adds
+//                 it to the base sum.  The entry's delta (sample one later minus sample) moves its channel one later.
+//   vdesc         per group: ntog + 1 chain words, word k = offset in the variant region of the variant "base sum +
+//                 deltas of the first k entries" (0xffffffff: no trial uses it); then ncorr x { offset, mask } for the
+//                 variants off the chain: all ntog deltas minus those in mask
 //   trial_off     ngrp x DT uint16 = word offset of the trial's read start in the variant region
 constexpr int kBlobHdrWords = 4;
 constexpr uint32_t kEntryAddBase = 1u << 26;

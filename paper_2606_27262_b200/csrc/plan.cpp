@@ -94,7 +94,7 @@ struct PendingVariant { int k; uint32_t plus, minus, bits; };
 struct PendingEntry { int j, level; bool addbase; int ones; };   // one pre-sum entry: channel offset j at shift s_j + level
 
 struct PendingGroup {
-    int32_t chan0, nch, dmin, vlen, nvar, nent;
+    int32_t chan0, nch, dmin, vlen, nvar, nent, ntog;
     std::vector<PendingEntry> ent;            // prefix order (most often taken delta first)
     std::vector<int16_t> smin, smax;          // [nch] by channel offset j
     std::vector<PendingVariant> vars;         // sorted by k
@@ -157,6 +157,7 @@ static bool make_group(const Plan& p, const RangePlan& rp, int32_t d0, int32_t n
         std::stable_sort(g.ent.begin(), g.ent.end(), [](const PendingEntry& a, const PendingEntry& b) { return a.ones > b.ones; });
         int ntog = 0;
         for (const PendingEntry& e : g.ent) ntog += e.ones > 0;
+        g.ntog = ntog;
         // distinct variants, as bit masks over the positions of the prefix order
         std::map<uint32_t, int> seen;
         std::vector<uint32_t> bits_of_trial(ntrial);
@@ -245,9 +246,9 @@ int build_tiling(Plan& p) {
             int64_t open_v = 0, open_r = 0;
             int since_flush = 0;
             auto blob_words_of = [&](const std::vector<PendingGroup>& gs, const PendingGroup* extra) {
-                int64_t w = kBlobHdrWords;
+                int64_t w = kBlobHdrWords + 3;
                 auto one = [&](const PendingGroup& g) {
-                    w += 4 + (g.vlen + kChunkU - 1) / kChunkU + g.nent + 2 * (g.nvar + 1) + DT / 2;
+                    w += 4 + (g.vlen + kChunkU - 1) / kChunkU + g.nent + (g.ntog + 1) + 2 * g.ncorrected + DT / 2;
                 };
                 for (const PendingGroup& g : gs) one(g);
                 if (extra) one(*extra);
@@ -284,12 +285,12 @@ int build_tiling(Plan& p) {
                         const RowDesc& r = g.rows[en.j];
                         const int32_t e0 = g.dmin + g.smin[en.j] + en.level - r.astart;   // element of the entry's u = 0 sample
                         const uint32_t byte = (uint32_t)(rbase + r.soff + e0 * es);
-                        cdesc.push_back((byte >> 2) | ((es == 1 ? (byte & 3u) : (uint32_t)(e0 & 1)) << 24) |
+                        cdesc.push_back((byte & ~3u) | ((es == 1 ? (byte & 3u) : (uint32_t)(e0 & 1)) << 24) |
                                         (en.addbase ? kEntryAddBase : 0u));
                     }
                     hdr[kBlobHdrWords + 4 * k + 0] = (uint32_t)vbase;
                     hdr[kBlobHdrWords + 4 * k + 1] = (uint32_t)g.vlen;
-                    hdr[kBlobHdrWords + 4 * k + 2] = (uint32_t)g.nent | ((uint32_t)g.nvar << 8);
+                    hdr[kBlobHdrWords + 4 * k + 2] = (uint32_t)g.nent | ((uint32_t)g.ntog << 8) | ((uint32_t)g.ncorrected << 16) | ((uint32_t)g.nvar << 24);
                     hdr[kBlobHdrWords + 4 * k + 3] = my_cdesc;                     // vdesc offset patched below
                     for (int i = 0; i < DT; ++i) {
                         const int ii = std::min(i, td.ntrial - 1);  // unused trial slots alias the last valid trial
@@ -304,14 +305,23 @@ int build_tiling(Plan& p) {
                 for (size_t k = 0; k < ngrp; ++k) {
                     PendingGroup& g = open[k];
                     hdr[kBlobHdrWords + 4 * k + 3] |= (vdesc0 + (uint32_t)vdesc.size()) << 16;
-                    for (int r = 0; r < g.nvar; ++r) {
-                        vdesc.push_back((uint32_t)(vbase + r * g.vlen));
-                        vdesc.push_back((uint32_t)g.vars[r].k | (g.vars[r].plus << 8) | (g.vars[r].minus << 16));
+                    // chain: the variant that is exactly "first k deltas taken", k = 0..ntog (or none)
+                    for (int k2 = 0; k2 <= g.ntog; ++k2) {
+                        uint32_t dst = 0xffffffffu;
+                        for (int r = 0; r < g.nvar; ++r)
+                            if (g.vars[r].k == k2 && !(g.vars[r].plus | g.vars[r].minus)) dst = (uint32_t)(vbase + r * g.vlen);
+                        vdesc.push_back(dst);
                     }
-                    vdesc.push_back(0); vdesc.push_back(255u);
+                    // off the chain: destination and the mask of the deltas NOT taken (subtracted from the full sum)
+                    for (int r = 0; r < g.nvar; ++r)
+                        if (g.vars[r].plus | g.vars[r].minus) {
+                            vdesc.push_back((uint32_t)(vbase + r * g.vlen));
+                            vdesc.push_back(~g.vars[r].bits & ((1u << g.ntog) - 1u));
+                        }
                     vbase += g.vwords;
                 }
                 hdr[0] = (uint32_t)ngrp; hdr[1] = flush ? 1u : 0u; hdr[2] = (uint32_t)tasks.size();
+                while ((vdesc0 + vdesc.size()) % 4) vdesc.push_back(0);   // trial_off rows are read with 128-bit loads
                 hdr[3] = vdesc0 + (uint32_t)vdesc.size();
                 rp.blob.insert(rp.blob.end(), hdr.begin(), hdr.end());
                 rp.blob.insert(rp.blob.end(), tasks.begin(), tasks.end());
