@@ -432,7 +432,7 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
             if (bits == 0xffffffffu) return SPT_ERR_STATE;
             for (int pass = 0; pass < 2; ++pass)       // pass 0: base shifts; pass 1: one sample later per delta taken
                 for (int32_t q = 0; q < nch; ++q) {
-                    const int32_t byte = (int32_t)(cd[q] & 0x3ffffu) + (int32_t)((cd[q] >> 24) & 3u) * es;
+                    const int32_t byte = (int32_t)(cd[2 * q] & 0x3ffffu) + (int32_t)((cd[2 * q] >> 24) & 3u) * es;
                     const RowDesc* row = nullptr;
                     for (uint32_t i = 0; i < si.nrows; ++i) {
                         const RowDesc& rr = rp->rows[si.row0 + i];
@@ -440,7 +440,7 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
                     }
                     if (!row) return SPT_ERR_STATE;
                     const bool taken = (bits >> q) & 1u;
-                    if (pass == 0 && (cd[q] & kEntryAddBase)) {
+                    if (pass == 0 && (cd[2 * q] & kEntryAddBase)) {
                         if (host_out[row->chan] != INT32_MIN) return SPT_ERR_STATE;   // every channel exactly once
                         host_out[row->chan] = row->astart + (byte - row->soff) / es + bb;
                     }

@@ -158,44 +158,54 @@ __device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, ui
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
 
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+    uint32_t d;
+    asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
+    return d;
+}
+
 // The five packed words w_i = y[u0+i] | y[u0+i+kH] << 16, i = 0..4, of one entry (a channel at one of its shifts).
-// addr: shared-memory byte address of the aligned 32-bit word holding the lane's first sample; a0: position of that
-// sample inside the word.
+// addr: shared-memory byte address of the aligned 32-bit word holding the lane's first sample; c1: the entry's second
+// descriptor word (uint8: bits 0-4 = 8 * position of that sample inside the word, bits 8-23 = PRMT selector of sample 4;
+// uint16: bit 0 = position).
 template <typename T>
-__device__ __forceinline__ void load_entry(uint32_t addr, uint32_t a0, uint32_t (&w)[5]) {
+__device__ __forceinline__ void load_entry(uint32_t addr, uint32_t c1, uint32_t (&w)[5]) {
     if (sizeof(T) == 1) {
         const uint32_t aL = lds32(addr), bL = lds32(addr + 4), aH = lds32(addr + kH), bH = lds32(addr + kH + 4);
-        const uint32_t sh = a0 * 8u;
-        const uint32_t Lw = __funnelshift_r(aL, bL, sh), Hw = __funnelshift_r(aH, bH, sh);   // samples 0..3
-        const uint32_t Le = Lw & 0x00FF00FFu, Lo = __byte_perm(Lw, 0u, 0x4341);
-        const uint32_t He = Hw & 0x00FF00FFu, Ho = __byte_perm(Hw, 0u, 0x4341);
-        w[0] = __byte_perm(Le, He, 0x5410);
-        w[1] = __byte_perm(Lo, Ho, 0x5410);
-        w[2] = __byte_perm(Le, He, 0x7632);
-        w[3] = __byte_perm(Lo, Ho, 0x7632);
-        w[4] = __byte_perm(bL, bH, a0 * 0x1111u + 0x4400u) & 0x00FF00FFu;                    // sample 4 = byte a0 of b
+        uint32_t Lw, Hw;   // samples 0..3 (the shift amount is taken modulo 32: the selector bits above do not matter)
+        asm("shf.r.wrap.b32 %0, %1, %2, %3;" : "=r"(Lw) : "r"(aL), "r"(bL), "r"(c1));
+        asm("shf.r.wrap.b32 %0, %1, %2, %3;" : "=r"(Hw) : "r"(aH), "r"(bH), "r"(c1));
+        const uint32_t Le = Lw & 0x00FF00FFu, Lo = prmt(Lw, 0u, 0x4341u);
+        const uint32_t He = Hw & 0x00FF00FFu, Ho = prmt(Hw, 0u, 0x4341u);
+        w[0] = prmt(Le, He, 0x5410u);
+        w[1] = prmt(Lo, Ho, 0x5410u);
+        w[2] = prmt(Le, He, 0x7632u);
+        w[3] = prmt(Lo, Ho, 0x7632u);
+        w[4] = prmt(bL, bH, c1 >> 8) & 0x00FF00FFu;                    // sample 4 = byte a0 of the second word
     } else {
         const uint32_t x0L = lds32(addr), x1L = lds32(addr + 4), x2L = lds32(addr + 8);
         const uint32_t x0H = lds32(addr + 2 * kH), x1H = lds32(addr + 2 * kH + 4), x2H = lds32(addr + 2 * kH + 8);
-        const uint32_t s_even = a0 ? 0x7632u : 0x5410u, s_odd = a0 ? 0x5410u : 0x7632u;
-        w[0] = __byte_perm(x0L, x0H, s_even);
-        w[1] = __byte_perm(a0 ? x1L : x0L, a0 ? x1H : x0H, s_odd);
-        w[2] = __byte_perm(x1L, x1H, s_even);
-        w[3] = __byte_perm(a0 ? x2L : x1L, a0 ? x2H : x1H, s_odd);
-        w[4] = __byte_perm(x2L, x2H, s_even);
+        const bool odd = (c1 & 1u) != 0u;
+        const uint32_t s_even = odd ? 0x7632u : 0x5410u, s_odd = odd ? 0x5410u : 0x7632u;
+        w[0] = prmt(x0L, x0H, s_even);
+        w[1] = prmt(odd ? x1L : x0L, odd ? x1H : x0H, s_odd);
+        w[2] = prmt(x1L, x1H, s_even);
+        w[3] = prmt(odd ? x2L : x1L, odd ? x2H : x1H, s_odd);
+        w[4] = prmt(x2L, x2H, s_even);
     }
 }
 
 // B: one warp task = kChunkU variant words (4 per lane) of every variant of one group.  All control flow is warp
-// uniform: a lane past the end of the variants works on the last four words and does not store.
+// uniform and the eight entries are straight-line code (unused entries repeat the first one; their deltas are never
+// taken): a lane past the end of the variants works on the last four words and does not store.
 template <typename T>
 __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uint32_t task, uint32_t var_addr,
                                             uint32_t raw_addr, int lane) {
     const uint32_t* gh = tb + kBlobHdrWords + 4 * (task & 0xffu);
     const int vlen = (int)gh[1];
     const uint32_t meta = gh[2];
-    const int nent = (int)(meta & 0xffu), ntog = (int)((meta >> 8) & 0xffu), ncorr = (int)((meta >> 16) & 0xffu);
-    const uint32_t* cd = tb + (gh[3] & 0xffffu);
+    const int ntog = (int)((meta >> 8) & 0xffu), ncorr = (int)((meta >> 16) & 0xffu);
+    const uint2* cd = reinterpret_cast<const uint2*>(tb + (gh[3] & 0xffffu));
     const uint32_t* vd = tb + (gh[3] >> 16);
     int u0 = (int)(task >> 8) * kChunkU + lane * 4;
     const bool active = u0 < vlen;                // vlen is a multiple of 4
@@ -206,19 +216,14 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
     uint32_t dl[kMaxG][4];
 #pragma unroll
     for (int q = 0; q < kMaxG; ++q) {
-        if (q < nent) {
-            const uint32_t c = cd[q];
-            uint32_t w[5];
-            load_entry<T>(rbase + (c & 0x3ffffu), (c >> 24) & 3u, w);
+        const uint2 c = cd[q];
+        uint32_t w[5];
+        load_entry<T>(rbase + (c.x & 0x3ffffu), c.y, w);
 #pragma unroll
-            for (int i = 0; i < 4; ++i) dl[q][i] = w[i + 1] - w[i];
-            if (c & kEntryAddBase) {
+        for (int i = 0; i < 4; ++i) dl[q][i] = w[i + 1] - w[i];
+        if (c.x & kEntryAddBase) {
 #pragma unroll
-                for (int i = 0; i < 4; ++i) cur[i] += w[i];
-            }
-        } else {
-#pragma unroll
-            for (int i = 0; i < 4; ++i) dl[q][i] = 0u;
+            for (int i = 0; i < 4; ++i) cur[i] += w[i];
         }
     }
     // prefix chain: after step k, cur = base sum + deltas of the first k entries
@@ -340,21 +345,36 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
         {
             const uint32_t lane_addr = var_addr + (uint32_t)lane * 4u;
             const uint16_t* to = toff + warp * TPW;
-            for (int g = 0; g < ngrp; ++g, to += DT) {
-                uint32_t off[TPW];
+            auto offsets = [&](const uint16_t* t, uint32_t (&off)[TPW]) {
                 if (TPW == 8) {
-                    const uint4 o4 = *reinterpret_cast<const uint4*>(to);
+                    const uint4 o4 = *reinterpret_cast<const uint4*>(t);
                     off[0] = o4.x & 0xffffu; off[1] = o4.x >> 16; off[2] = o4.y & 0xffffu; off[3] = o4.y >> 16;
                     off[4 % TPW] = o4.z & 0xffffu; off[5 % TPW] = o4.z >> 16; off[6 % TPW] = o4.w & 0xffffu; off[7 % TPW] = o4.w >> 16;
                 } else {
 #pragma unroll
-                    for (int q = 0; q < TPW; ++q) off[q] = to[q];
+                    for (int q = 0; q < TPW; ++q) off[q] = t[q];
                 }
+            };
+            int g = 0;
+            for (; g + 2 <= ngrp; g += 2, to += 2 * DT) {   // two groups per pass: one 3-input add per pair of loads
+                uint32_t off0[TPW], off1[TPW];
+                offsets(to, off0);
+                offsets(to + DT, off1);
 #pragma unroll
                 for (int q = 0; q < TPW; ++q) {
-                    const uint32_t src = lane_addr + off[q] * 4u;
+                    const uint32_t s0 = lane_addr + off0[q] * 4u, s1 = lane_addr + off1[q] * 4u;
 #pragma unroll
-                    for (int j = 0; j < NJ; ++j) acc[q][j] += lds32(src + 128u * j);
+                    for (int j = 0; j < NJ; ++j) acc[q][j] += lds32(s0 + 128u * j) + lds32(s1 + 128u * j);
+                }
+            }
+            if (g < ngrp) {
+                uint32_t off0[TPW];
+                offsets(to, off0);
+#pragma unroll
+                for (int q = 0; q < TPW; ++q) {
+                    const uint32_t s0 = lane_addr + off0[q] * 4u;
+#pragma unroll
+                    for (int j = 0; j < NJ; ++j) acc[q][j] += lds32(s0 + 128u * j);
                 }
             }
         }

@@ -246,9 +246,9 @@ int build_tiling(Plan& p) {
             int64_t open_v = 0, open_r = 0;
             int since_flush = 0;
             auto blob_words_of = [&](const std::vector<PendingGroup>& gs, const PendingGroup* extra) {
-                int64_t w = kBlobHdrWords + 3;
+                int64_t w = kBlobHdrWords + 4;
                 auto one = [&](const PendingGroup& g) {
-                    w += 4 + (g.vlen + kChunkU - 1) / kChunkU + g.nent + (g.ntog + 1) + 2 * g.ncorrected + DT / 2;
+                    w += 4 + (g.vlen + kChunkU - 1) / kChunkU + 2 * kMaxG + (g.ntog + 1) + 2 * g.ncorrected + DT / 2;
                 };
                 for (const PendingGroup& g : gs) one(g);
                 if (extra) one(*extra);
@@ -272,6 +272,8 @@ int build_tiling(Plan& p) {
                 for (size_t k = 0; k < ngrp; ++k)
                     for (int ch = 0; ch < (open[k].vlen + kChunkU - 1) / kChunkU; ++ch)
                         tasks.push_back((uint32_t)k | ((uint32_t)ch << 8));
+                const uint32_t ntask = (uint32_t)tasks.size();
+                if ((hdr.size() + tasks.size()) % 2) tasks.push_back(0xffffffffu);   // 64-bit loads of the entry descriptors
                 const uint32_t cdesc0 = (uint32_t)(hdr.size() + tasks.size());
                 for (size_t k = 0; k < ngrp; ++k) {
                     PendingGroup& g = open[k];
@@ -285,8 +287,15 @@ int build_tiling(Plan& p) {
                         const RowDesc& r = g.rows[en.j];
                         const int32_t e0 = g.dmin + g.smin[en.j] + en.level - r.astart;   // element of the entry's u = 0 sample
                         const uint32_t byte = (uint32_t)(rbase + r.soff + e0 * es);
-                        cdesc.push_back((byte & ~3u) | ((es == 1 ? (byte & 3u) : (uint32_t)(e0 & 1)) << 24) |
-                                        (en.addbase ? kEntryAddBase : 0u));
+                        const uint32_t a0 = es == 1 ? (byte & 3u) : (uint32_t)(e0 & 1);
+                        cdesc.push_back((byte & ~3u) | (a0 << 24) | (en.addbase ? kEntryAddBase : 0u));
+                        // second word, ready for the kernel: uint8: funnel-shift amount and the PRMT selector of sample 4
+                        cdesc.push_back(es == 1 ? (a0 * 8u) | ((a0 * 0x1111u + 0x4400u) << 8) : a0);
+                    }
+                    for (int q = g.nent; q < kMaxG; ++q) {   // padding: straight-line code in the kernel; deltas never taken
+                        const uint32_t c0 = cdesc[cdesc.size() - 2 * (size_t)g.nent], c1 = cdesc[cdesc.size() - 2 * (size_t)g.nent + 1];
+                        cdesc.push_back(c0 & ~kEntryAddBase);
+                        cdesc.push_back(c1);
                     }
                     hdr[kBlobHdrWords + 4 * k + 0] = (uint32_t)vbase;
                     hdr[kBlobHdrWords + 4 * k + 1] = (uint32_t)g.vlen;
@@ -320,7 +329,7 @@ int build_tiling(Plan& p) {
                         }
                     vbase += g.vwords;
                 }
-                hdr[0] = (uint32_t)ngrp; hdr[1] = flush ? 1u : 0u; hdr[2] = (uint32_t)tasks.size();
+                hdr[0] = (uint32_t)ngrp; hdr[1] = flush ? 1u : 0u; hdr[2] = ntask;
                 while ((vdesc0 + vdesc.size()) % 4) vdesc.push_back(0);   // trial_off rows are read with 128-bit loads
                 hdr[3] = vdesc0 + (uint32_t)vdesc.size();
                 rp.blob.insert(rp.blob.end(), hdr.begin(), hdr.end());
