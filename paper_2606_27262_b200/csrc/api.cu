@@ -372,7 +372,7 @@ int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int6
     if (rc != SPT_OK) return rc;
     const RangePlan& rp = p.ranges[range];
     if (ntiles_dm) *ntiles_dm = (int64_t)rp.tiles.size();
-    if (nstages) *nstages = (int64_t)rp.sidx.size();
+    if (nstages) *nstages = (int64_t)rp.sidx.size() - 1;   // the last entry is padding
     if (ngroups) *ngroups = rp.ngroups;
     if (nvariants) *nvariants = rp.nvariants;
     if (ntiles_t) *ntiles_t = rp.ntile_t;
@@ -380,7 +380,8 @@ int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int6
         // largest shared-memory footprint of a stage: variant words + raw-row bytes, plus the fixed control area
         const int es = rp.decim == 1 ? 1 : 2;
         int64_t m = 0;
-        for (const StageIndex& si : rp.sidx) {
+        for (size_t is = 0; is + 1 < rp.sidx.size(); ++is) {
+            const StageIndex& si = rp.sidx[is];
             const uint32_t* b = &rp.blob[si.blob_word0];
             int64_t v = 0, r = 0;
             for (uint32_t k = 0; k < b[0]; ++k)

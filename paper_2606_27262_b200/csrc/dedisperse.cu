@@ -263,6 +263,8 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     // control area: mbarrier, then per trial of the tile {row pointer, nout} for the flush
     int32_t** const s_rowp = reinterpret_cast<int32_t**>(smem + 64);
     int32_t* const s_nout = reinterpret_cast<int32_t*>(smem + 64 + kMaxDT * 8);
+    RowDesc* const s_rows = reinterpret_cast<RowDesc*>(smem + 64 + kMaxDT * 16);                          // [2][kMaxStageRows]
+    StageIndex* const s_sidx = reinterpret_cast<StageIndex*>(smem + 64 + kMaxDT * 16 + 2 * kMaxStageRows * 16);  // [2]
     uint32_t* const s_var = reinterpret_cast<uint32_t*>(smem + kSmemCtrlBytes + 2 * kBlobBytes);
     uint8_t* const s_rawb = reinterpret_cast<uint8_t*>(s_var + a.vcap_words);
     const uint32_t var_addr = smem_u32(s_var), raw_addr = smem_u32(s_rawb);
@@ -278,32 +280,32 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
 
     const T* in = reinterpret_cast<const T*>(a.in) + (int64_t)beam * a.beam_stride;
 
-    // T: the elected warp arms the stage barrier with the byte count and issues the bulk copies
+    // T: the elected warp issues the bulk copies of stage s (table blob, raw rows, and the NEXT stage's index and row
+    // descriptors, so that no global-memory latency sits between a stage's pre-sum and its gather), then arms the
+    // barrier with the byte count.  Stage 0 reads its descriptors from global memory, later stages from shared.
     auto issue_stage = [&](int s) {
-        const StageIndex si = a.sidx[td.stage0 + s];
+        const StageIndex si = s == 0 ? a.sidx[td.stage0] : s_sidx[s & 1];
+        const RowDesc* rows = s == 0 ? a.rows + si.row0 : s_rows + (s & 1) * kMaxStageRows;
+        if (lane == 0) fence_proxy_async();  // generic-proxy reads of the buffers (previous stage) before async-proxy writes
+        __syncwarp();
         uint32_t bytes = 0;
         for (uint32_t k = lane; k < si.nrows; k += 32) {
-            const RowDesc r = a.rows[si.row0 + k];
-            const int64_t room = a.row_stride - (t0 + r.astart);
-            const int64_t n = room < (int64_t)r.nelem ? (room > 0 ? room : 0) : (int64_t)r.nelem;
-            bytes += (uint32_t)n * (uint32_t)sizeof(T);
-        }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
-        if (lane == 0) {
-            fence_proxy_async();  // generic-proxy reads of the buffers (previous stage) before async-proxy writes
-            mbar_expect_tx(bar, bytes + si.blob_words * 4u);
-            bulk_g2s(smem_u32(smem + kSmemCtrlBytes + (s & 1) * kBlobBytes), a.blob + si.blob_word0, si.blob_words * 4u, bar);
-        }
-        __syncwarp();
-        for (uint32_t k = lane; k < si.nrows; k += 32) {
-            const RowDesc r = a.rows[si.row0 + k];
+            const RowDesc r = rows[k];
             const int64_t pos = t0 + r.astart;
             const int64_t room = a.row_stride - pos;
             const int64_t n = room < (int64_t)r.nelem ? (room > 0 ? room : 0) : (int64_t)r.nelem;
             if (n > 0)
                 bulk_g2s(smem_u32(s_rawb + r.soff), in + (int64_t)r.chan * a.row_stride + pos,
                          (uint32_t)n * (uint32_t)sizeof(T), bar);
+            bytes += (uint32_t)n * (uint32_t)sizeof(T);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
+        if (lane == 0) {
+            bulk_g2s(smem_u32(smem + kSmemCtrlBytes + (s & 1) * kBlobBytes), a.blob + si.blob_word0, si.blob_words * 4u, bar);
+            bulk_g2s(smem_u32(s_sidx + ((s + 1) & 1)), a.sidx + td.stage0 + s + 1, 16u, bar);
+            bulk_g2s(smem_u32(s_rows + ((s + 1) & 1) * kMaxStageRows), a.rows + si.row0 + si.nrows, kMaxStageRows * 16u, bar);
+            mbar_expect_tx(bar, bytes + si.blob_words * 4u + 16u + kMaxStageRows * 16u);   // the arrival that lets the phase end
         }
     };
 

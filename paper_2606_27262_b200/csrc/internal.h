@@ -30,7 +30,9 @@ constexpr int kMaxStageGroups = 8;   // groups per stage
 constexpr int kChunkU = 128;         // variant words one warp builds per pre-sum task (4 per lane)
 constexpr int kBlobBytes = 3072;     // per-stage table blob (two buffers in shared memory)
 constexpr int kSmemBytes = 113 * 1024;                                   // two blocks per SM (228 KB incl. 1 KB each reserved)
-constexpr int kSmemCtrlBytes = 64 + kMaxDT * 16;                         // mbarrier, per-trial {row pointer, nout}
+constexpr int kMaxStageRows = kMaxStageGroups * kMaxG;                   // raw rows of one stage
+constexpr int kSmemCtrlBytes = 64 + kMaxDT * 16 + 2 * (kMaxStageRows * 16 + 16);  // mbarrier, per-trial {row pointer, nout},
+                                                                         // next stage's {RowDesc[], StageIndex} x 2
 constexpr int kSmemDataBytes = kSmemBytes - kSmemCtrlBytes - 2 * kBlobBytes;  // variant region + raw-row region
 
 // Per-stage blob, 32-bit words (copied to shared memory with one bulk copy):

@@ -364,6 +364,9 @@ int build_tiling(Plan& p) {
             td.nstage = (int32_t)rp.sidx.size() - td.stage0;
             rp.tiles.push_back(td);
         }
+        // a stage's transaction also fetches the NEXT stage's index and a fixed-size slice of its rows: pad the arrays
+        rp.sidx.push_back(StageIndex{0, 0, 0, 0});
+        rp.rows.resize(rp.rows.size() + kMaxStageRows, RowDesc{0, 0, 0, 0});
     }
     p.tiling_built = true;
     return SPT_OK;
