@@ -236,21 +236,35 @@ def run_ours(args, rank, world, local_rank):
     for kind, name in ((0, "iadd3"), (1, "imad"), (2, "iadd3+imad"), (3, "lds32"), (4, "lds128")):
         r, _ = api.probe(kind, 3)
         probe[name + "_warp_instr_per_s"] = r
-    # peak INT32 add rate = 64 lanes/SM/clk (one IADD3 per 2 clk per SM sub-partition,
-    # B300_MICROARCH.md "Pipe rates") x SMs x max SM clock, one add per instruction
-    peak_adds = 64.0 * nsm * sm_max * 1e6
+    # peak INT32 add rate of the chip = what the two integer pipes can retire together:
+    # ALU pipe 64 lanes/SM/clk of IADD3 (two 2-input adds each) + FMA pipe 64 lanes/SM/clk of IMAD (one add each)
+    # = 192 adds/SM/clk (B300_MICROARCH.md "Pipe rates"; both rates re-measured by the in-library probes in this run:
+    # kind 0 retires 2 counted adds per IADD3, kind 1 one per IMAD).  `peak` is the MEASURED sum.
+    iadd3_adds = probe["iadd3_warp_instr_per_s"] * 32      # counted adds/s (= 2 x IADD3 lanes/s)
+    imad_adds = probe["imad_warp_instr_per_s"] * 32
+    peak_adds = iadd3_adds + imad_adds
+    nominal_adds = 192.0 * nsm * sm_max * 1e6
     dom = ktimes.get((2, 0), [])
     dom_ms = sum(dom) / len(dom) if dom else None
     dom_adds = adds_of_range(plan, w.nchan, 0) * nbeam
     roof = None
     if dom_ms:
         achieved = dom_adds / (dom_ms * 1e-3)
-        roof = {"bound": "alu", "kernel": "dedisp_tiled_kernel (range 0)", "achieved": achieved / 1e12,
+        # the other leg of north_star's roofline: compulsory HBM bytes of the launch at the measured copy bandwidth
+        _, rg, _, nout, _ = plan.trial_table()
+        hbm_bytes = (w.nchan * w.nsamp + 4 * int(nout[rg == 0].astype("int64").sum())) * nbeam
+        hbm_gbs = float(peaks.get("hbm_gbs", 6650.0))
+        t_alu, t_hbm = dom_adds / peak_adds, hbm_bytes / (hbm_gbs * 1e9)
+        roof = {"bound": "alu", "kernel": "dedisp_tiled_kernel<uint8> (range 0)", "achieved": achieved / 1e12,
                 "peak": peak_adds / 1e12, "unit": "Tadd/s", "frac": achieved / peak_adds,
-                "peak_source": f"derived: 64 INT32 lanes/SM/clk x {nsm} SMs x {sm_max:.0f} MHz, 1 add per instruction",
-                "measured_iadd3_Tadd_per_s": probe["iadd3_warp_instr_per_s"] * 32 / 1e12,
-                "frac_of_measured_iadd3": achieved / (probe["iadd3_warp_instr_per_s"] * 32),
+                "peak_source": "measured in this run by spt_probe: IADD3 (ALU pipe, 2 adds each) %.1f + IMAD (FMA pipe) %.1f Tadd/s; "
+                               "nominal 192 adds/SM/clk x %d SMs x %.0f MHz = %.1f" %
+                               (iadd3_adds / 1e12, imad_adds / 1e12, nsm, sm_max, nominal_adds / 1e12),
+                "frac_of_one_add_per_lane_clk": achieved / (128.0 * nsm * sm_max * 1e6),
                 "launch_ms": dom_ms, "adds_per_launch": dom_adds,
+                "roofline_ms": {"alu": t_alu * 1e3, "hbm": t_hbm * 1e3, "hbm_peak_gbs": hbm_gbs,
+                                "hbm_peak_source": "MEASURED_PEAKS.json" if "hbm_gbs" in peaks else "fallback"},
+                "algorithmic_hbm_bytes": hbm_bytes,
                 "traffic": NCU_TRAFFIC_BYTES.get(w.index)}
     kernels = {f"kind{k}_range{r}": sum(v) / len(v) for (k, r), v in sorted(ktimes.items())}
 
@@ -267,7 +281,7 @@ def run_ours(args, rank, world, local_rank):
                        "parallelism": f"beams sharded over {world} GPU(s), no collective",
                        "l2": "inputs larger than L2 (filterbank %.0f MiB, DM transform %.0f MiB per beam)" %
                              (w.nchan * w.nsamp / 2**20, plan.dmt_elems_per_beam * 4 / 2**20),
-                       "group": args.group or 4, "dm_tile": args.dm_tile or 64},
+                       "group": args.group or 8, "dm_tile": args.dm_tile or 64},
             "rtf": rtf, "realtime_beams": rtf, "candidates": ncand, "overflowed": ovf,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h_fb.numel()),
                     "d2h_bytes_per_step": 8, "ms_per_step": 1e3 * e2e_s / steps,
