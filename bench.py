@@ -138,7 +138,7 @@ def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
 
-    from paper_2606_27262_b200 import api, build, synth
+    from paper_2606_27262_b200 import api, build, shard, synth
     build.build()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the path has no CPU fallback")
@@ -154,8 +154,8 @@ def run_ours(args, rank, world, local_rank):
     # seeded synthetic input of this rank, in pinned host memory (the e2e leg copies from it every step)
     h_fb = torch.empty((nbeam, w.nchan, w.nsamp), dtype=torch.uint8, pin_memory=True)
     hv = h_fb.numpy()
-    for b in range(nbeam):
-        synth.generate(w, beam=b if world == 1 else rank * nbeam + b, out=hv[b])
+    for b, gb in enumerate(shard.beams_of_rank(rank, world, nbeam)):   # every rank brings its own beams (weak scaling)
+        synth.generate(w, beam=gb, out=hv[b])
     cap = {1: 1 << 20, 2: 1 << 24, 3: 1 << 26, 4: 1 << 27, 5: 1 << 29}[w.index]
     opts = {"profile": 1}
     if args.group:
@@ -197,10 +197,7 @@ def run_ours(args, rank, world, local_rank):
     clocks = sampler.stop()
     ms_total = e0.elapsed_time(e1)
     launches = plan.launches() - launches0
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = shard.max_over_ranks(ms_total, device="cuda")
     value = adds_step * world * steps / (ms_total * 1e-3)
     data_s = nbeam * w.nsamp * w.tsamp
     rtf = data_s * world * steps / (ms_total * 1e-3)
@@ -214,10 +211,8 @@ def run_ours(args, rank, world, local_rank):
         plan.search_host(h_fb, w.threshold)
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    if world > 1:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+    e2e_s = shard.max_over_ranks(e2e_s, device="cuda")
+    ncand = shard.sum_over_ranks(ncand, device="cuda")
     e2e_value = adds_step * world * steps / e2e_s
 
     if rank != 0:
