@@ -1,11 +1,15 @@
 // sps.cu -- a4: boxcar single-pulse search over the DM transform (readings C1-C5, D1).
 //
 // One block per (beam, trial) row of N = nout samples:
-//   pass 1  Sx = sum x (int64), Sxx = sum x^2 (uint64): exact, order independent -> mu, sigma in double
-//   pass 2  segments of kSeg samples: block-wide inclusive prefix sum C (uint32, modulo 2^32) in shared memory,
-//           S_w[t] = C[t+w] - C[t];  snr_w[t] = (N*S_w[t] - w*Sx) / (N*sigma*sqrt(w))  (numerator exact int64);
+//   pass 1  Sx = sum x (int64), Sxx = sum x^2 (uint64), min, max: exact, order independent -> mu, sigma in double
+//   pass 2  (row now in L2) segments staged as prefix sums in shared memory, S_w[t] = C[t+w] - C[t];
+//           snr_w[t] = (N*S_w[t] - w*Sx) / (N*sigma*sqrt(w))  (numerator exact int64, scaled in double);
 //           best width per t scanned in increasing w with strict '>' ; best >= threshold -> warp-aggregated
 //           atomic append of {beam, trial, t, width, snr}.
+//   Fast path (taken when wmax * max|x - m| < 2^30, m = round(Sx/N)): prefix sums of x - m, so that a boxcar sum is a
+//   small exact int32 S' and  snr_w >= threshold  <=>  S' >= tau_w = (threshold*N*sigma*sqrt(w) + w*(Sx - N*m))/N.  Every
+//   (t, w) costs one LDS, one subtract and one add-max against the integer floor of tau_w; only samples that pass
+//   it run the evaluation above, which decides.  The exact path (any plan the ABI accepts) evaluates every (t, w).
 // HBM bound by design (one compulsory read of the DM transform; the second pass of a row re-reads it from L2).
 #include <cuda_runtime.h>
 
@@ -14,10 +18,17 @@
 namespace spt {
 
 constexpr int kSpsThreads = 512;
-constexpr int kEpt = 8;                        // samples per thread per segment
-constexpr int kSeg = kSpsThreads * kEpt;       // 4096 samples per segment (outputs + halo of the widest boxcar)
+constexpr int kSpsWarps = kSpsThreads / 32;
+constexpr int kIters = 5;                           // 128-element warp rows per warp per segment
+constexpr int kWarpSpan = kIters * 128;             // 640 consecutive elements per warp
+constexpr int kSegLoad = kSpsWarps * kWarpSpan;     // 10240 elements staged per segment (outputs + halo of the widest boxcar)
+constexpr int kCOff = 3;                            // s_c[kCOff + 1 + e] = inclusive prefix through element e (16-byte aligned rows)
+constexpr int kEpt = 8;                             // outputs per thread per sub-block of the fast path
+// exact path geometry (kept from the first kernel): 8 samples per thread per segment
+constexpr int kXEpt = 8;
+constexpr int kXSeg = kSpsThreads * kXEpt;
 
-__device__ __forceinline__ int padi(int i) { return i + (i >> 5); }  // bank-conflict-free stride-8 access
+__device__ __forceinline__ int padi(int i) { return i + (i >> 5); }  // bank-conflict-free stride-8 access (exact path)
 
 __device__ __forceinline__ long long shfl_down_ll(long long v, int d) {
     int lo = (int)(v & 0xffffffffll), hi = (int)(v >> 32);
@@ -26,14 +37,53 @@ __device__ __forceinline__ long long shfl_down_ll(long long v, int d) {
     return ((long long)hi << 32) | (unsigned int)lo;
 }
 
-__global__ void __launch_bounds__(kSpsThreads) sps_kernel(const SpsArgs a) {
-    __shared__ uint32_t s_c[kSeg + 1 + (kSeg + 1) / 32 + 1];
-    __shared__ long long s_red[2][kSpsThreads / 32];
-    __shared__ uint32_t s_wtot[kSpsThreads / 32];
-    __shared__ double s_scale[kMaxWidths];
-    __shared__ long long s_wsum[kMaxWidths];
-    __shared__ int s_live;
+struct SpsShared {
+    uint32_t c[kSegLoad + 8];                       // prefix sums of the staged segment
+    long long red[2][kSpsWarps];
+    int redmin[kSpsWarps], redmax[kSpsWarps];
+    uint32_t wtot[kSpsWarps];
+    double scale[kMaxWidths];                       // 1 / (N sigma sqrt(w))
+    long long wsum[kMaxWidths];                     // exact path: w*Sx ; fast path: w*(Sx - N*m)
+    int negT[kMaxWidths];                           // fast path: -floor(tau_w), clamped to +-2^30
+    long long S;
+    unsigned long long Q;
+    int live, fast, m, nw_eff;
+};
 
+// Full evaluation of one sample (readings C3-C5): widths in increasing order, strict '>', numerator exact.
+// sp(k) returns the boxcar sum minus w*m' (m' = 0 on the exact path) as a signed 64-bit integer.
+template <typename F>
+__device__ __forceinline__ bool best_of(const SpsShared& sh, const SpsArgs& a, int t, int n, long long N64, F sp, double& best, int& bw) {
+    bool first = true;
+    best = 0.0; bw = a.widths[0];
+    for (int k = 0; k < sh.nw_eff; ++k) {
+        const int w = a.widths[k];
+        if (t + w > n) break;
+        const long long num = N64 * sp(k, w) - sh.wsum[k];            // exact int64
+        const double snr = (double)num * sh.scale[k];
+        if (first || snr > best) { best = snr; bw = w; first = false; }
+    }
+    return !first && best >= a.threshold;
+}
+
+__device__ __forceinline__ void append(const SpsArgs& a, bool hit, int b, int d, int t, int bw, double best, int lane) {
+    const unsigned m = __ballot_sync(0xffffffffu, hit);
+    if (!m) return;
+    unsigned long long slot0 = 0;
+    if (lane == 0) slot0 = atomicAdd(a.count, (unsigned long long)__popc(m));
+    slot0 = __shfl_sync(0xffffffffu, slot0, 0);
+    if (hit) {
+        const long long slot = (long long)(slot0 + __popc(m & ((1u << lane) - 1u)));
+        if (slot < a.capacity) {
+            spt_candidate c;
+            c.beam = b; c.trial = d; c.t = t; c.width = bw; c.snr = (float)best;
+            a.cand[slot] = c;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
+    __shared__ __align__(16) SpsShared sh;
     const int d = blockIdx.x, b = blockIdx.y;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n = a.nout[d];
@@ -43,10 +93,11 @@ __global__ void __launch_bounds__(kSpsThreads) sps_kernel(const SpsArgs a) {
     }
     const int32_t* x = a.dmt + (int64_t)b * a.beam_stride + a.offset[d];  // 128-byte aligned row
 
-    // ---- pass 1: exact integer statistics (reading C1) --------------------------------------------------------
-    long long sx = 0;
-    unsigned long long sxx = 0;
+    // ---- pass 1: exact integer statistics (reading C1), and the range of the row --------------------------------
     {
+        long long sx = 0;
+        unsigned long long sxx = 0;
+        int mn = 0x7fffffff, mx = (int)0x80000000;
         const int n4 = n >> 2;
         const int4* x4 = reinterpret_cast<const int4*>(x);
         for (int i = tid; i < n4; i += kSpsThreads) {
@@ -54,24 +105,31 @@ __global__ void __launch_bounds__(kSpsThreads) sps_kernel(const SpsArgs a) {
             sx += (long long)v.x + v.y + v.z + v.w;
             sxx += (unsigned long long)(unsigned)v.x * (unsigned)v.x + (unsigned long long)(unsigned)v.y * (unsigned)v.y +
                    (unsigned long long)(unsigned)v.z * (unsigned)v.z + (unsigned long long)(unsigned)v.w * (unsigned)v.w;
+            mn = min(min(mn, v.x), min(v.y, min(v.z, v.w)));
+            mx = max(max(mx, v.x), max(v.y, max(v.z, v.w)));
         }
         for (int i = (n4 << 2) + tid; i < n; i += kSpsThreads) {
             const int v = x[i];
             sx += v;
             sxx += (unsigned long long)(unsigned)v * (unsigned)v;
+            mn = min(mn, v); mx = max(mx, v);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             sx += shfl_down_ll(sx, o);
             sxx += (unsigned long long)shfl_down_ll((long long)sxx, o);
+            mn = min(mn, __shfl_down_sync(0xffffffffu, mn, o));
+            mx = max(mx, __shfl_down_sync(0xffffffffu, mx, o));
         }
-        if (lane == 0) { s_red[0][warp] = sx; s_red[1][warp] = (long long)sxx; }
+        if (lane == 0) { sh.red[0][warp] = sx; sh.red[1][warp] = (long long)sxx; sh.redmin[warp] = mn; sh.redmax[warp] = mx; }
         __syncthreads();
-        if (tid == 0) {
+        if (tid < kMaxWidths) {       // every one of these threads derives the row constants; thread k keeps width k's
             long long S = 0; unsigned long long Q = 0;
-            for (int w = 0; w < kSpsThreads / 32; ++w) { S += s_red[0][w]; Q += (unsigned long long)s_red[1][w]; }
-            a.sum[(int64_t)b * a.ntrials + d] = S;
-            a.sumsq[(int64_t)b * a.ntrials + d] = Q;
+            int rmn = 0x7fffffff, rmx = (int)0x80000000;
+            for (int w = 0; w < kSpsWarps; ++w) {
+                S += sh.red[0][w]; Q += (unsigned long long)sh.red[1][w];
+                rmn = min(rmn, sh.redmin[w]); rmx = max(rmx, sh.redmax[w]);
+            }
             // sigma^2 = (N*Sxx - Sx^2)/N^2 from 128-bit integers (N*Sxx reaches ~1e23)
             const unsigned long long N = (unsigned long long)n, US = (unsigned long long)S;
             const unsigned long long alo = N * Q, ahi = __umul64hi(N, Q);
@@ -81,94 +139,169 @@ __global__ void __launch_bounds__(kSpsThreads) sps_kernel(const SpsArgs a) {
             const double num = (double)dhi * 18446744073709551616.0 + (double)dlo;
             const double sigma = sqrt(num / ((double)n * (double)n));
             const int live = (sigma > 0.0 && n >= 2) ? 1 : 0;
-            s_live = live;
-            for (int k = 0; k < a.nw; ++k) {
-                const double w = (double)a.widths[k];
-                s_scale[k] = live ? 1.0 / (((double)n * sigma) * sqrt(w)) : 0.0;
-                s_wsum[k] = (long long)a.widths[k] * S;
+            // integer mean and the fast-path test: every boxcar sum of x - m stays below 2^30 in magnitude
+            const long long m = (2 * S + (long long)n) / (2 * (long long)n);             // S >= 0: round half up
+            const long long dev = max((long long)rmx - m, m - (long long)rmn);
+            const int wmax = a.widths[a.nw - 1];
+            const int fast = (dev * (long long)min(wmax, n) < (1ll << 30)) ? 1 : 0;
+            const long long r = S - (long long)n * m;                                    // |r| <= N/2
+            if (tid == 0) {
+                a.sum[(int64_t)b * a.ntrials + d] = S;
+                a.sumsq[(int64_t)b * a.ntrials + d] = Q;
+                sh.S = S; sh.Q = Q; sh.live = live; sh.fast = fast; sh.m = (int)m;
+                int ne = 0;
+                while (ne < a.nw && a.widths[ne] <= n) ++ne;                             // widths > N never apply
+                sh.nw_eff = ne;
+            }
+            if (tid < a.nw) {
+                const double w = (double)a.widths[tid];
+                const double nsig = ((double)n * sigma) * sqrt(w);
+                sh.scale[tid] = live ? 1.0 / nsig : 0.0;
+                sh.wsum[tid] = (long long)a.widths[tid] * (fast ? r : S);
+                // tau_w = (threshold*N*sigma*sqrt(w) + w*r)/N ; the integer test uses a floor that can only be too low
+                double tau = (a.threshold * nsig + (double)((long long)a.widths[tid] * r)) / (double)n;
+                tau = floor(tau - fabs(tau) * 1e-9 - 1e-6);
+                tau = fmin(fmax(tau, -1073741824.0), 1073741824.0);
+                sh.negT[tid] = -(int)tau;
             }
         }
         __syncthreads();
     }
-    if (!s_live) return;  // sigma == 0 or N < 2: S/N == 0 everywhere, no candidates (reading C1)
+    if (!sh.live) return;  // sigma == 0 or N < 2: S/N == 0 everywhere, no candidates (reading C1)
 
-    // ---- pass 2: boxcars, best width, threshold ------------------------------------------------------------------
     const int w0 = a.widths[0], wmax = a.widths[a.nw - 1];
     const int nbest = n - w0 + 1;              // best[t] is defined for t in [0, N - wmin]  (reading C5)
     if (nbest <= 0) return;
     const int halo = min(wmax, n);             // widths > N never apply
-    const int adv = (kSeg - halo) & ~31;       // outputs per segment (launch_sps guarantees wmax <= kSeg - 32)
     const long long N64 = n;
 
-    for (int tb = 0; tb < nbest; tb += adv) {
-        // load kEpt consecutive samples per thread (coalesced via shared memory), zero beyond N
-        __syncthreads();
-        for (int i = tid; i < kSeg; i += kSpsThreads) {
-            const int t = tb + i;
-            s_c[padi(i + 1)] = t < n ? (uint32_t)x[t] : 0u;
-        }
-        __syncthreads();
-        uint32_t v[kEpt];
-        uint32_t run = 0;
+    if (sh.fast) {
+        // ---- pass 2, fast path ---------------------------------------------------------------------------------------
+        const int m = sh.m;
+        const int nw_eff = sh.nw_eff;
+        const int adv = (kSegLoad - halo) & ~3;                 // outputs per segment (launch_sps: wmax <= kXSeg - 32)
+        for (int tb = 0; tb < nbest; tb += adv) {
+            __syncthreads();                                    // the previous segment's readers are done
+            // stage x - m: warp `warp` owns elements [warp*640, +640) of the segment; zero beyond N
+            int4 v[kIters];
+            int tot = 0;
 #pragma unroll
-        for (int i = 0; i < kEpt; ++i) { run += s_c[padi(tid * kEpt + i + 1)]; v[i] = run; }
-        uint32_t incl = run;
+            for (int it = 0; it < kIters; ++it) {
+                const int e = tb + warp * kWarpSpan + it * 128 + lane * 4;
+                if (e + 4 <= n) {
+                    v[it] = *reinterpret_cast<const int4*>(x + e);
+                    v[it].x -= m; v[it].y -= m; v[it].z -= m; v[it].w -= m;
+                } else {
+                    v[it].x = e < n ? x[e] - m : 0;
+                    v[it].y = e + 1 < n ? x[e + 1] - m : 0;
+                    v[it].z = e + 2 < n ? x[e + 2] - m : 0;
+                    v[it].w = 0;
+                }
+                tot += v[it].x + v[it].y + v[it].z + v[it].w;
+            }
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += y;
+            for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
+            if (lane == 0) sh.wtot[warp] = (uint32_t)tot;
+            __syncthreads();
+            uint32_t run = 0;
+            for (int w = 0; w < warp; ++w) run += sh.wtot[w];   // exclusive offset of this warp
+#pragma unroll
+            for (int it = 0; it < kIters; ++it) {
+                const uint32_t p0 = (uint32_t)v[it].x, p1 = p0 + (uint32_t)v[it].y, p2 = p1 + (uint32_t)v[it].z,
+                               p3 = p2 + (uint32_t)v[it].w;
+                uint32_t incl = p3;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+                    if (lane >= o) incl += y;
+                }
+                const uint32_t base = run + incl - p3;
+                *reinterpret_cast<uint4*>(&sh.c[kCOff + 1 + warp * kWarpSpan + it * 128 + lane * 4]) =
+                    make_uint4(base + p0, base + p1, base + p2, base + p3);
+                run += __shfl_sync(0xffffffffu, incl, 31);
+            }
+            if (tid == 0) sh.c[kCOff] = 0u;
+            __syncthreads();
+
+            // S'_w[i] = c[kCOff + i + w] - c[kCOff + i]   (i relative to the segment)
+            const int nthis = min(adv, nbest - tb);
+            for (int i0 = 0; i0 < nthis; i0 += kSpsThreads * kEpt) {
+                int idx[kEpt], mxv[kEpt];
+                uint32_t c0[kEpt];
+#pragma unroll
+                for (int e = 0; e < kEpt; ++e) {
+                    idx[e] = min(i0 + e * kSpsThreads + tid, nthis - 1);    // clamped: out-of-range slots repeat the last one
+                    c0[e] = sh.c[kCOff + idx[e]];
+                    mxv[e] = (int)0x80000000;
+                }
+                for (int k = 0; k < nw_eff; ++k) {
+                    const int w = a.widths[k], nT = sh.negT[k];
+#pragma unroll
+                    for (int e = 0; e < kEpt; ++e)
+                        mxv[e] = max(mxv[e], (int)(sh.c[kCOff + idx[e] + w] - c0[e]) + nT);
+                }
+#pragma unroll
+                for (int e = 0; e < kEpt; ++e) {
+                    const int i = i0 + e * kSpsThreads + tid;
+                    const bool pre = i < nthis && mxv[e] >= 0;
+                    if (!__any_sync(0xffffffffu, pre)) continue;
+                    bool hit = false;
+                    double best = 0.0;
+                    int bw = w0;
+                    const int t = tb + i;
+                    if (pre)
+                        hit = best_of(sh, a, t, n, N64, [&](int, int w) { return (long long)(int)(sh.c[kCOff + i + w] - sh.c[kCOff + i]); },
+                                      best, bw);
+                    append(a, hit, b, d, t, bw, best, lane);
+                }
+            }
         }
-        if (lane == 31) s_wtot[warp] = incl;
-        __syncthreads();
-        if (warp == 0) {
-            uint32_t wt = lane < kSpsThreads / 32 ? s_wtot[lane] : 0u;
+        return;
+    }
+
+    // ---- pass 2, exact path: every (t, w) evaluated from unsigned prefix sums of x itself ----------------------------
+    {
+        uint32_t* s_c = sh.c;                      // padi() layout, kXSeg + 1 entries
+        const int adv = (kXSeg - halo) & ~31;      // outputs per segment (plan check: wmax <= kXSeg - 32)
+        for (int tb = 0; tb < nbest; tb += adv) {
+            // load kXEpt consecutive samples per thread (coalesced via shared memory), zero beyond N
+            __syncthreads();
+            for (int i = tid; i < kXSeg; i += kSpsThreads) {
+                const int t = tb + i;
+                s_c[padi(i + 1)] = t < n ? (uint32_t)x[t] : 0u;
+            }
+            __syncthreads();
+            uint32_t v[kXEpt];
+            uint32_t run = 0;
+#pragma unroll
+            for (int i = 0; i < kXEpt; ++i) { run += s_c[padi(tid * kXEpt + i + 1)]; v[i] = run; }
+            uint32_t incl = run;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
-                const uint32_t y = __shfl_up_sync(0xffffffffu, wt, o);
-                if (lane >= o) wt += y;
+                const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += y;
             }
-            if (lane < kSpsThreads / 32) s_wtot[lane] = wt;  // inclusive over warps
-        }
-        __syncthreads();
-        const uint32_t base = (incl - run) + (warp > 0 ? s_wtot[warp - 1] : 0u);
+            if (lane == 31) sh.wtot[warp] = incl;
+            __syncthreads();
+            uint32_t woff = 0;
+            for (int w = 0; w < warp; ++w) woff += sh.wtot[w];
+            const uint32_t base = (incl - run) + woff;
 #pragma unroll
-        for (int i = 0; i < kEpt; ++i) s_c[padi(tid * kEpt + i + 1)] = base + v[i];
-        if (tid == 0) s_c[0] = 0u;
-        __syncthreads();
+            for (int i = 0; i < kXEpt; ++i) s_c[padi(tid * kXEpt + i + 1)] = base + v[i];
+            if (tid == 0) s_c[0] = 0u;
+            __syncthreads();
 
-        const int nthis = min(adv, nbest - tb);
-        for (int i0 = 0; i0 < nthis; i0 += kSpsThreads) {
-            const int i = i0 + tid;
-            const int t = tb + i;
-            bool hit = false;
-            double best = 0.0;
-            int bw = w0;
-            if (i < nthis) {
-                const uint32_t c0 = s_c[padi(i)];
-                bool first = true;
-                for (int k = 0; k < a.nw; ++k) {
-                    const int w = a.widths[k];
-                    if (t + w > n) break;
-                    const uint32_t S = s_c[padi(i + w)] - c0;                       // exact: S < 2^32 (plan check)
-                    const long long num = N64 * (long long)S - s_wsum[k];           // exact int64
-                    const double snr = (double)num * s_scale[k];
-                    if (first || snr > best) { best = snr; bw = w; first = false; }
-                }
-                hit = best >= a.threshold;
-            }
-            const unsigned m = __ballot_sync(0xffffffffu, hit);
-            if (m) {
-                unsigned long long slot0 = 0;
-                if (lane == 0) slot0 = atomicAdd(a.count, (unsigned long long)__popc(m));
-                slot0 = __shfl_sync(0xffffffffu, slot0, 0);
-                if (hit) {
-                    const long long slot = (long long)(slot0 + __popc(m & ((1u << lane) - 1u)));
-                    if (slot < a.capacity) {
-                        spt_candidate c;
-                        c.beam = b; c.trial = d; c.t = t; c.width = bw; c.snr = (float)best;
-                        a.cand[slot] = c;
-                    }
-                }
+            const int nthis = min(adv, nbest - tb);
+            for (int i0 = 0; i0 < nthis; i0 += kSpsThreads) {
+                const int i = i0 + tid;
+                const int t = tb + i;
+                bool hit = false;
+                double best = 0.0;
+                int bw = w0;
+                if (i < nthis)
+                    hit = best_of(sh, a, t, n, N64, [&](int, int w) { return (long long)(uint32_t)(s_c[padi(i + w)] - s_c[padi(i)]); },
+                                  best, bw);                          // exact: S < 2^32 (plan check)
+                append(a, hit, b, d, t, bw, best, lane);
             }
         }
     }

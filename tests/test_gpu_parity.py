@@ -163,6 +163,25 @@ def test_all255_wide_band_lane_limits(cuda, api, orc):
     assert dmt.max() == 4096 * 255 * 4
 
 
+def test_square_wave_takes_the_exact_search_path(cuda, api, orc):
+    """Rows whose samples sit 2e6 counts from their mean with a 1024-wide boxcar: boxcar sums of x - mean do not fit
+    the fast path's int32 test (wmax * max|x - m| >= 2^30), so the search kernel must take its exact path."""
+    w = Shape(500.0, -0.048828125, 4096, 8192, [(0.0, 0.2, 12, 1), (0.0, 1.0, 12, 4)], [1, 4, 64, 1024], 1.5)
+    t = np.arange(w.nsamp)
+    fb = np.where((t // 96) % 2 == 0, 255, 0).astype(np.uint8)[None, :].repeat(w.nchan, axis=0)
+    fb[::7, 5000:5003] = 17
+    ref = oracle_path(orc, w, fb)
+    ncand = sum(int(r.search.candoff[-1]) for r in ref)
+    assert ncand > 1000
+    plan, dmt, cands = run_gpu(cuda, api, w, fb[None], cand_capacity=ncand + 4096)
+    check_dmt_against_oracle(plan, dmt, ref)
+    check_stats_against_oracle(plan, ref)
+    st = check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+    assert st["matched"] >= st["oracle"] - st["near_threshold_only_oracle"]
+    row = dmt[0][: 100]
+    assert int(row.max()) - int(row.min()) > (1 << 20)          # the premise: deviations of order 1e6
+
+
 # ---- config 2 at reduced length -----------------------------------------------------------------------------------
 def test_cfg2_reduced(cuda, api, orc, synth):
     w = synth.workload(2, nsamp=16384)
