@@ -28,8 +28,8 @@ METRIC = "DM-trial*chan*samples/s and real-time beams per B200 (dedisp + boxcar 
 UNIT = "DM-trial*chan*samples/s"
 
 # DRAM bytes per launch of the dominant kernel (dedisp_tiled, range 0 of config 3) from the committed
-# `ncu --set full` capture (profiles/): dram__bytes_read.sum + dram__bytes_write.sum.  None until captured.
-NCU_TRAFFIC_BYTES = {3: None}
+# `ncu --set full` capture (profiles/): dram__bytes_read.sum + dram__bytes_write.sum.
+NCU_TRAFFIC_BYTES = {3: 4284057000}   # profiles/r01_v33_summary.md: 1.04 GB read + 3.25 GB written
 
 
 def algorithmic_adds(plan, nchan):
@@ -62,7 +62,7 @@ class ClockSampler(threading.Thread):
                     self.rows.append(f)
             except Exception:
                 pass
-            self._stop_evt.wait(0.2)
+            self._stop_evt.wait(0.05)
 
     def stop(self):
         self._stop_evt.set()
@@ -86,7 +86,7 @@ def oracle_sample(w, fb, seconds_target=20.0):
     import oracle
     oracle.build()
     cores = oracle.num_threads()
-    per_range = {1: 96, 2: 64, 4: 64}
+    per_range = {1: 480, 2: 320, 4: 320}      # about 10 s of oracle work on 16 host threads
     t_total, adds, picked = 0.0, 0, []
     for (lo, step, ndm, k) in w.ranges:
         n = min(ndm, per_range.get(k, 16))
@@ -291,7 +291,7 @@ def run_ours(args, rank, world, local_rank):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
