@@ -79,14 +79,16 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.rows), "reasons": sorted(reasons)}
 
 
-def oracle_sample(w, fb, seconds_target=20.0):
+def oracle_sample(w, fb, seconds_target=10.0):
     """The oracle, as it stands, on a bounded sample of the same workload: a few trials of every range dedispersed
     and searched on the host cores.  Returns (adds per second, cores, description)."""
     import numpy as np
     import oracle
     oracle.build()
     cores = oracle.num_threads()
-    per_range = {1: 480, 2: 320, 4: 320}      # about 10 s of oracle work on 16 host threads
+    # 96 / 64 / 64 trials of the three ranges take about 2 s on 16 host threads; scaled to the target
+    f = max(0.25, seconds_target / 2.0)
+    per_range = {1: int(96 * f), 2: int(64 * f), 4: int(64 * f)}
     t_total, adds, picked = 0.0, 0, []
     for (lo, step, ndm, k) in w.ranges:
         n = min(ndm, per_range.get(k, 16))
@@ -118,7 +120,8 @@ def run_reference(args, rank, world):
     rate, cores, sample = 0.0, 1, ""
     t_sum, adds_sum = 0.0, 0.0
     for i in range(warm + steps):
-        r, cores, sample, t, adds = oracle_sample(w, fb)   # each step is the same bounded sample
+        # each step is the same bounded sample, sized so that the whole run ends within a few minutes
+        r, cores, sample, t, adds = oracle_sample(w, fb, seconds_target=min(10.0, 150.0 / (steps + warm)))
         if i >= warm:
             t_sum += t
             adds_sum += adds
