@@ -168,6 +168,21 @@ int spt_candidates_read(spt_plan* plan, spt_candidate* host_out, int64_t cap, in
 int spt_search_host(spt_plan* plan, const uint8_t* h_fb, int32_t nbeam, float threshold, int32_t* h_dmt,
                     int64_t* ncand, int32_t* overflowed);
 
+/* -------------------------------------------------------------------------------------------------------
+ * Streaming form of spt_search_host: a two-deep pipeline in which the H2D copy of one batch runs on the copy engine
+ * while the kernels of the previous batch run (the search consumes a continuous stream of blocks).
+ *   spt_stream_push: enqueue {H2D of h_fb, decimation, dedispersion, search, count readback} and return at once.
+ *       h_fb (HOST, pinned for a truly asynchronous copy) must stay valid and unchanged until the matching pop.
+ *       At most two batches may be in flight: a third push returns SPT_ERR_STATE.
+ *   spt_stream_pop: wait for the OLDEST batch in flight; ncand / overflowed as in spt_search_host.  Until the next push
+ *       (which reuses this batch's buffers), spt_candidates_read / spt_candidates_count / spt_trial_stats* refer to this
+ *       batch, while the other batch keeps running (the two batches in flight have their own lists and statistics; the DM
+ *       transform buffer is shared and not kept).  SPT_ERR_STATE if nothing is in flight.
+ * Results are identical to spt_search_host on the same input.
+ * ----------------------------------------------------------------------------------------------------- */
+int spt_stream_push(spt_plan* plan, const uint8_t* h_fb /*HOST*/, int32_t nbeam, float threshold);
+int spt_stream_pop(spt_plan* plan, int64_t* ncand, int32_t* overflowed);
+
 /* With option "profile" = 1: device time (ms) of each kernel launched by the LAST spt_dedisperse and the LAST
  * spt_single_pulse_search, in launch order; kinds: 1 = decimate, 2 = dedisperse, 3 = single-pulse search; `range` is the
  * DM range the launch served (-1 for the search).  Synchronises.  Arrays (HOST) hold `cap` entries; n = entries written. */

@@ -54,6 +54,8 @@ SYMBOLS = {
     "spt_candidates_count": (ctypes.c_int, [_vp, _P(_i64), _P(_i32)]),
     "spt_candidates_read": (ctypes.c_int, [_vp, _vp, _i64, _P(_i64)]),
     "spt_search_host": (ctypes.c_int, [_vp, _vp, _i32, _f32, _vp, _P(_i64), _P(_i32)]),
+    "spt_stream_push": (ctypes.c_int, [_vp, _vp, _i32, _f32]),
+    "spt_stream_pop": (ctypes.c_int, [_vp, _P(_i64), _P(_i32)]),
     "spt_plan_kernel_times": (ctypes.c_int, [_vp, _i32, _vp, _vp, _vp, _P(_i32)]),
     "spt_plan_launches": (ctypes.c_int, [_vp, _P(_i64)]),
     "spt_probe": (ctypes.c_int, [_i32, _i32, _P(_f64), _P(_f64)]),
@@ -239,6 +241,17 @@ class Plan:
         n, o = ctypes.c_int64(), ctypes.c_int32()
         _check(lib().spt_search_host(self._h, ptr, nbeam, float(threshold), dptr, ctypes.byref(n), ctypes.byref(o)),
                "spt_search_host")
+        return int(n.value), bool(o.value)
+
+    def stream_push(self, h_fb, threshold: float):
+        """Enqueue one batch (HOST uint8 [nbeam][nchan][nsamp], pinned) into the two-deep pipeline; returns at once."""
+        ptr, nbeam = _host_ptr_and_beams(h_fb, self.nchan, self.nsamp)
+        _check(lib().spt_stream_push(self._h, ptr, nbeam, float(threshold)), "spt_stream_push")
+
+    def stream_pop(self):
+        """Wait for the oldest batch in flight; returns (ncand, overflowed)."""
+        n, o = ctypes.c_int64(), ctypes.c_int32()
+        _check(lib().spt_stream_pop(self._h, ctypes.byref(n), ctypes.byref(o)), "spt_stream_pop")
         return int(n.value), bool(o.value)
 
     def kernel_times(self):

@@ -38,10 +38,26 @@ struct DeviceState {
     std::vector<RangeDev> r;
     int32_t* nout = nullptr;        // [ntrials]
     int64_t* offset = nullptr;      // [ntrials]
-    int64_t* sum = nullptr;         // [max_beams][ntrials]
-    unsigned long long* sumsq = nullptr;
-    spt_candidate* cand = nullptr;
-    unsigned long long* count = nullptr;
+    // results of a search: statistics [max_beams][ntrials], candidate list, exact count.  Set 0 serves the plain calls;
+    // the streaming calls (spt_stream_push/pop) alternate between set 0 and a lazily allocated set 1.
+    struct SearchBufs {
+        int64_t* sum = nullptr;
+        unsigned long long* sumsq = nullptr;
+        spt_candidate* cand = nullptr;
+        unsigned long long* count = nullptr;
+    } bufs[2];
+    int cur = 0;                    // the set the read-out calls look at
+    // streaming pipeline (two batches in flight)
+    struct Slot {
+        uint8_t* fb = nullptr;                  // device copy of the batch's filterbank
+        unsigned long long* h_count = nullptr;  // pinned host word the count lands in
+        cudaEvent_t copied = nullptr, done = nullptr;
+        int32_t nbeam = 0;
+        bool pending = false;
+    } slot[2];
+    int push_next = 0, pop_next = 0;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t wait_event = nullptr;   // when set, read-out calls wait for this event instead of the whole stream
     uint8_t* fb_pad = nullptr;      // aligned copy of an input whose rows are not 16-byte multiples
     int64_t fb_pad_stride = 0;
     uint8_t* h_fb = nullptr;        // spt_search_host: device copy of the host filterbank
@@ -93,13 +109,32 @@ static void free_device(Plan* p) {
         cudaFree(r.delay); cudaFree(r.tiles); cudaFree(r.sidx); cudaFree(r.rows); cudaFree(r.blob);
         cudaFree(r.series);
     }
-    cudaFree(d->nout); cudaFree(d->offset); cudaFree(d->sum); cudaFree(d->sumsq);
-    cudaFree(d->cand); cudaFree(d->count); cudaFree(d->fb_pad); cudaFree(d->h_fb); cudaFree(d->h_dmt);
+    cudaFree(d->nout); cudaFree(d->offset);
+    for (auto& b : d->bufs) { cudaFree(b.sum); cudaFree(b.sumsq); cudaFree(b.cand); cudaFree(b.count); }
+    for (auto& sl : d->slot) {
+        cudaFree(sl.fb);
+        if (sl.h_count) cudaFreeHost(sl.h_count);
+        if (sl.copied) cudaEventDestroy(sl.copied);
+        if (sl.done) cudaEventDestroy(sl.done);
+    }
+    cudaFree(d->fb_pad); cudaFree(d->h_fb); cudaFree(d->h_dmt);
     if (d->own_stream) cudaStreamDestroy(d->own_stream);
+    if (d->copy_stream) cudaStreamDestroy(d->copy_stream);
     timed_clear(d, 0); timed_clear(d, 1);
     for (cudaEvent_t e : d->event_pool) cudaEventDestroy(e);
     delete d;
     p->dev = nullptr;
+}
+
+static int alloc_search_bufs(Plan* p, DeviceState::SearchBufs& b) {
+    const size_t n = (size_t)p->max_beams * p->ntrials;
+    cudaError_t ce = cudaMalloc((void**)&b.sum, n * 8);
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&b.sumsq, n * 8);
+    if (ce == cudaSuccess) ce = cudaMalloc((void**)&b.count, 8);
+    if (ce == cudaSuccess) ce = cudaMemset(b.count, 0, 8);
+    if (ce == cudaSuccess && p->cand_capacity > 0)
+        ce = cudaMalloc((void**)&b.cand, (size_t)p->cand_capacity * sizeof(spt_candidate));
+    return ce == cudaSuccess ? SPT_OK : cuda_fail(ce, "search buffers");
 }
 
 static int ensure_device(Plan* p) {
@@ -140,16 +175,10 @@ static int ensure_device(Plan* p) {
     }
     if (rc == SPT_OK) rc = upload(&d->nout, nout_all);
     if (rc == SPT_OK) rc = upload(&d->offset, off_all);
+    if (rc == SPT_OK) rc = alloc_search_bufs(p, d->bufs[0]);
     if (rc == SPT_OK) {
-        const size_t n = (size_t)p->max_beams * p->ntrials;
-        cudaError_t ce = cudaMalloc((void**)&d->sum, n * 8);
-        if (ce == cudaSuccess) ce = cudaMalloc((void**)&d->sumsq, n * 8);
-        if (ce == cudaSuccess) ce = cudaMalloc((void**)&d->count, 8);
-        if (ce == cudaSuccess) ce = cudaMemset(d->count, 0, 8);
-        if (ce == cudaSuccess && p->cand_capacity > 0)
-            ce = cudaMalloc((void**)&d->cand, (size_t)p->cand_capacity * sizeof(spt_candidate));
-        if (ce == cudaSuccess) ce = cudaStreamCreateWithFlags(&d->own_stream, cudaStreamNonBlocking);
-        if (ce != cudaSuccess) rc = cuda_fail(ce, "plan buffers");
+        cudaError_t ce = cudaStreamCreateWithFlags(&d->own_stream, cudaStreamNonBlocking);
+        if (ce != cudaSuccess) rc = cuda_fail(ce, "plan stream");
     }
     if (rc != SPT_OK) free_device(p);
     return rc;
@@ -213,9 +242,10 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
     return SPT_OK;
 }
 
-static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float threshold, cudaStream_t st) {
+static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float threshold, cudaStream_t st, int set = 0) {
     DeviceState* d = p->dev;
-    SPT_CUDA(cudaMemsetAsync(d->count, 0, 8, st));
+    const DeviceState::SearchBufs& bf = d->bufs[set];
+    SPT_CUDA(cudaMemsetAsync(bf.count, 0, 8, st));
     SpsArgs a{};
     a.dmt = d_dmt;
     a.beam_stride = p->dmt_elems;
@@ -225,10 +255,10 @@ static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float thresho
     a.nw = (int32_t)p->widths.size();
     for (int i = 0; i < a.nw; ++i) a.widths[i] = p->widths[i];
     a.threshold = (double)threshold;
-    a.sum = d->sum;
-    a.sumsq = d->sumsq;
-    a.cand = d->cand;
-    a.count = d->count;
+    a.sum = bf.sum;
+    a.sumsq = bf.sumsq;
+    a.cand = bf.cand;
+    a.count = bf.count;
     a.capacity = p->cand_capacity;
     timed_clear(d, 1);
     {
@@ -240,6 +270,16 @@ static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float thresho
     d->last_stream = st;
     d->nbeam_search = nbeam;
     d->searched = true;
+    d->cur = set;
+    d->wait_event = nullptr;
+    return SPT_OK;
+}
+
+// Read-out calls wait for the results they look at: the whole stream of the last plain call, or the completion event of the
+// batch spt_stream_pop returned last (later batches may still be running).
+static int sync_results(DeviceState* d) {
+    if (d->wait_event) SPT_CUDA(cudaEventSynchronize(d->wait_event));
+    else SPT_CUDA(cudaStreamSynchronize(d->last_stream));
     return SPT_OK;
 }
 
@@ -522,13 +562,13 @@ int spt_trial_stats(spt_plan* plan, int32_t beam, int32_t trial, int64_t* n, int
     Plan& p = plan->p;
     if (!p.dev || !p.dev->searched) return SPT_ERR_STATE;
     if (beam < 0 || beam >= p.dev->nbeam_search || trial < 0 || trial >= p.ntrials) return SPT_ERR_SHAPE;
-    SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
+    { const int rc = sync_results(p.dev); if (rc != SPT_OK) return rc; }
     int32_t loc = 0;
     const RangePlan* rp = range_of_trial(p, trial, &loc);
     if (n) *n = rp->nout[loc];
     const size_t idx = (size_t)beam * p.ntrials + trial;
-    if (sum) SPT_CUDA(cudaMemcpy(sum, p.dev->sum + idx, 8, cudaMemcpyDeviceToHost));
-    if (sumsq) SPT_CUDA(cudaMemcpy(sumsq, p.dev->sumsq + idx, 8, cudaMemcpyDeviceToHost));
+    if (sum) SPT_CUDA(cudaMemcpy(sum, p.dev->bufs[p.dev->cur].sum + idx, 8, cudaMemcpyDeviceToHost));
+    if (sumsq) SPT_CUDA(cudaMemcpy(sumsq, p.dev->bufs[p.dev->cur].sumsq + idx, 8, cudaMemcpyDeviceToHost));
     return SPT_OK;
 }
 
@@ -537,10 +577,10 @@ int spt_trial_stats_all(spt_plan* plan, int32_t nbeam, int64_t* sum, uint64_t* s
     Plan& p = plan->p;
     if (!p.dev || !p.dev->searched) return SPT_ERR_STATE;
     if (nbeam < 1 || nbeam > p.dev->nbeam_search) return SPT_ERR_SHAPE;
-    SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
+    { const int rc = sync_results(p.dev); if (rc != SPT_OK) return rc; }
     const size_t bytes = (size_t)nbeam * p.ntrials * 8;
-    if (sum) SPT_CUDA(cudaMemcpy(sum, p.dev->sum, bytes, cudaMemcpyDeviceToHost));
-    if (sumsq) SPT_CUDA(cudaMemcpy(sumsq, p.dev->sumsq, bytes, cudaMemcpyDeviceToHost));
+    if (sum) SPT_CUDA(cudaMemcpy(sum, p.dev->bufs[p.dev->cur].sum, bytes, cudaMemcpyDeviceToHost));
+    if (sumsq) SPT_CUDA(cudaMemcpy(sumsq, p.dev->bufs[p.dev->cur].sumsq, bytes, cudaMemcpyDeviceToHost));
     return SPT_OK;
 }
 
@@ -548,9 +588,9 @@ int spt_candidates_count(spt_plan* plan, int64_t* total, int32_t* overflowed) {
     if (!plan) return SPT_ERR_INVALID;
     Plan& p = plan->p;
     if (!p.dev || !p.dev->searched) return SPT_ERR_STATE;
-    SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
+    { const int rc = sync_results(p.dev); if (rc != SPT_OK) return rc; }
     unsigned long long c = 0;
-    SPT_CUDA(cudaMemcpy(&c, p.dev->count, 8, cudaMemcpyDeviceToHost));
+    SPT_CUDA(cudaMemcpy(&c, p.dev->bufs[p.dev->cur].count, 8, cudaMemcpyDeviceToHost));
     if (total) *total = (int64_t)c;
     if (overflowed) *overflowed = (int64_t)c > p.cand_capacity ? 1 : 0;
     return SPT_OK;
@@ -564,7 +604,8 @@ int spt_candidates_read(spt_plan* plan, spt_candidate* host_out, int64_t cap, in
     int64_t n = total;
     if (n > plan->p.cand_capacity) n = plan->p.cand_capacity;
     if (n > cap) n = cap;
-    if (n > 0) SPT_CUDA(cudaMemcpy(host_out, plan->p.dev->cand, (size_t)n * sizeof(spt_candidate), cudaMemcpyDeviceToHost));
+    if (n > 0)
+        SPT_CUDA(cudaMemcpy(host_out, plan->p.dev->bufs[plan->p.dev->cur].cand, (size_t)n * sizeof(spt_candidate), cudaMemcpyDeviceToHost));
     if (nwritten) *nwritten = n;
     return SPT_OK;
 }
@@ -594,6 +635,70 @@ int spt_search_host(spt_plan* plan, const uint8_t* h_fb, int32_t nbeam, float th
     if ((rc = spt_candidates_count(plan, &total, &ovf)) != SPT_OK) return rc;
     if (ncand) *ncand = total;
     if (overflowed) *overflowed = ovf;
+    return SPT_OK;
+}
+
+int spt_stream_push(spt_plan* plan, const uint8_t* h_fb, int32_t nbeam, float threshold) {
+    if (!plan || !h_fb || nbeam < 1 || nbeam > plan->p.max_beams || !(threshold == threshold)) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    int rc;
+    try {
+        rc = ensure_device(&p);
+    } catch (const std::bad_alloc&) {
+        rc = SPT_ERR_NOMEM;
+    }
+    if (rc != SPT_OK) return rc;
+    DeviceState* d = p.dev;
+    const int k = d->push_next;
+    DeviceState::Slot& sl = d->slot[k];
+    if (sl.pending) return SPT_ERR_STATE;                        // two batches are in flight: pop first
+    const size_t fb_bytes = (size_t)p.nchan * p.nsamp;
+    if (!d->copy_stream) SPT_CUDA(cudaStreamCreateWithFlags(&d->copy_stream, cudaStreamNonBlocking));
+    if (!sl.fb) {
+        SPT_CUDA(cudaMalloc((void**)&sl.fb, fb_bytes * p.max_beams));
+        SPT_CUDA(cudaMallocHost((void**)&sl.h_count, 8));
+        SPT_CUDA(cudaEventCreateWithFlags(&sl.copied, cudaEventDisableTiming));
+        SPT_CUDA(cudaEventCreateWithFlags(&sl.done, cudaEventDisableTiming));
+        if (k == 1 && !d->bufs[1].sum && (rc = alloc_search_bufs(&p, d->bufs[1])) != SPT_OK) return rc;
+    }
+    if (!d->h_dmt) SPT_CUDA(cudaMalloc((void**)&d->h_dmt, (size_t)p.dmt_elems * 4 * p.max_beams + 128));
+    // copy engine: this batch's input, while the kernels of the previous batch run on the compute stream
+    SPT_CUDA(cudaMemcpyAsync(sl.fb, h_fb, fb_bytes * nbeam, cudaMemcpyHostToDevice, d->copy_stream));
+    SPT_CUDA(cudaEventRecord(sl.copied, d->copy_stream));
+    cudaStream_t st = d->own_stream;
+    SPT_CUDA(cudaStreamWaitEvent(st, sl.copied, 0));
+    const cudaEvent_t keep = d->wait_event;                     // the read-out calls keep looking at the batch popped last
+    const int keep_cur = d->cur;
+    const bool keep_searched = d->searched;
+    if ((rc = do_dedisperse(&p, sl.fb, nbeam, d->h_dmt, st)) != SPT_OK) return rc;
+    if ((rc = do_search(&p, d->h_dmt, nbeam, threshold, st, k)) != SPT_OK) return rc;
+    SPT_CUDA(cudaMemcpyAsync(sl.h_count, d->bufs[k].count, 8, cudaMemcpyDeviceToHost, st));
+    SPT_CUDA(cudaEventRecord(sl.done, st));
+    d->wait_event = keep; d->cur = keep_cur; d->searched = keep_searched;
+    sl.nbeam = nbeam;
+    sl.pending = true;
+    d->push_next = k ^ 1;
+    return SPT_OK;
+}
+
+int spt_stream_pop(spt_plan* plan, int64_t* ncand, int32_t* overflowed) {
+    if (!plan) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (!p.dev) return SPT_ERR_STATE;
+    DeviceState* d = p.dev;
+    const int k = d->pop_next;
+    DeviceState::Slot& sl = d->slot[k];
+    if (!sl.pending) return SPT_ERR_STATE;                       // nothing pushed
+    SPT_CUDA(cudaEventSynchronize(sl.done));
+    const int64_t total = (int64_t)*sl.h_count;
+    if (ncand) *ncand = total;
+    if (overflowed) *overflowed = total > p.cand_capacity ? 1 : 0;
+    sl.pending = false;
+    d->pop_next = k ^ 1;
+    d->cur = k;                                                  // read-out calls now look at this batch's results
+    d->wait_event = sl.done;
+    d->nbeam_search = sl.nbeam;
+    d->searched = true;
     return SPT_OK;
 }
 

@@ -227,6 +227,45 @@ def test_search_host_matches_device_path(cuda, api, orc, synth):
     assert plan.launches() >= 2
 
 
+def test_stream_pipeline_matches_search_host(cuda, api, synth):
+    """Two batches in flight (H2D of one overlapping the kernels of the other): every pop gives what the synchronous call
+    gives for that batch, and the read-out calls follow the popped batch."""
+    w = synth.workload(4, nsamp=1 << 13, nbeam=2)
+    w.ranges = [(0.0, 0.2, 70, 1), (500.0, 0.5, 40, 2)]
+    w.threshold = 5.0
+    batches = []
+    for i in range(4):
+        fb = np.stack([synth.generate(w, beam=2 * i + b) for b in range(2)])
+        fb[0, :, 3000 + 100 * i: 3004 + 100 * i] += 25             # a different zero-DM spike per batch
+        batches.append(cuda.from_numpy(fb).pin_memory())
+    ref_plan = make_plan(api, w, nbeam=2)
+    expect = []
+    for hb in batches:
+        n, ovf = ref_plan.search_host(hb, w.threshold)
+        c = ref_plan.candidates_read()
+        s, q = ref_plan.trial_stats_all(2)
+        expect.append((n, np.sort(c, order=["beam", "trial", "t"]), s.copy(), q.copy()))
+    assert len({e[0] for e in expect}) > 1 and all(e[0] > 0 for e in expect)
+    plan = make_plan(api, w, nbeam=2)
+    with pytest.raises(api.SptError) as e:
+        plan.stream_pop()                                            # nothing in flight
+    assert e.value.code == api.SPT_ERR_STATE
+    plan.stream_push(batches[0], w.threshold)
+    plan.stream_push(batches[1], w.threshold)
+    with pytest.raises(api.SptError) as e:
+        plan.stream_push(batches[2], w.threshold)                    # a third batch must wait for a pop
+    assert e.value.code == api.SPT_ERR_STATE
+    for i in range(4):
+        n, ovf = plan.stream_pop()                                   # batch i + 1 is still in flight
+        assert (n, ovf) == (expect[i][0], False)
+        c = np.sort(plan.candidates_read(), order=["beam", "trial", "t"])
+        assert np.array_equal(c, expect[i][1])
+        s, q = plan.trial_stats_all(2)
+        assert np.array_equal(s, expect[i][2]) and np.array_equal(q, expect[i][3])
+        if i + 2 < 4:
+            plan.stream_push(batches[i + 2], w.threshold)            # reuses the buffers of the batch just read out
+
+
 def test_candidate_overflow_is_reported(cuda, api, synth):
     w = synth.workload(1)
     fb = synth.generate(w)
