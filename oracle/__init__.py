@@ -52,6 +52,8 @@ def lib():
         L.orc_best_width.argtypes = [vp, i64, vp, i32, vp, vp]
         L.orc_snr_at.argtypes = [vp, i64, i32, i64, vp]
         L.orc_search_plane.argtypes = [vp, i32, vp, vp, vp, i32, f64, vp, vp, vp, vp, vp, vp, vp]
+        L.orc_peak_filter.argtypes = [i64, vp, vp, vp, vp, vp, i32, i32, vp]
+        L.orc_peak_filter.restype = ctypes.c_int
         for name in ("orc_delay_table", "orc_nout", "orc_decimate", "orc_dedisperse_u16", "orc_dedisperse_u8",
                      "orc_dedisperse_point_u8", "orc_stats", "orc_mean_sigma", "orc_boxcar_snr", "orc_best_width",
                      "orc_snr_at", "orc_search_plane"):
@@ -199,6 +201,22 @@ def search_plane(dmt: np.ndarray, rowoff: np.ndarray, nout_: np.ndarray, widths:
                                       _ptr(s), _ptr(q), _ptr(cnt), _ptr(candoff), _ptr(ct), _ptr(cw), _ptr(cs)),
                "search_plane(fill)")
     return PlaneSearch(s, q, cnt, candoff, ct, cw, cs)
+
+
+# ---- E. peak filtering --------------------------------------------------------------------
+def peak_filter(beam: np.ndarray, trial: np.ndarray, t: np.ndarray, snr: np.ndarray, range_of_trial: np.ndarray,
+                windows: Sequence[int] = (3, 11)) -> np.ndarray:
+    """Boolean mask of the candidates that survive the stencils applied one after the other."""
+    beam = np.ascontiguousarray(beam, dtype=np.int32)
+    trial = np.ascontiguousarray(trial, dtype=np.int32)
+    t = np.ascontiguousarray(t, dtype=np.int32)
+    snr = np.ascontiguousarray(snr, dtype=np.float64)
+    rot = np.ascontiguousarray(range_of_trial, dtype=np.int32)
+    alive = np.ones(beam.size, dtype=np.uint8)
+    for w in windows:
+        _check(lib().orc_peak_filter(beam.size, _ptr(beam), _ptr(trial), _ptr(t), _ptr(snr), _ptr(rot), rot.size, int(w),
+                                     _ptr(alive)), "peak_filter")
+    return alive.astype(bool)
 
 
 # ---- whole path over a plan (one beam) ----------------------------------------------------------------

@@ -24,6 +24,8 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <map>
+#include <tuple>
 #include <vector>
 #ifdef _OPENMP
 #include <omp.h>
@@ -330,6 +332,49 @@ int orc_search_plane(const int32_t* dmt, int32_t ntrial, const int64_t* rowoff, 
         count[d] = cnt;
     }
     return bad ? -1 : 0;
+}
+
+/* ------------------------------------------------------------------------------------------------
+ * E. Peak filtering of the candidate plane -- PAPER.md:96: "Peaks are filtered out by sliding a window across
+ * the candidates in the DM-time plane.  From each window, the peak with the highest S/N is picked, and all
+ * others are rejected.  Two different stencils are used: a 3x3 window, and an 11x11 window."
+ * Reading E: the plane of one beam and one DM range has axes (trial index, sample index of the
+ * range's own rate); the window of odd size P is centred on each candidate in turn (it slides by one cell); a
+ * candidate is kept iff no OTHER live candidate of the same beam and range inside its window is stronger, where
+ * stronger = larger S/N, or equal S/N and smaller (trial, t) in that order -- so exactly one of an exact tie
+ * survives.  Stencils are applied one after the other by calling this once per window: `alive` is both input
+ * (only live candidates compete) and output.
+ * Plain form: for every candidate, every cell of its window is looked up in an ordered map.
+ * ---------------------------------------------------------------------------------------------- */
+int orc_peak_filter(int64_t n, const int32_t* beam, const int32_t* trial, const int32_t* t, const double* snr,
+                    const int32_t* range_of_trial /* [ntrial] */, int32_t ntrial, int32_t window, uint8_t* alive /* [n] in/out */) {
+    if (n < 0 || window < 1 || (window & 1) == 0 || !alive || (n > 0 && (!beam || !trial || !t || !snr || !range_of_trial))) return -1;
+    const int32_t h = (window - 1) / 2;
+    std::map<std::tuple<int32_t, int32_t, int32_t>, int64_t> at;   /* (beam, trial, t) -> index, live candidates only */
+    for (int64_t i = 0; i < n; ++i) {
+        if (trial[i] < 0 || trial[i] >= ntrial) return -1;
+        if (alive[i] && !at.emplace(std::make_tuple(beam[i], trial[i], t[i]), i).second) return -2;   /* duplicate cell */
+    }
+    std::vector<uint8_t> out((size_t)n, 0);
+    for (int64_t i = 0; i < n; ++i) {
+        if (!alive[i]) continue;
+        bool beaten = false;
+        for (int32_t dd = trial[i] - h; dd <= trial[i] + h && !beaten; ++dd) {
+            if (dd < 0 || dd >= ntrial || range_of_trial[dd] != range_of_trial[trial[i]]) continue;
+            for (int32_t tt = t[i] - h; tt <= t[i] + h; ++tt) {
+                if (dd == trial[i] && tt == t[i]) continue;
+                auto it = at.find(std::make_tuple(beam[i], dd, tt));
+                if (it == at.end()) continue;
+                const int64_t j = it->second;
+                const bool stronger = snr[j] > snr[i] ||
+                                      (snr[j] == snr[i] && (trial[j] < trial[i] || (trial[j] == trial[i] && t[j] < t[i])));
+                if (stronger) { beaten = true; break; }
+            }
+        }
+        out[(size_t)i] = beaten ? 0 : 1;
+    }
+    for (int64_t i = 0; i < n; ++i) alive[i] = out[(size_t)i];
+    return 0;
 }
 
 }  // extern "C"
