@@ -205,6 +205,16 @@ def run_ours(args, rank, world, local_rank):
     data_s = nbeam * w.nsamp * w.tsamp
     rtf = data_s * world * steps / (ms_total * 1e-3)
 
+    # ---- NEXT-1, outside the timed step: 3x3 then 11x11 peak filtering of the step's candidate list ------
+    pk0, pk1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    plan.peak_filter((3, 11), stream)                      # warm-up (allocates the lookup plane)
+    pk0.record(stream)
+    npeaks = int(plan.peak_filter((3, 11), stream).size)
+    pk1.record(stream)
+    torch.cuda.synchronize()
+    peak_info = {"windows": [3, 11], "candidates_in": int(ncand), "peaks_out": npeaks,
+                 "ms_with_readback": pk0.elapsed_time(pk1)}
+
     # ---- e2e: the same path from HOST memory through the library's streaming entry points (spt_stream_push / pop): every
     # step's filterbank is copied from pinned host memory inside the timed region (the copy of step i+1 overlaps the kernels
     # of step i, two batches in flight) and every step's candidate count is read back to the host ---------------------
@@ -299,7 +309,7 @@ def run_ours(args, rank, world, local_rank):
                     "d2h_bytes_per_step": 8, "ms_per_step": 1e3 * e2e_s / steps,
                     "rtf": data_s * world * steps / e2e_s, "api": "spt_stream_push/spt_stream_pop (two batches in flight)",
                     "ms_per_step_synchronous_call": e2e_sync_ms},
-            "gpu_launches": launches, "clocks": clocks, "kernel_ms": kernels, "probe": probe,
+            "peak_filter": peak_info, "gpu_launches": launches, "clocks": clocks, "kernel_ms": kernels, "probe": probe,
             "roofline": roof, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if world > 1:

@@ -160,6 +160,23 @@ int spt_candidates_count(spt_plan* plan, int64_t* total, int32_t* overflowed);
 int spt_candidates_read(spt_plan* plan, spt_candidate* host_out, int64_t cap, int64_t* nwritten);
 
 /* -------------------------------------------------------------------------------------------------------
+ * spt_peak_filter -- the stage after the search ("Peaks are filtered out by sliding a window across the
+ * candidates in the DM-time plane.  From each window, the peak with the highest S/N is picked, and all others are
+ * rejected.  Two different stencils are used: a 3x3 window, and an 11x11 window"; reading E).
+ * Works on the candidate list of the last search (or of the batch popped last).  The plane of one beam and one DM
+ * range has axes (trial, t); the window of odd size windows[i] is centred on each candidate in turn; a candidate is
+ * kept iff no other live candidate of the same beam and range inside its window is stronger (larger snr field, or
+ * equal snr and smaller (trial, t)).  The windows are applied one after the other on the survivors; {3, 11} is the
+ * paper's pair.  windows: HOST, odd, 1..255, at most 8.  The candidate list itself is left untouched.
+ * SPT_ERR_SHAPE if the list overflowed its capacity (an incomplete list cannot be filtered).  Waits for the search,
+ * then enqueues on cuda_stream and returns.
+ * spt_peaks_count / spt_peaks_read synchronise and return the survivors (order arbitrary).
+ * ----------------------------------------------------------------------------------------------------- */
+int spt_peak_filter(spt_plan* plan, const int32_t* windows /*HOST*/, int32_t nwindows, void* cuda_stream);
+int spt_peaks_count(spt_plan* plan, int64_t* total);
+int spt_peaks_read(spt_plan* plan, spt_candidate* host_out /*HOST*/, int64_t cap, int64_t* nwritten);
+
+/* -------------------------------------------------------------------------------------------------------
  * spt_search_host -- the whole path from HOST memory: H2D copy of h_fb (uint8 [nbeam][nchan][nsamp]; pinned
  * memory makes the copy asynchronous), spt_dedisperse + spt_single_pulse_search into a library-owned DM
  * transform, then the candidate count back to the host.  Synchronous.  Candidates are then read with

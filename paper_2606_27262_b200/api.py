@@ -54,6 +54,9 @@ SYMBOLS = {
     "spt_candidates_count": (ctypes.c_int, [_vp, _P(_i64), _P(_i32)]),
     "spt_candidates_read": (ctypes.c_int, [_vp, _vp, _i64, _P(_i64)]),
     "spt_search_host": (ctypes.c_int, [_vp, _vp, _i32, _f32, _vp, _P(_i64), _P(_i32)]),
+    "spt_peak_filter": (ctypes.c_int, [_vp, _P(_i32), _i32, _vp]),
+    "spt_peaks_count": (ctypes.c_int, [_vp, _P(_i64)]),
+    "spt_peaks_read": (ctypes.c_int, [_vp, _vp, _i64, _P(_i64)]),
     "spt_stream_push": (ctypes.c_int, [_vp, _vp, _i32, _f32]),
     "spt_stream_pop": (ctypes.c_int, [_vp, _P(_i64), _P(_i32)]),
     "spt_plan_kernel_times": (ctypes.c_int, [_vp, _i32, _vp, _vp, _vp, _P(_i32)]),
@@ -242,6 +245,17 @@ class Plan:
         _check(lib().spt_search_host(self._h, ptr, nbeam, float(threshold), dptr, ctypes.byref(n), ctypes.byref(o)),
                "spt_search_host")
         return int(n.value), bool(o.value)
+
+    def peak_filter(self, windows: Sequence[int] = (3, 11), stream=None) -> np.ndarray:
+        """Peak filtering of the last search's candidates; returns the surviving records."""
+        w = (ctypes.c_int32 * len(windows))(*[int(x) for x in windows])
+        _check(lib().spt_peak_filter(self._h, w, len(windows), _stream_ptr(stream)), "spt_peak_filter")
+        n = ctypes.c_int64()
+        _check(lib().spt_peaks_count(self._h, ctypes.byref(n)), "spt_peaks_count")
+        out = np.empty(max(int(n.value), 1), dtype=CAND_DTYPE)
+        k = ctypes.c_int64()
+        _check(lib().spt_peaks_read(self._h, out.ctypes.data, int(n.value), ctypes.byref(k)), "spt_peaks_read")
+        return out[: int(k.value)]
 
     def stream_push(self, h_fb, threshold: float):
         """Enqueue one batch (HOST uint8 [nbeam][nchan][nsamp], pinned) into the two-deep pipeline; returns at once."""

@@ -38,6 +38,16 @@ struct DeviceState {
     std::vector<RangeDev> r;
     int32_t* nout = nullptr;        // [ntrials]
     int64_t* offset = nullptr;      // [ntrials]
+    int32_t* range_lo = nullptr;    // [ntrials] first / last trial of the trial's DM range (peak filter)
+    int32_t* range_hi = nullptr;
+    // peak filter (lazily allocated): lookup plane laid out like the DM transform, live flags, peak list
+    uint32_t* plane = nullptr;
+    uint8_t* alive[2] = {nullptr, nullptr};
+    int64_t alive_cap = 0;
+    spt_candidate* peaks = nullptr;
+    int64_t peaks_cap = 0;
+    unsigned long long* peaks_count = nullptr;
+    bool peaks_valid = false;
     // results of a search: statistics [max_beams][ntrials], candidate list, exact count.  Set 0 serves the plain calls;
     // the streaming calls (spt_stream_push/pop) alternate between set 0 and a lazily allocated set 1.
     struct SearchBufs {
@@ -109,7 +119,8 @@ static void free_device(Plan* p) {
         cudaFree(r.delay); cudaFree(r.tiles); cudaFree(r.sidx); cudaFree(r.rows); cudaFree(r.blob);
         cudaFree(r.series);
     }
-    cudaFree(d->nout); cudaFree(d->offset);
+    cudaFree(d->nout); cudaFree(d->offset); cudaFree(d->range_lo); cudaFree(d->range_hi);
+    cudaFree(d->plane); cudaFree(d->alive[0]); cudaFree(d->alive[1]); cudaFree(d->peaks); cudaFree(d->peaks_count);
     for (auto& b : d->bufs) { cudaFree(b.sum); cudaFree(b.sumsq); cudaFree(b.cand); cudaFree(b.count); }
     for (auto& sl : d->slot) {
         cudaFree(sl.fb);
@@ -151,7 +162,7 @@ static int ensure_device(Plan* p) {
     if (!d) return SPT_ERR_NOMEM;
     p->dev = d;
     d->r.resize(p->ranges.size());
-    std::vector<int32_t> nout_all;
+    std::vector<int32_t> nout_all, lo_all, hi_all;
     std::vector<int64_t> off_all;
     int rc = SPT_OK;
     for (size_t i = 0; i < p->ranges.size() && rc == SPT_OK; ++i) {
@@ -159,6 +170,8 @@ static int ensure_device(Plan* p) {
         RangeDev& rd = d->r[i];
         nout_all.insert(nout_all.end(), rp.nout.begin(), rp.nout.end());
         off_all.insert(off_all.end(), rp.offset.begin(), rp.offset.end());
+        lo_all.insert(lo_all.end(), (size_t)rp.ndm, rp.trial0);
+        hi_all.insert(hi_all.end(), (size_t)rp.ndm, rp.trial0 + rp.ndm - 1);
         if (p->opt_kernel == 1) rc = upload(&rd.delay, rp.delay);
         else {
             if ((rc = upload(&rd.tiles, rp.tiles)) != SPT_OK) break;
@@ -175,6 +188,8 @@ static int ensure_device(Plan* p) {
     }
     if (rc == SPT_OK) rc = upload(&d->nout, nout_all);
     if (rc == SPT_OK) rc = upload(&d->offset, off_all);
+    if (rc == SPT_OK) rc = upload(&d->range_lo, lo_all);
+    if (rc == SPT_OK) rc = upload(&d->range_hi, hi_all);
     if (rc == SPT_OK) rc = alloc_search_bufs(p, d->bufs[0]);
     if (rc == SPT_OK) {
         cudaError_t ce = cudaStreamCreateWithFlags(&d->own_stream, cudaStreamNonBlocking);
@@ -272,6 +287,7 @@ static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float thresho
     d->searched = true;
     d->cur = set;
     d->wait_event = nullptr;
+    d->peaks_valid = false;
     return SPT_OK;
 }
 
@@ -699,6 +715,73 @@ int spt_stream_pop(spt_plan* plan, int64_t* ncand, int32_t* overflowed) {
     d->wait_event = sl.done;
     d->nbeam_search = sl.nbeam;
     d->searched = true;
+    return SPT_OK;
+}
+
+int spt_peak_filter(spt_plan* plan, const int32_t* windows, int32_t nwindows, void* cuda_stream) {
+    if (!plan || !windows || nwindows < 1 || nwindows > 8) return SPT_ERR_INVALID;
+    for (int32_t i = 0; i < nwindows; ++i)
+        if (windows[i] < 1 || (windows[i] & 1) == 0 || windows[i] > 255) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (!p.dev || !p.dev->searched) return SPT_ERR_STATE;
+    DeviceState* d = p.dev;
+    int64_t total = 0;
+    int32_t ovf = 0;
+    int rc = spt_candidates_count(plan, &total, &ovf);           // waits for the search the list comes from
+    if (rc != SPT_OK) return rc;
+    if (ovf) return SPT_ERR_SHAPE;                               // an incomplete list cannot be filtered
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if (!d->plane) {
+        const size_t bytes = (size_t)p.max_beams * p.dmt_elems * sizeof(uint32_t);
+        SPT_CUDA(cudaMalloc((void**)&d->plane, bytes ? bytes : 4));
+        SPT_CUDA(cudaMemset(d->plane, 0, bytes));
+        SPT_CUDA(cudaMalloc((void**)&d->peaks_count, 8));
+    }
+    if (total > d->alive_cap) {
+        cudaFree(d->alive[0]); cudaFree(d->alive[1]); cudaFree(d->peaks);
+        d->alive[0] = d->alive[1] = nullptr; d->peaks = nullptr; d->alive_cap = d->peaks_cap = 0;
+        SPT_CUDA(cudaMalloc((void**)&d->alive[0], (size_t)total));
+        SPT_CUDA(cudaMalloc((void**)&d->alive[1], (size_t)total));
+        SPT_CUDA(cudaMalloc((void**)&d->peaks, (size_t)total * sizeof(spt_candidate)));
+        d->alive_cap = d->peaks_cap = total;
+    }
+    SPT_CUDA(cudaMemsetAsync(d->peaks_count, 0, 8, st));
+    PeakArgs a{d->bufs[d->cur].cand, total, d->plane, p.dmt_elems, d->nout, d->offset, d->range_lo, d->range_hi};
+    launch_peaks_scatter(a, true, st);
+    const uint8_t* in = nullptr;
+    for (int32_t i = 0; i < nwindows; ++i) {
+        launch_peaks_stencil(a, windows[i], in, d->alive[i & 1], st);
+        in = d->alive[i & 1];
+    }
+    launch_peaks_compact(a, in, d->peaks, d->peaks_count, d->peaks_cap, st);
+    launch_peaks_scatter(a, false, st);                          // the plane is all zero again
+    p.launches += (total > 0) ? 3 + nwindows : 0;
+    SPT_CUDA(cudaGetLastError());
+    d->last_stream = st;
+    d->wait_event = nullptr;
+    d->peaks_valid = true;
+    return SPT_OK;
+}
+
+int spt_peaks_count(spt_plan* plan, int64_t* total) {
+    if (!plan || !total) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (!p.dev || !p.dev->peaks_valid) return SPT_ERR_STATE;
+    SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
+    unsigned long long c = 0;
+    SPT_CUDA(cudaMemcpy(&c, p.dev->peaks_count, 8, cudaMemcpyDeviceToHost));
+    *total = (int64_t)c;
+    return SPT_OK;
+}
+
+int spt_peaks_read(spt_plan* plan, spt_candidate* host_out, int64_t cap, int64_t* nwritten) {
+    if (!plan || (!host_out && cap > 0) || cap < 0) return SPT_ERR_INVALID;
+    int64_t n = 0;
+    const int rc = spt_peaks_count(plan, &n);
+    if (rc != SPT_OK) return rc;
+    if (n > cap) n = cap;
+    if (n > 0) SPT_CUDA(cudaMemcpy(host_out, plan->p.dev->peaks, (size_t)n * sizeof(spt_candidate), cudaMemcpyDeviceToHost));
+    if (nwritten) *nwritten = n;
     return SPT_OK;
 }
 

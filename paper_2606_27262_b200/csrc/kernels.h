@@ -38,6 +38,21 @@ struct SpsArgs {
 };
 void launch_sps(const SpsArgs& a, int32_t nbeam, cudaStream_t st);
 
+struct PeakArgs {
+    const spt_candidate* cand;      // the list of the last search
+    int64_t n;                      // records in it
+    uint32_t* plane;                // [nbeam][beam_stride] lookup table, all zero between calls
+    int64_t beam_stride;
+    const int32_t* nout;            // [ntrials]
+    const int64_t* offset;          // [ntrials]
+    const int32_t* range_lo;        // [ntrials] first / last trial of the trial's DM range
+    const int32_t* range_hi;
+};
+void launch_peaks_scatter(const PeakArgs& a, bool set, cudaStream_t st);
+void launch_peaks_stencil(const PeakArgs& a, int32_t window, const uint8_t* alive_in, uint8_t* alive_out, cudaStream_t st);
+void launch_peaks_compact(const PeakArgs& a, const uint8_t* alive, spt_candidate* out, unsigned long long* out_count,
+                          long long out_capacity, cudaStream_t st);
+
 int run_probe(int kind, int reps, double* warp_instr_per_s, double* elapsed_ms);
 
 }  // namespace spt

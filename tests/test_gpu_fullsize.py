@@ -131,6 +131,12 @@ def test_cfg3_full_injected_bursts_found(cuda, api, orc, synth):
         if near.size and near["snr"].max() >= max(w.threshold, 0.3 * b.snr):
             found += 1
     assert found == len(strong), (found, len(strong))
+    # NEXT-1 at full size: the 3x3 + 11x11 peak filter on the same list, exact against the oracle's filter
+    peaks = plan.peak_filter((3, 11))
+    keep = orc.peak_filter(cands["beam"], cands["trial"], cands["t"], cands["snr"].astype(np.float64), rg, (3, 11))
+    key = lambda c: set(zip(c["trial"].tolist(), c["t"].tolist(), c["width"].tolist(), c["snr"].tolist()))
+    assert key(peaks) == key(cands[keep])
+    assert peaks.size * 5 < cands.size            # "an order-of-magnitude reduction"
 
 
 def test_cfg5_full_rfi_volume(cuda, api, orc, synth):
