@@ -97,8 +97,10 @@ int spt_plan_delays(const spt_plan* plan, int32_t trial, int32_t* host_out);
 /* Kernel-selection knobs, for A/B measurements and tests; must be set before the first spt_dedisperse.
  *   "dedisp_kernel": 0 = tiled shared-memory kernel (default, the product), 1 = one-thread-per-output kernel
  *                    reading global memory (bring-up / cross-check kernel, same results)
- *   "group":         channels per pre-summed group G of the tiled kernel: 1, 2, 4 (default) or 8
+ *   "group":         largest pre-summed channel group of the tiled kernel: 1, 2, 4 or 8 (default)
  *   "dm_tile":       trials per block tile (32 or 64; default 64)
+ *   "skew":          1 (default) = every trial of a DM tile computes an output window shifted by its own delay at a
+ *                    reference channel, which narrows the windows the tile reads; 0 = one window start per tile
  *   "profile":       1 = bracket every kernel launch with CUDA events on the caller's stream (see
  *                    spt_plan_kernel_times); may be switched at any time
  * Unknown names / values -> SPT_ERR_INVALID. */

@@ -31,6 +31,7 @@ struct RangeDev {
     StageIndex* sidx = nullptr;
     RowDesc* rows = nullptr;
     uint32_t* blob = nullptr;
+    int32_t* skew = nullptr;
     uint16_t* series = nullptr;     // decimated input [max_beams][nchan][stride_k] (decim > 1)
 };
 
@@ -116,7 +117,7 @@ static void free_device(Plan* p) {
     DeviceState* d = p->dev;
     if (!d) return;
     for (RangeDev& r : d->r) {
-        cudaFree(r.delay); cudaFree(r.tiles); cudaFree(r.sidx); cudaFree(r.rows); cudaFree(r.blob);
+        cudaFree(r.delay); cudaFree(r.tiles); cudaFree(r.sidx); cudaFree(r.rows); cudaFree(r.blob); cudaFree(r.skew);
         cudaFree(r.series);
     }
     cudaFree(d->nout); cudaFree(d->offset); cudaFree(d->range_lo); cudaFree(d->range_hi);
@@ -178,6 +179,7 @@ static int ensure_device(Plan* p) {
             if ((rc = upload(&rd.sidx, rp.sidx)) != SPT_OK) break;
             if ((rc = upload(&rd.rows, rp.rows)) != SPT_OK) break;
             if ((rc = upload(&rd.blob, rp.blob)) != SPT_OK) break;
+            if ((rc = upload(&rd.skew, rp.skew)) != SPT_OK) break;
         }
         if (rc == SPT_OK && rp.decim > 1) {
             const size_t bytes = (size_t)p->max_beams * p->nchan * rp.stride_k * sizeof(uint16_t);
@@ -245,7 +247,7 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
                                               p->nchan, rp.ndm, nbeam, rp.max_nout, d_dmt, p->dmt_elems, st);
         } else {
             const int rc = launch_dedisp_tiled(u16, p->opt_dm_tile, src, rs, (int64_t)p->nchan * rs, d_dmt, p->dmt_elems,
-                                               rd.tiles, rd.sidx, rd.rows, rd.blob, rp.vcap_words, nout, off,
+                                               rd.tiles, rd.sidx, rd.rows, rd.blob, rd.skew, rp.skew_max, rp.vcap_words, nout, off,
                                                (int32_t)rp.tiles.size(), rp.ntile_t, nbeam, st);
             if (rc != 0) { g_last_error = "dedisp_tiled: launch configuration rejected"; return SPT_ERR_CUDA; }
         }
@@ -401,6 +403,9 @@ int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value) {
     } else if (!std::strcmp(name, "group")) {
         if (value != 1 && value != 2 && value != 4 && value != 8) return SPT_ERR_INVALID;
         p.opt_group = (int32_t)value; p.tiling_built = false;
+    } else if (!std::strcmp(name, "skew")) {
+        if (value != 0 && value != 1) return SPT_ERR_INVALID;
+        p.opt_skew = (int32_t)value; p.tiling_built = false;
     } else if (!std::strcmp(name, "dm_tile")) {
         if (value != 32 && value != 64) return SPT_ERR_INVALID;
         p.opt_dm_tile = (int32_t)value; p.tiling_built = false;
@@ -508,6 +513,10 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
                 }
         }
     }
+    // the tables hold the delays relative to the trial's skewed output window
+    const int32_t sk = rp->skew[(size_t)td.skew0 + dl];
+    for (int32_t c = 0; c < p.nchan; ++c)
+        if (host_out[c] != INT32_MIN) host_out[c] += sk;
     return SPT_OK;
 }
 

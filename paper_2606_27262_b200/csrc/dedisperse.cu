@@ -122,6 +122,8 @@ struct TiledArgs {
     const StageIndex* sidx;
     const RowDesc* rows;
     const uint32_t* blob;
+    const int32_t* skew;       // [ntile_dm][DT] output skew of every trial of a DM tile
+    int32_t skew_max;
     const int32_t* nout;       // range local
     const int64_t* offset;     // range local
     int32_t vcap_words, ntile_dm, ntile_t, nbeam;
@@ -262,7 +264,7 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     const uint32_t bar = smem_u32(smem);
     // control area: mbarrier, then per trial of the tile {row pointer, nout} for the flush
     int32_t** const s_rowp = reinterpret_cast<int32_t**>(smem + 64);
-    int32_t* const s_nout = reinterpret_cast<int32_t*>(smem + 64 + kMaxDT * 8);
+    int2* const s_valid = reinterpret_cast<int2*>(smem + 64 + kMaxDT * 8);      // [lo, hi) valid outputs of the trial in this tile
     RowDesc* const s_rows = reinterpret_cast<RowDesc*>(smem + 64 + kMaxDT * 16);                          // [2][kMaxStageRows]
     StageIndex* const s_sidx = reinterpret_cast<StageIndex*>(smem + 64 + kMaxDT * 16 + 2 * kMaxStageRows * 16);  // [2]
     uint32_t* const s_var = reinterpret_cast<uint32_t*>(smem + kSmemCtrlBytes + 2 * kBlobBytes);
@@ -275,8 +277,7 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     const int tt = bid % a.ntile_t;
     const int beam = bid / a.ntile_t;
     const TileDesc td = a.tiles[dmt];
-    const int64_t t0 = (int64_t)tt * kTT;
-    if (t0 >= a.nout[td.trial0]) return;  // nout is non-increasing in the trial index (delays grow with DM)
+    const int64_t t0 = (int64_t)tt * kTT;   // trial i of the tile computes the outputs t0 - skew[i] + [0, kTT)
 
     const T* in = reinterpret_cast<const T*>(a.in) + (int64_t)beam * a.beam_stride;
 
@@ -291,12 +292,15 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
         uint32_t bytes = 0;
         for (uint32_t k = lane; k < si.nrows; k += 32) {
             const RowDesc r = rows[k];
+            // the window [pos, pos + nelem) of the channel's row, clipped to the row: the part before the row (skewed
+            // output windows start before t = 0) and the part after it are not copied (all multiples of 16 elements)
             const int64_t pos = t0 + r.astart;
-            const int64_t room = a.row_stride - pos;
-            const int64_t n = room < (int64_t)r.nelem ? (room > 0 ? room : 0) : (int64_t)r.nelem;
+            const int64_t beg = pos < 0 ? 0 : pos;
+            const int64_t end = min(pos + (int64_t)r.nelem, a.row_stride);
+            const int64_t n = end > beg ? end - beg : 0;
             if (n > 0)
-                bulk_g2s(smem_u32(s_rawb + r.soff), in + (int64_t)r.chan * a.row_stride + pos,
-                         (uint32_t)n * (uint32_t)sizeof(T), bar);
+                bulk_g2s(smem_u32(s_rawb + r.soff) + (uint32_t)(beg - pos) * (uint32_t)sizeof(T),
+                         in + (int64_t)r.chan * a.row_stride + beg, (uint32_t)n * (uint32_t)sizeof(T), bar);
             bytes += (uint32_t)n * (uint32_t)sizeof(T);
         }
 #pragma unroll
@@ -314,12 +318,26 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_proxy_async();
     }
+    int have = 0;
     if (tid < DT) {
         const int d = td.trial0 + (tid < td.ntrial ? tid : td.ntrial - 1);
-        s_rowp[tid] = a.out + (int64_t)beam * a.out_beam_stride + a.offset[d] + t0;
-        s_nout[tid] = tid < td.ntrial ? (int32_t)min((int64_t)kTT, max((int64_t)0, (int64_t)a.nout[d] - t0)) : 0;  // valid outputs of the tile
+        const int64_t first = t0 - a.skew[td.skew0 + tid];                 // output sample of accumulator index 0
+        s_rowp[tid] = a.out + (int64_t)beam * a.out_beam_stride + a.offset[d] + first;
+        const int lo = (int)min((int64_t)kTT, max((int64_t)0, -first));
+        const int hi = tid < td.ntrial ? (int)min((int64_t)kTT, max((int64_t)lo, (int64_t)a.nout[d] - first)) : lo;
+        s_valid[tid] = make_int2(lo, hi);
+        have = hi > lo;
     }
-    __syncthreads();
+    if (!__syncthreads_or(have)) return;    // no trial of the tile has an output here (ragged rows, skewed windows)
+    if (sizeof(T) > 1 && t0 < (int64_t)a.skew_max + 32) {
+        // Windows that start before the row are not copied.  What the raw region holds there feeds only outputs with t < 0,
+        // which are discarded, but their 16-bit lanes must not carry into the valid high lanes: make the first contents
+        // zero (later stages find there the bounded samples of an earlier stage).
+        uint4* r4 = reinterpret_cast<uint4*>(s_rawb);
+        const int n4 = (kSmemDataBytes - a.vcap_words * 4) / 16;
+        for (int i = tid; i < n4; i += kThreads) r4[i] = make_uint4(0u, 0u, 0u, 0u);
+        __syncthreads();
+    }
     if (warp == 0) issue_stage(0);
 
     uint32_t acc[TPW][NJ];
@@ -386,17 +404,18 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
             for (int q = 0; q < TPW; ++q) {
                 const int dl = warp * TPW + q;
                 int32_t* row = s_rowp[dl];
-                const int n = s_nout[dl];
+                const int2 ok = s_valid[dl];
 #pragma unroll
                 for (int j = 0; j < NJ; ++j) {
                     const int i = lane + 32 * j;
                     const int32_t lo = (int32_t)(acc[q][j] & 0xFFFFu), hi = (int32_t)(acc[q][j] >> 16);
+                    const bool ok_lo = i >= ok.x && i < ok.y, ok_hi = i + kH >= ok.x && i + kH < ok.y;
                     if (first_flush) {
-                        if (i < n) row[i] = lo;
-                        if (i + kH < n) row[i + kH] = hi;
+                        if (ok_lo) row[i] = lo;
+                        if (ok_hi) row[i + kH] = hi;
                     } else {
-                        if (i < n) atomicAdd(row + i, lo);          // result unused: a fire-and-forget RED in L2
-                        if (i + kH < n) atomicAdd(row + i + kH, hi);
+                        if (ok_lo) atomicAdd(row + i, lo);          // result unused: a fire-and-forget RED in L2
+                        if (ok_hi) atomicAdd(row + i + kH, hi);
                     }
                     acc[q][j] = 0u;
                 }
@@ -424,9 +443,9 @@ static int launch_tiled_inst(const TiledArgs& a, cudaStream_t st) {
 
 int launch_dedisp_tiled(bool is_u16, int DT, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
                         int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
-                        const uint32_t* blob, int32_t vcap_words, const int32_t* nout, const int64_t* offset,
-                        int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, cudaStream_t st) {
-    TiledArgs a{in, row_stride, beam_stride, out, out_beam_stride, tiles, sidx, rows, blob, nout, offset,
+                        const uint32_t* blob, const int32_t* skew, int32_t skew_max, int32_t vcap_words, const int32_t* nout,
+                        const int64_t* offset, int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, cudaStream_t st) {
+    TiledArgs a{in, row_stride, beam_stride, out, out_beam_stride, tiles, sidx, rows, blob, skew, skew_max, nout, offset,
                 vcap_words, ntile_dm, ntile_t, nbeam};
     if (DT == 64) return is_u16 ? launch_tiled_inst<uint16_t, 64>(a, st) : launch_tiled_inst<uint8_t, 64>(a, st);
     if (DT == 32) return is_u16 ? launch_tiled_inst<uint16_t, 32>(a, st) : launch_tiled_inst<uint8_t, 32>(a, st);

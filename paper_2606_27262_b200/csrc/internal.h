@@ -74,6 +74,8 @@ struct TileDesc {           // one DM tile of a range
     int32_t ntrial;         // <= DT
     int32_t stage0;
     int32_t nstage;
+    int32_t skew0;          // first entry of the tile's DT per-trial output skews (RangePlan::skew)
+    int32_t pad_[3];
 };
 
 struct RangePlan {
@@ -91,6 +93,8 @@ struct RangePlan {
     std::vector<StageIndex> sidx;
     std::vector<RowDesc> rows;
     std::vector<uint32_t> blob;
+    std::vector<int32_t> skew;       // [ntiles_dm][DT]: trial i of a tile computes the outputs t0 - skew[i] + [0, kTT)
+    int32_t skew_max = 0;
     int32_t vcap_words = 0;          // words of the variant region; the raw region follows it
     int32_t ntile_t = 0;             // time tiles
     int64_t ngroups = 0, nvariants = 0, ncorrected = 0;   // totals, for reports (ncorrected: variants off the prefix chain)
@@ -113,6 +117,7 @@ struct Plan {
     int32_t opt_group = 8;
     int32_t opt_dm_tile = 64;
     int32_t opt_profile = 0;
+    int32_t opt_skew = 1;            // per-trial output skew inside a DM tile (0: all trials of a tile share t0)
     bool tiling_built = false;
     int64_t launches = 0;
     DeviceState* dev = nullptr;

@@ -18,7 +18,8 @@ void launch_dedisp_naive(const T* y, int64_t row_stride, int64_t beam_stride, co
 
 int launch_dedisp_tiled(bool is_u16, int DT, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
                         int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
-                        const uint32_t* blob, int32_t vcap_words, const int32_t* nout, const int64_t* offset,
+                        const uint32_t* blob, const int32_t* skew, int32_t skew_max, int32_t vcap_words, const int32_t* nout,
+                        const int64_t* offset,
                         int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, cudaStream_t st);
 
 struct SpsArgs {

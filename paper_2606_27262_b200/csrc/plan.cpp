@@ -112,18 +112,20 @@ inline int popcount32(uint32_t x) { return __builtin_popcount(x); }
 // base sum); a channel whose relative delay reaches s_j + L over the tile has L entries, at s_j .. s_j+L-1, and the
 // delta of the entry at level l (sample one later minus sample) moves the channel from s_j+l to s_j+l+1: bit
 // "tau_j > l".  Bits sorted by how often they are set form the prefix chain.
+// skew[i] (tile local): trial i's output window starts skew[i] samples early, i.e. its effective delays are
+// delay - skew[i] (they may be negative); relative delays between channels do not change.
 static bool make_group(const Plan& p, const RangePlan& rp, int32_t d0, int32_t ntrial, int32_t c0, int G, int es,
-                       PendingGroup& g) {
+                       const int32_t* skew, PendingGroup& g) {
     g.chan0 = c0;
-    int32_t dmin = INT32_MAX, dmax = 0;
+    int32_t dmin = INT32_MAX, dmax = INT32_MIN;
     for (int i = 0; i < ntrial; ++i) {
-        const int32_t v = rp.delay[(size_t)(d0 + i) * p.nchan + c0];
+        const int32_t v = rp.delay[(size_t)(d0 + i) * p.nchan + c0] - skew[i];
         dmin = std::min(dmin, v); dmax = std::max(dmax, v);
     }
     g.dmin = dmin;
     g.vlen = (int32_t)round_up(kH + (dmax - dmin), 4);
     g.b.resize(ntrial);
-    for (int i = 0; i < ntrial; ++i) g.b[i] = rp.delay[(size_t)(d0 + i) * p.nchan + c0] - dmin;
+    for (int i = 0; i < ntrial; ++i) g.b[i] = rp.delay[(size_t)(d0 + i) * p.nchan + c0] - skew[i] - dmin;
     g.var_of.assign(ntrial, 0);
     // the group shrinks until its entries fit the kernel's registers and the variants are few (widely spaced
     // channels at high DM have a different relative delay for every trial: nothing to share)
@@ -214,7 +216,37 @@ int build_tiling(Plan& p) {
     for (RangePlan& rp : p.ranges) {
         rp.tiles.clear(); rp.sidx.clear(); rp.rows.clear(); rp.blob.clear();
         rp.ngroups = rp.nvariants = rp.ncorrected = 0;
-        rp.ntile_t = (int32_t)((rp.max_nout + kTT - 1) / kTT);
+        // Output skew per trial: trial i of a DM tile computes the outputs t0 - skew[i] + [0, kTT)
+        // with skew[i] = delay[i][cref] - delay[0][cref], so that at channel cref all trials of the tile read the same
+        // window and elsewhere the windows spread by |delay slope(c) - delay slope(cref)| only.  cref minimises the sum
+        // of the spreads over the band.
+        rp.skew.assign((size_t)((rp.ndm + DT - 1) / DT) * DT, 0);
+        rp.skew_max = 0;
+        for (int32_t d0 = 0; d0 < rp.ndm && p.opt_skew; d0 += DT) {
+            const int32_t nt = std::min(DT, rp.ndm - d0);
+            int64_t best = -1;
+            int32_t best_c = 0;
+            for (int32_t cref = 0; cref < p.nchan; cref += std::max(1, p.nchan / 64)) {
+                int64_t sum = 0;
+                for (int32_t c = 0; c < p.nchan; c += 8) {
+                    int32_t lo = INT32_MAX, hi = INT32_MIN;
+                    for (int i = 0; i < nt; ++i) {
+                        const int32_t* row = &rp.delay[(size_t)(d0 + i) * p.nchan];
+                        const int32_t v = row[c] - (row[cref] - rp.delay[(size_t)d0 * p.nchan + cref]);
+                        lo = std::min(lo, v); hi = std::max(hi, v);
+                    }
+                    sum += hi - lo;
+                }
+                if (best < 0 || sum < best) { best = sum; best_c = cref; }
+            }
+            for (int i = 0; i < DT; ++i) {
+                const int ii = std::min(i, nt - 1);
+                const int32_t sk = rp.delay[(size_t)(d0 + ii) * p.nchan + best_c] - rp.delay[(size_t)d0 * p.nchan + best_c];
+                rp.skew[(size_t)(d0 / DT) * DT + i] = sk;      // >= 0: delays grow with DM
+                rp.skew_max = std::max(rp.skew_max, sk);
+            }
+        }
+        rp.ntile_t = (int32_t)((rp.max_nout + rp.skew_max + kTT - 1) / kTT);
         const int es = rp.decim == 1 ? 1 : 2;
         // 16-bit lanes hold sums of at most floor(65535 / (255*decim)) channel samples
         const int lane_channels = 65535 / (255 * rp.decim);
@@ -226,7 +258,7 @@ int build_tiling(Plan& p) {
             int64_t vb = 0, rb = 0;
             for (int32_t c = 0; c < p.nchan;) {
                 PendingGroup g;
-                if (!make_group(p, rp, d0, nt, c, G, es, g)) return SPT_ERR_UNSUPPORTED;
+                if (!make_group(p, rp, d0, nt, c, G, es, &rp.skew[(size_t)(d0 / DT) * DT], g)) return SPT_ERR_UNSUPPORTED;
                 vb += (int64_t)g.vwords * 4; rb += g.raw_bytes;
                 c += g.nch;
             }
@@ -238,7 +270,8 @@ int build_tiling(Plan& p) {
         const int64_t rcap_bytes = kSmemDataBytes - (int64_t)rp.vcap_words * 4;
 
         for (int32_t d0 = 0; d0 < rp.ndm; d0 += DT) {
-            TileDesc td;
+            TileDesc td{};
+            td.skew0 = (d0 / DT) * DT;
             td.trial0 = d0;
             td.ntrial = std::min(DT, rp.ndm - d0);
             td.stage0 = (int32_t)rp.sidx.size();
@@ -348,7 +381,7 @@ int build_tiling(Plan& p) {
             };
             for (int32_t c = 0; c < p.nchan;) {
                 PendingGroup g;
-                if (!make_group(p, rp, d0, td.ntrial, c, G, es, g)) return SPT_ERR_UNSUPPORTED;
+                if (!make_group(p, rp, d0, td.ntrial, c, G, es, &rp.skew[(size_t)(d0 / DT) * DT], g)) return SPT_ERR_UNSUPPORTED;
                 c += g.nch;
                 if (g.vwords > rp.vcap_words || g.raw_bytes > rcap_bytes || blob_words_of({}, &g) * 4 > kBlobBytes)
                     return SPT_ERR_UNSUPPORTED;  // one group must fit a stage

@@ -64,7 +64,8 @@ def test_options_and_state_errors(api):
     p.set_option("group", 8)
     p.set_option("dm_tile", 32)
     p.set_option("dedisp_kernel", 1)
-    for name, v in (("group", 3), ("dm_tile", 48), ("dedisp_kernel", 2), ("nonsense", 1)):
+    p.set_option("skew", 0)
+    for name, v in (("group", 3), ("dm_tile", 48), ("dedisp_kernel", 2), ("skew", 2), ("nonsense", 1)):
         with pytest.raises(api.SptError) as e:
             p.set_option(name, v)
         assert e.value.code == api.SPT_ERR_INVALID
@@ -92,12 +93,12 @@ def test_plan_cfg4_zero_length_trials(api, orc, synth):
     check_plan_against_oracle(orc, p, w, stride=499)
 
 
-@pytest.mark.parametrize("group,dm_tile", [(1, 64), (2, 64), (4, 64), (8, 64), (4, 32)])
-def test_tiling_tables_reproduce_the_delay_table(api, synth, group, dm_tile):
-    """Host logic of the tiled kernel: the (window, variant, offset) factorisation gives back every delay."""
+@pytest.mark.parametrize("group,dm_tile,skew", [(1, 64, 1), (2, 64, 1), (4, 64, 1), (8, 64, 1), (4, 32, 1), (8, 64, 0)])
+def test_tiling_tables_reproduce_the_delay_table(api, synth, group, dm_tile, skew):
+    """Host logic of the tiled kernel: the (skew, window, variant, offset) factorisation gives back every delay."""
     for cfg, stride in ((1, 1), (3, 173)):
         w = synth.workload(cfg)
-        p = make_plan(api, w, options={"group": group, "dm_tile": dm_tile})
+        p = make_plan(api, w, options={"group": group, "dm_tile": dm_tile, "skew": skew})
         for d in list(range(0, p.ntrials, stride)) + [p.ntrials - 1]:
             assert np.array_equal(p.tiling_delays(d), p.delays(d)), (cfg, d)
         for r in range(len(w.ranges)):

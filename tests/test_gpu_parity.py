@@ -47,6 +47,7 @@ def oracle_path(orc, w, fb, search=True):
 @pytest.mark.parametrize("options", [
     {"dedisp_kernel": 1},
     {"group": 1}, {"group": 2}, {"group": 4}, {"group": 8}, {"group": 4, "dm_tile": 32}, {"group": 8, "dm_tile": 32},
+    {"group": 8, "skew": 0},
 ])
 def test_cfg1_dm_transform_bit_exact(cuda, api, orc, synth, options):
     w = synth.workload(1)
@@ -93,7 +94,8 @@ def mini3(synth, seed, nsamp=65536, nchan=1024):
     return w
 
 
-@pytest.mark.parametrize("options", [{"group": 4}, {"group": 8}, {"group": 2, "dm_tile": 32}, {"dedisp_kernel": 1}])
+@pytest.mark.parametrize("options", [{"group": 4}, {"group": 8}, {"group": 2, "dm_tile": 32}, {"dedisp_kernel": 1},
+                                     {"group": 8, "skew": 0}])
 def test_multirange_decimated_bit_exact(cuda, api, orc, synth, options):
     w = mini3(synth, 11)
     fb = synth.generate(w)
