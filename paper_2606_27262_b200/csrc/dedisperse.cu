@@ -281,17 +281,21 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
 
     const T* in = reinterpret_cast<const T*>(a.in) + (int64_t)beam * a.beam_stride;
 
-    // T: the elected warp issues the bulk copies of stage s (table blob, raw rows, and the NEXT stage's index and row
-    // descriptors, so that no global-memory latency sits between a stage's pre-sum and its gather), then arms the
-    // barrier with the byte count.  Stage 0 reads its descriptors from global memory, later stages from shared.
+    // T: every warp issues its share of the bulk copies of stage s (a warp issues the copies of its lanes one after the
+    // other, so eight short chains instead of one long one) and arrives on the stage barrier with the byte count of its
+    // share: rows k = warp, warp + NW, ...; warp 0 also copies the table blob and the NEXT stage's index and row
+    // descriptors, so that no global-memory latency sits between a stage's pre-sum and its gather.  Stage 0 reads its
+    // descriptors from global memory, later stages from shared.
     auto issue_stage = [&](int s) {
         const StageIndex si = s == 0 ? a.sidx[td.stage0] : s_sidx[s & 1];
         const RowDesc* rows = s == 0 ? a.rows + si.row0 : s_rows + (s & 1) * kMaxStageRows;
-        if (lane == 0) fence_proxy_async();  // generic-proxy reads of the buffers (previous stage) before async-proxy writes
-        __syncwarp();
         uint32_t bytes = 0;
-        for (uint32_t k = lane; k < si.nrows; k += 32) {
-            const RowDesc r = rows[k];
+        const uint32_t k = (uint32_t)warp + (uint32_t)NW * (uint32_t)lane;
+        RowDesc r{0, 0, 0, 0};
+        if (k < si.nrows) r = rows[k];
+        __syncwarp();
+        fence_proxy_async();  // generic-proxy reads of the buffers (previous stage) before async-proxy writes
+        if (k < si.nrows) {
             // the window [pos, pos + nelem) of the channel's row, clipped to the row: the part before the row (skewed
             // output windows start before t = 0) and the part after it are not copied (all multiples of 16 elements)
             const int64_t pos = t0 + r.astart;
@@ -301,20 +305,23 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
             if (n > 0)
                 bulk_g2s(smem_u32(s_rawb + r.soff) + (uint32_t)(beg - pos) * (uint32_t)sizeof(T),
                          in + (int64_t)r.chan * a.row_stride + beg, (uint32_t)n * (uint32_t)sizeof(T), bar);
-            bytes += (uint32_t)n * (uint32_t)sizeof(T);
+            bytes = (uint32_t)n * (uint32_t)sizeof(T);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) bytes += __shfl_xor_sync(0xffffffffu, bytes, o);
         if (lane == 0) {
-            bulk_g2s(smem_u32(smem + kSmemCtrlBytes + (s & 1) * kBlobBytes), a.blob + si.blob_word0, si.blob_words * 4u, bar);
-            bulk_g2s(smem_u32(s_sidx + ((s + 1) & 1)), a.sidx + td.stage0 + s + 1, 16u, bar);
-            bulk_g2s(smem_u32(s_rows + ((s + 1) & 1) * kMaxStageRows), a.rows + si.row0 + si.nrows, kMaxStageRows * 16u, bar);
-            mbar_expect_tx(bar, bytes + si.blob_words * 4u + 16u + kMaxStageRows * 16u);   // the arrival that lets the phase end
+            if (warp == 0) {
+                bulk_g2s(smem_u32(smem + kSmemCtrlBytes + (s & 1) * kBlobBytes), a.blob + si.blob_word0, si.blob_words * 4u, bar);
+                bulk_g2s(smem_u32(s_sidx + ((s + 1) & 1)), a.sidx + td.stage0 + s + 1, 16u, bar);
+                bulk_g2s(smem_u32(s_rows + ((s + 1) & 1) * kMaxStageRows), a.rows + si.row0 + si.nrows, kMaxStageRows * 16u, bar);
+                bytes += si.blob_words * 4u + 16u + kMaxStageRows * 16u;
+            }
+            mbar_expect_tx(bar, bytes);   // one of the NW arrivals that let the phase end
         }
     };
 
     if (tid == 0) {
-        mbar_init(bar, 1);
+        mbar_init(bar, NW);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         fence_proxy_async();
     }
@@ -338,7 +345,7 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
         for (int i = tid; i < n4; i += kThreads) r4[i] = make_uint4(0u, 0u, 0u, 0u);
         __syncthreads();
     }
-    if (warp == 0) issue_stage(0);
+    issue_stage(0);
 
     uint32_t acc[TPW][NJ];
 #pragma unroll
@@ -359,7 +366,7 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
         for (int tk = warp; tk < ntask; tk += NW)
             presum_task<T>(tb, tb[kBlobHdrWords + 4 * ngrp + tk], var_addr, raw_addr, lane);
         __syncthreads();  // variants complete; raw rows and the other blob buffer are free
-        if (warp == 0 && s + 1 < td.nstage) issue_stage(s + 1);
+        if (s + 1 < td.nstage) issue_stage(s + 1);
 
         // ---- C: gather-accumulate ------------------------------------------------------------------------------
         {
