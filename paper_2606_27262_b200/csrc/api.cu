@@ -490,7 +490,7 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
             for (int32_t k = 0; k <= ntog; ++k)
                 if (vd[k] == (uint32_t)(vbase + r * vlen)) bits = (1u << k) - 1u;
             for (int32_t c = 0; c < ncorr; ++c)
-                if (vd[ntog + 1 + 2 * c] == (uint32_t)(vbase + r * vlen)) bits = ((1u << ntog) - 1u) & ~vd[ntog + 2 + 2 * c];
+                if (vd[kChainWords + 2 * c] == (uint32_t)(vbase + r * vlen)) bits = ((1u << ntog) - 1u) & ~vd[kChainWords + 1 + 2 * c];
             if (bits == 0xffffffffu) return SPT_ERR_STATE;
             for (int pass = 0; pass < 2; ++pass)       // pass 0: base shifts; pass 1: one sample later per delta taken
                 for (int32_t q = 0; q < nch; ++q) {

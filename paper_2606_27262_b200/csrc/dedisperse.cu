@@ -203,12 +203,12 @@ __device__ __forceinline__ void load_entry(uint32_t addr, uint32_t c1, uint32_t 
 template <typename T>
 __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uint32_t task, uint32_t var_addr,
                                             uint32_t raw_addr, int lane) {
-    const uint32_t* gh = tb + kBlobHdrWords + 4 * (task & 0xffu);
-    const int vlen = (int)gh[1];
-    const uint32_t meta = gh[2];
+    const uint4 gh = *reinterpret_cast<const uint4*>(tb + kBlobHdrWords + 4 * (task & 0xffu));   // 128-bit broadcast loads
+    const int vlen = (int)gh.y;
+    const uint32_t meta = gh.z;
     const int ntog = (int)((meta >> 8) & 0xffu), ncorr = (int)((meta >> 16) & 0xffu);
-    const uint2* cd = reinterpret_cast<const uint2*>(tb + (gh[3] & 0xffffu));
-    const uint32_t* vd = tb + (gh[3] >> 16);
+    const uint4* cd = reinterpret_cast<const uint4*>(tb + (gh.w & 0xffffu));
+    const uint4* vd = reinterpret_cast<const uint4*>(tb + (gh.w >> 16));
     int u0 = (int)(task >> 8) * kChunkU + lane * 4;
     const bool active = u0 < vlen;                // vlen is a multiple of 4
     u0 = active ? u0 : vlen - 4;
@@ -217,18 +217,24 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
     uint32_t cur[4] = {0u, 0u, 0u, 0u};
     uint32_t dl[kMaxG][4];
 #pragma unroll
-    for (int q = 0; q < kMaxG; ++q) {
-        const uint2 c = cd[q];
-        uint32_t w[5];
-        load_entry<T>(rbase + (c.x & 0x3ffffu), c.y, w);
+    for (int q2 = 0; q2 < kMaxG / 2; ++q2) {
+        const uint4 c2 = cd[q2];                  // two entries per load
 #pragma unroll
-        for (int i = 0; i < 4; ++i) dl[q][i] = w[i + 1] - w[i];
-        if (c.x & kEntryAddBase) {
+        for (int h = 0; h < 2; ++h) {
+            const int q = 2 * q2 + h;
+            const uint32_t cx = h ? c2.z : c2.x, cy = h ? c2.w : c2.y;
+            uint32_t w[5];
+            load_entry<T>(rbase + (cx & 0x3ffffu), cy, w);
 #pragma unroll
-            for (int i = 0; i < 4; ++i) cur[i] += w[i];
+            for (int i = 0; i < 4; ++i) dl[q][i] = w[i + 1] - w[i];
+            if (cx & kEntryAddBase) {
+#pragma unroll
+                for (int i = 0; i < 4; ++i) cur[i] += w[i];
+            }
         }
     }
     // prefix chain: after step k, cur = base sum + deltas of the first k entries
+    uint4 v4 = vd[0];
 #pragma unroll
     for (int k = 0; k <= kMaxG; ++k) {
         if (k <= ntog) {
@@ -236,13 +242,15 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
 #pragma unroll
                 for (int i = 0; i < 4; ++i) cur[i] += dl[k - 1][i];
             }
-            const uint32_t dst = vd[k];
+            if (k > 0 && (k & 3) == 0) v4 = vd[k >> 2];
+            const uint32_t dst = (k & 3) == 0 ? v4.x : (k & 3) == 1 ? v4.y : (k & 3) == 2 ? v4.z : v4.w;
             if (dst != 0xffffffffu && active) sts128(vbase + dst * 4u, cur[0], cur[1], cur[2], cur[3]);
         }
     }
     // variants off the chain (few): all deltas, minus those the variant does not take
     for (int c = 0; c < ncorr; ++c) {
-        const uint32_t dst = vd[ntog + 1 + 2 * c], mask = vd[ntog + 2 + 2 * c];
+        const uint32_t* vc = reinterpret_cast<const uint32_t*>(vd) + kChainWords + 2 * c;
+        const uint32_t dst = vc[0], mask = vc[1];
         uint32_t o[4] = {cur[0], cur[1], cur[2], cur[3]};
 #pragma unroll
         for (int q = 0; q < kMaxG; ++q)

@@ -48,11 +48,13 @@ constexpr int kSmemDataBytes = kSmemBytes - kSmemCtrlBytes - 2 * kBlobBytes;  //
 //                 it to the base sum.  The entry's delta (sample one later minus sample) moves its channel one later.
 //                 Second word: what the kernel's realignment needs (uint8: bits 0-4 funnel-shift amount, bits 8-23 PRMT
 //                 selector of the fifth sample; uint16: bit 0 = odd position).
-//   vdesc         per group: ntog + 1 chain words, word k = offset in the variant region of the variant "base sum +
-//                 deltas of the first k entries" (0xffffffff: no trial uses it); then ncorr x { offset, mask } for the
-//                 variants off the chain: all ntog deltas minus those in mask
+//   vdesc         per group: kChainWords chain words, word k <= ntog = offset in the variant region of the variant "base sum
+//                 + deltas of the first k entries" (0xffffffff: no trial uses it); then ncorr x { offset, mask } for the
+//                 variants off the chain: all ntog deltas minus those in mask.  Headers, cdesc and vdesc are 16-byte
+//                 aligned: the kernel reads them with 128-bit broadcast loads.
 //   trial_off     ngrp x DT uint16 = word offset of the trial's read start in the variant region
 constexpr int kBlobHdrWords = 4;
+constexpr int kChainWords = 12;      // chain words of a group's vdesc, padded (kMaxG + 1 used at most); corrections follow
 constexpr uint32_t kEntryAddBase = 1u << 26;
 
 struct RowDesc {            // one raw channel row of a stage; 16 bytes

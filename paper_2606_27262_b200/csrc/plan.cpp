@@ -281,7 +281,7 @@ int build_tiling(Plan& p) {
             auto blob_words_of = [&](const std::vector<PendingGroup>& gs, const PendingGroup* extra) {
                 int64_t w = kBlobHdrWords + 4;
                 auto one = [&](const PendingGroup& g) {
-                    w += 4 + (g.vlen + kChunkU - 1) / kChunkU + 2 * kMaxG + (g.ntog + 1) + 2 * g.ncorrected + DT / 2;
+                    w += 4 + (g.vlen + kChunkU - 1) / kChunkU + 2 * kMaxG + kChainWords + 2 * g.ncorrected + 3 + DT / 2;
                 };
                 for (const PendingGroup& g : gs) one(g);
                 if (extra) one(*extra);
@@ -306,7 +306,7 @@ int build_tiling(Plan& p) {
                     for (int ch = 0; ch < (open[k].vlen + kChunkU - 1) / kChunkU; ++ch)
                         tasks.push_back((uint32_t)k | ((uint32_t)ch << 8));
                 const uint32_t ntask = (uint32_t)tasks.size();
-                if ((hdr.size() + tasks.size()) % 2) tasks.push_back(0xffffffffu);   // 64-bit loads of the entry descriptors
+                while ((hdr.size() + tasks.size()) % 4) tasks.push_back(0xffffffffu);   // 128-bit loads of the descriptors
                 const uint32_t cdesc0 = (uint32_t)(hdr.size() + tasks.size());
                 for (size_t k = 0; k < ngrp; ++k) {
                     PendingGroup& g = open[k];
@@ -354,12 +354,14 @@ int build_tiling(Plan& p) {
                             if (g.vars[r].k == k2 && !(g.vars[r].plus | g.vars[r].minus)) dst = (uint32_t)(vbase + r * g.vlen);
                         vdesc.push_back(dst);
                     }
+                    for (int k2 = g.ntog + 1; k2 < kChainWords; ++k2) vdesc.push_back(0xffffffffu);   // three 128-bit loads
                     // off the chain: destination and the mask of the deltas NOT taken (subtracted from the full sum)
                     for (int r = 0; r < g.nvar; ++r)
                         if (g.vars[r].plus | g.vars[r].minus) {
                             vdesc.push_back((uint32_t)(vbase + r * g.vlen));
                             vdesc.push_back(~g.vars[r].bits & ((1u << g.ntog) - 1u));
                         }
+                    while (vdesc.size() % 4) vdesc.push_back(0);
                     vbase += g.vwords;
                 }
                 hdr[0] = (uint32_t)ngrp; hdr[1] = flush ? 1u : 0u; hdr[2] = ntask;
