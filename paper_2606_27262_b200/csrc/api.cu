@@ -39,6 +39,7 @@ struct DeviceState {
     std::vector<RangeDev> r;
     int32_t* nout = nullptr;        // [ntrials]
     int64_t* offset = nullptr;      // [ntrials]
+    uint32_t* maxval = nullptr;     // [nranges] largest sample of the series each range read in the last dedisperse
     int32_t* range_lo = nullptr;    // [ntrials] first / last trial of the trial's DM range (peak filter)
     int32_t* range_hi = nullptr;
     // peak filter (lazily allocated): lookup plane laid out like the DM transform, live flags, peak list
@@ -120,7 +121,7 @@ static void free_device(Plan* p) {
         cudaFree(r.delay); cudaFree(r.tiles); cudaFree(r.sidx); cudaFree(r.rows); cudaFree(r.blob); cudaFree(r.skew);
         cudaFree(r.series);
     }
-    cudaFree(d->nout); cudaFree(d->offset); cudaFree(d->range_lo); cudaFree(d->range_hi);
+    cudaFree(d->maxval); cudaFree(d->nout); cudaFree(d->offset); cudaFree(d->range_lo); cudaFree(d->range_hi);
     cudaFree(d->plane); cudaFree(d->alive[0]); cudaFree(d->alive[1]); cudaFree(d->peaks); cudaFree(d->peaks_count);
     for (auto& b : d->bufs) { cudaFree(b.sum); cudaFree(b.sumsq); cudaFree(b.cand); cudaFree(b.count); }
     for (auto& sl : d->slot) {
@@ -190,6 +191,10 @@ static int ensure_device(Plan* p) {
     }
     if (rc == SPT_OK) rc = upload(&d->nout, nout_all);
     if (rc == SPT_OK) rc = upload(&d->offset, off_all);
+    if (rc == SPT_OK) {
+        cudaError_t ce = cudaMalloc((void**)&d->maxval, sizeof(uint32_t) * p->ranges.size());
+        if (ce != cudaSuccess) rc = cuda_fail(ce, "maxval");
+    }
     if (rc == SPT_OK) rc = upload(&d->range_lo, lo_all);
     if (rc == SPT_OK) rc = upload(&d->range_hi, hi_all);
     if (rc == SPT_OK) rc = alloc_search_bufs(p, d->bufs[0]);
@@ -220,13 +225,20 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
         in_stride = pitch;
     }
     timed_clear(d, 0);
+    // largest sample of every series (bounds the 16-bit lanes of the dedispersion)
+    SPT_CUDA(cudaMemsetAsync(d->maxval, 0, sizeof(uint32_t) * p->ranges.size(), st));
+    for (size_t i = 0; i < p->ranges.size(); ++i)
+        if (p->ranges[i].decim == 1 && p->ranges[i].max_nout > 0) {
+            launch_max_u8(in, (int64_t)nbeam * p->nchan * in_stride, d->maxval + i, st);
+            p->launches++;
+        }
     // a2: decimated series of every range that needs one
     for (size_t i = 0; i < p->ranges.size(); ++i) {
         const RangePlan& rp = p->ranges[i];
         if (rp.decim == 1 || rp.nsamp_k <= 0) continue;
         ScopedTimer tm(p, st, 0, 1, (int)i);
         launch_decimate(in, in_stride, (int64_t)p->nchan * in_stride, d->r[i].series, rp.stride_k,
-                        (int64_t)p->nchan * rp.stride_k, p->nchan, nbeam, rp.nsamp_k, rp.decim, st);
+                        (int64_t)p->nchan * rp.stride_k, p->nchan, nbeam, rp.nsamp_k, rp.decim, d->maxval + i, st);
         p->launches++;
     }
     // a3: DM transform, range by range
@@ -247,7 +259,7 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
                                               p->nchan, rp.ndm, nbeam, rp.max_nout, d_dmt, p->dmt_elems, st);
         } else {
             const int rc = launch_dedisp_tiled(u16, p->opt_dm_tile, src, rs, (int64_t)p->nchan * rs, d_dmt, p->dmt_elems,
-                                               rd.tiles, rd.sidx, rd.rows, rd.blob, rd.skew, rp.skew_max, rp.vcap_words, nout, off,
+                                               rd.tiles, rd.sidx, rd.rows, rd.blob, d->maxval + i, rd.skew, rp.skew_max, rp.vcap_words, nout, off,
                                                (int32_t)rp.tiles.size(), rp.ntile_t, nbeam, st);
             if (rc != 0) { g_last_error = "dedisp_tiled: launch configuration rejected"; return SPT_ERR_CUDA; }
         }

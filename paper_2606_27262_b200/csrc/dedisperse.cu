@@ -18,10 +18,11 @@ namespace spt {
 // ---------------------------------------------------------------------------------------------------------------
 __global__ void decimate_kernel(const uint8_t* __restrict__ x, int64_t in_row_stride, int64_t in_beam_stride,
                                 uint16_t* __restrict__ y, int64_t out_row_stride, int64_t out_beam_stride,
-                                int32_t nchan, int64_t nsamp_k, int32_t k) {
+                                int32_t nchan, int64_t nsamp_k, int32_t k, uint32_t* __restrict__ maxval) {
     const int64_t quads = (nsamp_k + 3) >> 2;  // groups of 4 outputs per row
     const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= quads) return;
+    uint32_t mx = 0;
+    if (q < quads) {
     const int32_t c = blockIdx.y, b = blockIdx.z;
     const uint8_t* src = x + (int64_t)b * in_beam_stride + (int64_t)c * in_row_stride;
     uint16_t* dst = y + (int64_t)b * out_beam_stride + (int64_t)c * out_row_stride;
@@ -43,23 +44,47 @@ __global__ void decimate_kernel(const uint8_t* __restrict__ x, int64_t in_row_st
         pk.x = o[0] | (o[1] << 16);
         pk.y = o[2] | (o[3] << 16);
         *reinterpret_cast<uint2*>(dst + j0) = pk;
+        mx = max(max(o[0], o[1]), max(o[2], o[3]));
     } else {  // ragged tail of the row
         for (int64_t j = j0; j < nsamp_k; ++j) {
             uint32_t s = 0;
             for (int m = 0; m < k; ++m) s += src[j * k + m];
             dst[j] = (uint16_t)s;
+            mx = max(mx, s);
         }
     }
+    }
+    // largest decimated sample of the launch: bounds how many channels a 16-bit lane of the dedispersion may sum
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    if ((threadIdx.x & 31) == 0 && mx > 0) atomicMax(maxval, mx);
+}
+
+// Largest sample of a uint8 filterbank (the same bound for the ranges that read the raw input).
+__global__ void max_u8_kernel(const uint4* __restrict__ x, int64_t n16, uint32_t* __restrict__ maxval) {
+    uint32_t m = 0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (int64_t)gridDim.x * blockDim.x) {
+        const uint4 v = __ldg(x + i);
+        m = __vmaxu4(__vmaxu4(v.x, v.y), __vmaxu4(__vmaxu4(v.z, v.w), m));
+    }
+    m = max(max(m & 0xffu, (m >> 8) & 0xffu), max((m >> 16) & 0xffu, m >> 24));
+    m = __reduce_max_sync(0xffffffffu, m);
+    if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(maxval, m);
+}
+
+void launch_max_u8(const uint8_t* x, int64_t nbytes, uint32_t* maxval, cudaStream_t st) {
+    const int64_t n16 = nbytes / 16;          // rows are 16-byte multiples
+    if (n16 <= 0) return;
+    max_u8_kernel<<<148 * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(x), n16, maxval);
 }
 
 void launch_decimate(const uint8_t* x, int64_t in_row_stride, int64_t in_beam_stride, uint16_t* y,
                      int64_t out_row_stride, int64_t out_beam_stride, int32_t nchan, int32_t nbeam, int64_t nsamp_k,
-                     int32_t k, cudaStream_t st) {
+                     int32_t k, uint32_t* maxval, cudaStream_t st) {
     const int64_t quads = (nsamp_k + 3) >> 2;
     if (quads <= 0) return;
     dim3 grid((unsigned)((quads + 255) / 256), (unsigned)nchan, (unsigned)nbeam);
     decimate_kernel<<<grid, 256, 0, st>>>(x, in_row_stride, in_beam_stride, y, out_row_stride, out_beam_stride, nchan,
-                                          nsamp_k, k);
+                                          nsamp_k, k, maxval);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -110,7 +135,8 @@ template void launch_dedisp_naive<uint16_t>(const uint16_t*, int64_t, int64_t, c
 //               five samples u..u+4 as packed words w0..w4, base += w_i, delta_i = w_{i+1} - w_i (the alternate shift
 //               is one sample later), then walks the prefix chain: variant k = base + delta of the first k channels.
 //   C  gather : acc[d][q] += P_{r(d)}[q + b(d)]       one LDS.32 + one add = 2*G algorithmic adds
-//   F  flush  : every <= 257/decim channels the 16-bit lanes are widened into the int32 DM transform (L2 RMW).
+//   F  flush  : before a lane could exceed 65535 (every floor(65535 / largest sample of the launch) channels, at worst
+//               every 257/decim) the 16-bit lanes are widened into the int32 DM transform (first time a store, then RED).
 // ---------------------------------------------------------------------------------------------------------------
 struct TiledArgs {
     const void* in;            // series of beam 0
@@ -122,6 +148,7 @@ struct TiledArgs {
     const StageIndex* sidx;
     const RowDesc* rows;
     const uint32_t* blob;
+    const uint32_t* maxval;    // largest input sample of this launch (device scalar): bounds the 16-bit lanes
     const int32_t* skew;       // [ntile_dm][DT] output skew of every trial of a DM tile
     int32_t skew_max;
     const int32_t* nout;       // range local
@@ -361,12 +388,39 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
 #pragma unroll
         for (int j = 0; j < NJ; ++j) acc[q][j] = 0u;
     bool first_flush = true;
+    // F: widen the 16-bit lanes into the int32 DM transform.  A lane may sum floor(65535 / largest sample) channels: the
+    // bound comes from the data of this launch (255 * decimation in the worst case, which is what the stages are cut for)
+    const int lane_cap = (int)(65535u / max(1u, __ldg(a.maxval)));
+    int since = 0;
+    auto flush_lanes = [&]() {
+#pragma unroll
+        for (int q = 0; q < TPW; ++q) {
+            const int dl = warp * TPW + q;
+            int32_t* row = s_rowp[dl];
+            const int2 ok = s_valid[dl];
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) {
+                const int i = lane + 32 * j;
+                const int32_t lo = (int32_t)(acc[q][j] & 0xFFFFu), hi = (int32_t)(acc[q][j] >> 16);
+                const bool ok_lo = i >= ok.x && i < ok.y, ok_hi = i + kH >= ok.x && i + kH < ok.y;
+                if (first_flush) {
+                    if (ok_lo) row[i] = lo;
+                    if (ok_hi) row[i + kH] = hi;
+                } else {
+                    if (ok_lo) atomicAdd(row + i, lo);          // result unused: a fire-and-forget RED in L2
+                    if (ok_hi) atomicAdd(row + i + kH, hi);
+                }
+                acc[q][j] = 0u;
+            }
+        }
+        first_flush = false;
+    };
 
     for (int s = 0; s < td.nstage; ++s) {
         mbar_wait(bar, (uint32_t)(s & 1));
         const uint32_t* tb = reinterpret_cast<const uint32_t*>(smem + kSmemCtrlBytes + (s & 1) * kBlobBytes);
         const int ngrp = (int)tb[0];
-        const bool flush = tb[1] != 0u;
+        const int nch_stage = (int)(tb[1] >> 8);      // channels this stage adds to every lane
         const int ntask = (int)tb[2];
         const uint16_t* toff = reinterpret_cast<const uint16_t*>(tb + tb[3]);
 
@@ -376,6 +430,7 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
         __syncthreads();  // variants complete; raw rows and the other blob buffer are free
         if (s + 1 < td.nstage) issue_stage(s + 1);
 
+        if (since + nch_stage > lane_cap) { flush_lanes(); since = 0; }
         // ---- C: gather-accumulate ------------------------------------------------------------------------------
         {
             const uint32_t lane_addr = var_addr + (uint32_t)lane * 4u;
@@ -413,32 +468,10 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
                 }
             }
         }
-        // ---- F: widen the 16-bit lanes into the int32 DM transform -------------------------------------------
-        if (flush) {
-#pragma unroll
-            for (int q = 0; q < TPW; ++q) {
-                const int dl = warp * TPW + q;
-                int32_t* row = s_rowp[dl];
-                const int2 ok = s_valid[dl];
-#pragma unroll
-                for (int j = 0; j < NJ; ++j) {
-                    const int i = lane + 32 * j;
-                    const int32_t lo = (int32_t)(acc[q][j] & 0xFFFFu), hi = (int32_t)(acc[q][j] >> 16);
-                    const bool ok_lo = i >= ok.x && i < ok.y, ok_hi = i + kH >= ok.x && i + kH < ok.y;
-                    if (first_flush) {
-                        if (ok_lo) row[i] = lo;
-                        if (ok_hi) row[i + kH] = hi;
-                    } else {
-                        if (ok_lo) atomicAdd(row + i, lo);          // result unused: a fire-and-forget RED in L2
-                        if (ok_hi) atomicAdd(row + i + kH, hi);
-                    }
-                    acc[q][j] = 0u;
-                }
-            }
-            first_flush = false;
-        }
+        since += nch_stage;
         __syncthreads();  // everyone is done with this stage's variants
     }
+    flush_lanes();
 }
 
 template <typename T, int DT>
@@ -458,9 +491,9 @@ static int launch_tiled_inst(const TiledArgs& a, cudaStream_t st) {
 
 int launch_dedisp_tiled(bool is_u16, int DT, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
                         int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
-                        const uint32_t* blob, const int32_t* skew, int32_t skew_max, int32_t vcap_words, const int32_t* nout,
-                        const int64_t* offset, int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, cudaStream_t st) {
-    TiledArgs a{in, row_stride, beam_stride, out, out_beam_stride, tiles, sidx, rows, blob, skew, skew_max, nout, offset,
+                        const uint32_t* blob, const uint32_t* maxval, const int32_t* skew, int32_t skew_max, int32_t vcap_words,
+                        const int32_t* nout, const int64_t* offset, int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, cudaStream_t st) {
+    TiledArgs a{in, row_stride, beam_stride, out, out_beam_stride, tiles, sidx, rows, blob, maxval, skew, skew_max, nout, offset,
                 vcap_words, ntile_dm, ntile_t, nbeam};
     if (DT == 64) return is_u16 ? launch_tiled_inst<uint16_t, 64>(a, st) : launch_tiled_inst<uint8_t, 64>(a, st);
     if (DT == 32) return is_u16 ? launch_tiled_inst<uint16_t, 32>(a, st) : launch_tiled_inst<uint8_t, 32>(a, st);

@@ -36,7 +36,7 @@ constexpr int kSmemCtrlBytes = 64 + kMaxDT * 16 + 2 * (kMaxStageRows * 16 + 16);
 constexpr int kSmemDataBytes = kSmemBytes - kSmemCtrlBytes - 2 * kBlobBytes;  // variant region + raw-row region
 
 // Per-stage blob, 32-bit words (copied to shared memory with one bulk copy):
-//   [0] ngrp  [1] flush  [2] ntask  [3] word offset of the trial_off table
+//   [0] ngrp  [1] (worst-case lane interval ends here) | channels of the stage << 8  [2] ntask  [3] word offset of the trial_off table
 //   [4 ..)        ngrp x { vbase, vlen, nent | ntog << 8 | ncorr << 16 | nvar << 24, cdesc_off | vdesc_off << 16 }
 //                 (offsets inside the blob)
 //   task table    ntask x { group | chunk << 8 }: warp task = kChunkU variant words of every variant of one group

@@ -9,7 +9,8 @@ namespace spt {
 
 void launch_decimate(const uint8_t* x, int64_t in_row_stride, int64_t in_beam_stride, uint16_t* y,
                      int64_t out_row_stride, int64_t out_beam_stride, int32_t nchan, int32_t nbeam, int64_t nsamp_k,
-                     int32_t k, cudaStream_t st);
+                     int32_t k, uint32_t* maxval, cudaStream_t st);
+void launch_max_u8(const uint8_t* x, int64_t nbytes, uint32_t* maxval, cudaStream_t st);
 
 template <typename T>
 void launch_dedisp_naive(const T* y, int64_t row_stride, int64_t beam_stride, const int32_t* d_delay,
@@ -18,8 +19,8 @@ void launch_dedisp_naive(const T* y, int64_t row_stride, int64_t beam_stride, co
 
 int launch_dedisp_tiled(bool is_u16, int DT, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
                         int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
-                        const uint32_t* blob, const int32_t* skew, int32_t skew_max, int32_t vcap_words, const int32_t* nout,
-                        const int64_t* offset,
+                        const uint32_t* blob, const uint32_t* maxval, const int32_t* skew, int32_t skew_max, int32_t vcap_words,
+                        const int32_t* nout, const int64_t* offset,
                         int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, cudaStream_t st);
 
 struct SpsArgs {

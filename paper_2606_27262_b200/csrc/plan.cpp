@@ -290,7 +290,7 @@ int build_tiling(Plan& p) {
             auto close_stage = [&](bool flush) {
                 if (open.empty()) {
                     if (flush && (int32_t)rp.sidx.size() > td.stage0) {
-                        rp.blob[rp.sidx.back().blob_word0 + 1] = 1;
+                        rp.blob[rp.sidx.back().blob_word0 + 1] |= 1u;
                         since_flush = 0;
                     }
                     return;
@@ -364,7 +364,9 @@ int build_tiling(Plan& p) {
                     while (vdesc.size() % 4) vdesc.push_back(0);
                     vbase += g.vwords;
                 }
-                hdr[0] = (uint32_t)ngrp; hdr[1] = flush ? 1u : 0u; hdr[2] = ntask;
+                int nch_stage = 0;
+                for (const PendingGroup& g : open) nch_stage += g.nch;
+                hdr[0] = (uint32_t)ngrp; hdr[1] = (flush ? 1u : 0u) | ((uint32_t)nch_stage << 8); hdr[2] = ntask;
                 while ((vdesc0 + vdesc.size()) % 4) vdesc.push_back(0);   // trial_off rows are read with 128-bit loads
                 hdr[3] = vdesc0 + (uint32_t)vdesc.size();
                 rp.blob.insert(rp.blob.end(), hdr.begin(), hdr.end());
