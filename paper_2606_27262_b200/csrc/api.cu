@@ -39,7 +39,7 @@ struct DeviceState {
     std::vector<RangeDev> r;
     int32_t* nout = nullptr;        // [ntrials]
     int64_t* offset = nullptr;      // [ntrials]
-    uint32_t* maxval = nullptr;     // [nranges] largest sample of the series each range read in the last dedisperse
+    uint32_t* maxval = nullptr;     // [nranges][2] largest and smallest sample of the series each range read last
     int32_t* range_lo = nullptr;    // [ntrials] first / last trial of the trial's DM range (peak filter)
     int32_t* range_hi = nullptr;
     // peak filter (lazily allocated): lookup plane laid out like the DM transform, live flags, peak list
@@ -192,7 +192,7 @@ static int ensure_device(Plan* p) {
     if (rc == SPT_OK) rc = upload(&d->nout, nout_all);
     if (rc == SPT_OK) rc = upload(&d->offset, off_all);
     if (rc == SPT_OK) {
-        cudaError_t ce = cudaMalloc((void**)&d->maxval, sizeof(uint32_t) * p->ranges.size());
+        cudaError_t ce = cudaMalloc((void**)&d->maxval, 2 * sizeof(uint32_t) * p->ranges.size());
         if (ce != cudaSuccess) rc = cuda_fail(ce, "maxval");
     }
     if (rc == SPT_OK) rc = upload(&d->range_lo, lo_all);
@@ -226,10 +226,13 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
     }
     timed_clear(d, 0);
     // largest sample of every series (bounds the 16-bit lanes of the dedispersion)
-    SPT_CUDA(cudaMemsetAsync(d->maxval, 0, sizeof(uint32_t) * p->ranges.size(), st));
+    for (size_t i = 0; i < p->ranges.size(); ++i) {     // {largest, smallest} = {0, 0xffffffff}
+        SPT_CUDA(cudaMemsetAsync(d->maxval + 2 * i, 0, 4, st));
+        SPT_CUDA(cudaMemsetAsync(d->maxval + 2 * i + 1, 0xff, 4, st));
+    }
     for (size_t i = 0; i < p->ranges.size(); ++i)
         if (p->ranges[i].decim == 1 && p->ranges[i].max_nout > 0) {
-            launch_max_u8(in, (int64_t)nbeam * p->nchan * in_stride, d->maxval + i, st);
+            launch_max_u8(in, (int64_t)nbeam * p->nchan * in_stride, d->maxval + 2 * i, st);
             p->launches++;
         }
     // a2: decimated series of every range that needs one
@@ -238,8 +241,9 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
         if (rp.decim == 1 || rp.nsamp_k <= 0) continue;
         ScopedTimer tm(p, st, 0, 1, (int)i);
         launch_decimate(in, in_stride, (int64_t)p->nchan * in_stride, d->r[i].series, rp.stride_k,
-                        (int64_t)p->nchan * rp.stride_k, p->nchan, nbeam, rp.nsamp_k, rp.decim, d->maxval + i, st);
-        p->launches++;
+                        (int64_t)p->nchan * rp.stride_k, p->nchan, nbeam, rp.nsamp_k, rp.decim, st);
+        launch_max_u16(d->r[i].series, (int64_t)nbeam * p->nchan * rp.stride_k, d->maxval + 2 * i, st);
+        p->launches += 2;
     }
     // a3: DM transform, range by range
     for (size_t i = 0; i < p->ranges.size(); ++i) {
@@ -259,7 +263,7 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
                                               p->nchan, rp.ndm, nbeam, rp.max_nout, d_dmt, p->dmt_elems, st);
         } else {
             const int rc = launch_dedisp_tiled(u16, p->opt_dm_tile, src, rs, (int64_t)p->nchan * rs, d_dmt, p->dmt_elems,
-                                               rd.tiles, rd.sidx, rd.rows, rd.blob, d->maxval + i, rd.skew, rp.skew_max, rp.vcap_words, nout, off,
+                                               rd.tiles, rd.sidx, rd.rows, rd.blob, d->maxval + 2 * i, rd.skew, rp.skew_max, rp.vcap_words, nout, off,
                                                (int32_t)rp.tiles.size(), rp.ntile_t, nbeam, st);
             if (rc != 0) { g_last_error = "dedisp_tiled: launch configuration rejected"; return SPT_ERR_CUDA; }
         }
@@ -488,7 +492,7 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
         const uint16_t* toff = reinterpret_cast<const uint16_t*>(b + b[3]);
         for (uint32_t g = 0; g < ngrp; ++g) {
             const uint32_t* gh = b + kBlobHdrWords + 4 * g;
-            const int32_t vbase = (int32_t)gh[0], vlen = (int32_t)gh[1];
+            const int32_t vbase = (int32_t)(gh[0] & 0xffffu), vlen = (int32_t)gh[1];
             const int32_t nch = (int32_t)(gh[2] & 0xffu), ntog = (int32_t)((gh[2] >> 8) & 0xffu);
             const int32_t ncorr = (int32_t)((gh[2] >> 16) & 0xffu), nvar = (int32_t)(gh[2] >> 24);
             const uint32_t* cd = b + (gh[3] & 0xffffu);

@@ -18,11 +18,10 @@ namespace spt {
 // ---------------------------------------------------------------------------------------------------------------
 __global__ void decimate_kernel(const uint8_t* __restrict__ x, int64_t in_row_stride, int64_t in_beam_stride,
                                 uint16_t* __restrict__ y, int64_t out_row_stride, int64_t out_beam_stride,
-                                int32_t nchan, int64_t nsamp_k, int32_t k, uint32_t* __restrict__ maxval) {
+                                int32_t nchan, int64_t nsamp_k, int32_t k) {
     const int64_t quads = (nsamp_k + 3) >> 2;  // groups of 4 outputs per row
     const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    uint32_t mx = 0;
-    if (q < quads) {
+    if (q >= quads) return;
     const int32_t c = blockIdx.y, b = blockIdx.z;
     const uint8_t* src = x + (int64_t)b * in_beam_stride + (int64_t)c * in_row_stride;
     uint16_t* dst = y + (int64_t)b * out_beam_stride + (int64_t)c * out_row_stride;
@@ -44,31 +43,55 @@ __global__ void decimate_kernel(const uint8_t* __restrict__ x, int64_t in_row_st
         pk.x = o[0] | (o[1] << 16);
         pk.y = o[2] | (o[3] << 16);
         *reinterpret_cast<uint2*>(dst + j0) = pk;
-        mx = max(max(o[0], o[1]), max(o[2], o[3]));
     } else {  // ragged tail of the row
         for (int64_t j = j0; j < nsamp_k; ++j) {
             uint32_t s = 0;
             for (int m = 0; m < k; ++m) s += src[j * k + m];
             dst[j] = (uint16_t)s;
-            mx = max(mx, s);
         }
     }
-    }
-    // largest decimated sample of the launch: bounds how many channels a 16-bit lane of the dedispersion may sum
-    mx = __reduce_max_sync(0xffffffffu, mx);
-    if ((threadIdx.x & 31) == 0 && mx > 0) atomicMax(maxval, mx);
 }
 
-// Largest sample of a uint8 filterbank (the same bound for the ranges that read the raw input).
+// Largest and smallest sample of a uint8 filterbank -> maxval[0], maxval[1] (bounds for the ranges that read the raw input).
 __global__ void max_u8_kernel(const uint4* __restrict__ x, int64_t n16, uint32_t* __restrict__ maxval) {
-    uint32_t m = 0;
+    uint32_t m = 0, lo = 0xffffffffu;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (int64_t)gridDim.x * blockDim.x) {
         const uint4 v = __ldg(x + i);
         m = __vmaxu4(__vmaxu4(v.x, v.y), __vmaxu4(__vmaxu4(v.z, v.w), m));
+        lo = __vminu4(__vminu4(v.x, v.y), __vminu4(__vminu4(v.z, v.w), lo));
     }
     m = max(max(m & 0xffu, (m >> 8) & 0xffu), max((m >> 16) & 0xffu, m >> 24));
+    lo = min(min(lo & 0xffu, (lo >> 8) & 0xffu), min((lo >> 16) & 0xffu, lo >> 24));
     m = __reduce_max_sync(0xffffffffu, m);
-    if ((threadIdx.x & 31) == 0 && m > 0) atomicMax(maxval, m);
+    lo = __reduce_min_sync(0xffffffffu, lo);
+    if ((threadIdx.x & 31) == 0) {
+        if (m > 0) atomicMax(maxval, m);
+        atomicMin(maxval + 1, lo);
+    }
+}
+
+// The same for a decimated (uint16) series; its zero row padding, where there is any, only makes the bound looser.
+__global__ void max_u16_kernel(const uint4* __restrict__ x, int64_t n16, uint32_t* __restrict__ maxval) {
+    uint32_t m = 0, lo = 0xffffffffu;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (int64_t)gridDim.x * blockDim.x) {
+        const uint4 v = __ldg(x + i);
+        m = __vmaxu2(__vmaxu2(v.x, v.y), __vmaxu2(__vmaxu2(v.z, v.w), m));
+        lo = __vminu2(__vminu2(v.x, v.y), __vminu2(__vminu2(v.z, v.w), lo));
+    }
+    m = max(m & 0xffffu, m >> 16);
+    lo = min(lo & 0xffffu, lo >> 16);
+    m = __reduce_max_sync(0xffffffffu, m);
+    lo = __reduce_min_sync(0xffffffffu, lo);
+    if ((threadIdx.x & 31) == 0) {
+        if (m > 0) atomicMax(maxval, m);
+        atomicMin(maxval + 1, lo);
+    }
+}
+
+void launch_max_u16(const uint16_t* x, int64_t nelem, uint32_t* maxval, cudaStream_t st) {
+    const int64_t n16 = nelem / 8;            // rows are 16-element multiples
+    if (n16 <= 0) return;
+    max_u16_kernel<<<148 * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(x), n16, maxval);
 }
 
 void launch_max_u8(const uint8_t* x, int64_t nbytes, uint32_t* maxval, cudaStream_t st) {
@@ -79,12 +102,12 @@ void launch_max_u8(const uint8_t* x, int64_t nbytes, uint32_t* maxval, cudaStrea
 
 void launch_decimate(const uint8_t* x, int64_t in_row_stride, int64_t in_beam_stride, uint16_t* y,
                      int64_t out_row_stride, int64_t out_beam_stride, int32_t nchan, int32_t nbeam, int64_t nsamp_k,
-                     int32_t k, uint32_t* maxval, cudaStream_t st) {
+                     int32_t k, cudaStream_t st) {
     const int64_t quads = (nsamp_k + 3) >> 2;
     if (quads <= 0) return;
     dim3 grid((unsigned)((quads + 255) / 256), (unsigned)nchan, (unsigned)nbeam);
     decimate_kernel<<<grid, 256, 0, st>>>(x, in_row_stride, in_beam_stride, y, out_row_stride, out_beam_stride, nchan,
-                                          nsamp_k, k, maxval);
+                                          nsamp_k, k);
 }
 
 // ---------------------------------------------------------------------------------------------------------------
@@ -148,7 +171,7 @@ struct TiledArgs {
     const StageIndex* sidx;
     const RowDesc* rows;
     const uint32_t* blob;
-    const uint32_t* maxval;    // largest input sample of this launch (device scalar): bounds the 16-bit lanes
+    const uint32_t* maxval;    // {largest, smallest} input sample of this launch (device): bound the 16-bit lanes
     const int32_t* skew;       // [ntile_dm][DT] output skew of every trial of a DM tile
     int32_t skew_max;
     const int32_t* nout;       // range local
@@ -229,7 +252,7 @@ __device__ __forceinline__ void load_entry(uint32_t addr, uint32_t c1, uint32_t 
 // taken): a lane past the end of the variants works on the last four words and does not store.
 template <typename T>
 __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uint32_t task, uint32_t var_addr,
-                                            uint32_t raw_addr, int lane) {
+                                            uint32_t raw_addr, int lane, uint32_t floor2) {
     const uint4 gh = *reinterpret_cast<const uint4*>(tb + kBlobHdrWords + 4 * (task & 0xffu));   // 128-bit broadcast loads
     const int vlen = (int)gh.y;
     const uint32_t meta = gh.z;
@@ -241,7 +264,9 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
     u0 = active ? u0 : vlen - 4;
     const uint32_t rbase = raw_addr + (uint32_t)u0 * (uint32_t)sizeof(T);
     const uint32_t vbase = var_addr + (uint32_t)u0 * 4u;
-    uint32_t cur[4] = {0u, 0u, 0u, 0u};
+    // every channel of the group enters the base sum once: take the launch's smallest sample off each (both lanes)
+    const uint32_t bias = 0u - (gh.x >> 16) * floor2;
+    uint32_t cur[4] = {bias, bias, bias, bias};
     uint32_t dl[kMaxG][4];
 #pragma unroll
     for (int q2 = 0; q2 < kMaxG / 2; ++q2) {
@@ -371,7 +396,7 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
         have = hi > lo;
     }
     if (!__syncthreads_or(have)) return;    // no trial of the tile has an output here (ragged rows, skewed windows)
-    if (sizeof(T) > 1 && t0 < (int64_t)a.skew_max + 32) {
+    if (t0 < (int64_t)a.skew_max + 32) {
         // Windows that start before the row are not copied.  What the raw region holds there feeds only outputs with t < 0,
         // which are discarded, but their 16-bit lanes must not carry into the valid high lanes: make the first contents
         // zero (later stages find there the bounded samples of an earlier stage).
@@ -390,9 +415,16 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     bool first_flush = true;
     // F: widen the 16-bit lanes into the int32 DM transform.  A lane may sum floor(65535 / largest sample) channels: the
     // bound comes from the data of this launch (255 * decimation in the worst case, which is what the stages are cut for)
-    const int lane_cap = (int)(65535u / max(1u, __ldg(a.maxval)));
+    // What a lane sums is (sample - floor) with floor = the smallest sample of the launch, added back here: a lane may
+    // then sum floor(65535 / (largest - smallest sample)) channels.  Tiles whose windows start before the rows (skew) keep
+    // floor = 0: there the lanes of discarded outputs read zeros, which must not go negative next to a valid lane.
+    const uint32_t vmax = __ldg(a.maxval), vmin = __ldg(a.maxval + 1);
+    const uint32_t floor1 = (t0 < (int64_t)a.skew_max + 32 || vmin > vmax) ? 0u : vmin;
+    const uint32_t floor2 = floor1 * 0x00010001u;
+    const int lane_cap = (int)(65535u / max(1u, vmax - floor1));
     int since = 0;
     auto flush_lanes = [&]() {
+        const uint32_t back = (uint32_t)since * floor1;   // the floor of the channels summed since the last pass
 #pragma unroll
         for (int q = 0; q < TPW; ++q) {
             const int dl = warp * TPW + q;
@@ -401,7 +433,7 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
 #pragma unroll
             for (int j = 0; j < NJ; ++j) {
                 const int i = lane + 32 * j;
-                const int32_t lo = (int32_t)(acc[q][j] & 0xFFFFu), hi = (int32_t)(acc[q][j] >> 16);
+                const int32_t lo = (int32_t)((acc[q][j] & 0xFFFFu) + back), hi = (int32_t)((acc[q][j] >> 16) + back);
                 const bool ok_lo = i >= ok.x && i < ok.y, ok_hi = i + kH >= ok.x && i + kH < ok.y;
                 if (first_flush) {
                     if (ok_lo) row[i] = lo;
@@ -426,7 +458,7 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
 
         // ---- B: pre-sum every variant of every group ---------------------------------------------------------
         for (int tk = warp; tk < ntask; tk += NW)
-            presum_task<T>(tb, tb[kBlobHdrWords + 4 * ngrp + tk], var_addr, raw_addr, lane);
+            presum_task<T>(tb, tb[kBlobHdrWords + 4 * ngrp + tk], var_addr, raw_addr, lane, floor2);
         __syncthreads();  // variants complete; raw rows and the other blob buffer are free
         if (s + 1 < td.nstage) issue_stage(s + 1);
 

@@ -37,7 +37,7 @@ constexpr int kSmemDataBytes = kSmemBytes - kSmemCtrlBytes - 2 * kBlobBytes;  //
 
 // Per-stage blob, 32-bit words (copied to shared memory with one bulk copy):
 //   [0] ngrp  [1] (worst-case lane interval ends here) | channels of the stage << 8  [2] ntask  [3] word offset of the trial_off table
-//   [4 ..)        ngrp x { vbase, vlen, nent | ntog << 8 | ncorr << 16 | nvar << 24, cdesc_off | vdesc_off << 16 }
+//   [4 ..)        ngrp x { vbase | channels << 16, vlen, nent | ntog << 8 | ncorr << 16 | nvar << 24, cdesc_off | vdesc_off << 16 }
 //                 (offsets inside the blob)
 //   task table    ntask x { group | chunk << 8 }: warp task = kChunkU variant words of every variant of one group
 //   cdesc         per group, kMaxG entries of 2 words (the first nent are real, the rest repeat the first one without

@@ -330,7 +330,7 @@ int build_tiling(Plan& p) {
                         cdesc.push_back(c0 & ~kEntryAddBase);
                         cdesc.push_back(c1);
                     }
-                    hdr[kBlobHdrWords + 4 * k + 0] = (uint32_t)vbase;
+                    hdr[kBlobHdrWords + 4 * k + 0] = (uint32_t)vbase | ((uint32_t)g.nch << 16);
                     hdr[kBlobHdrWords + 4 * k + 1] = (uint32_t)g.vlen;
                     hdr[kBlobHdrWords + 4 * k + 2] = (uint32_t)g.nent | ((uint32_t)g.ntog << 8) | ((uint32_t)g.ncorrected << 16) | ((uint32_t)g.nvar << 24);
                     hdr[kBlobHdrWords + 4 * k + 3] = my_cdesc;                     // vdesc offset patched below

@@ -185,6 +185,20 @@ def test_square_wave_takes_the_exact_search_path(cuda, api, orc):
     assert int(row.max()) - int(row.min()) > (1 << 21)          # the premise: 1024 * max|x - m| >= 2^30
 
 
+@pytest.mark.parametrize("lo,hi", [(200, 203), (0, 3), (250, 255), (17, 17)])
+def test_narrow_value_ranges_bit_exact(cuda, api, orc, lo, hi):
+    """The packed lanes sum (sample - smallest sample of the launch) and may then go floor(65535 / (largest - smallest))
+    channels without widening: data confined to a narrow band of values far from zero, at both ends of the uint8 range,
+    constant data, decimated ranges, and tiles whose skewed windows start before the rows."""
+    w = Shape(500.0, -0.048828125, 4096, 6000, [(0.0, 0.2, 70, 1), (300.0, 0.5, 70, 2), (900.0, 1.0, 40, 4)], [1, 2, 8], 6.0)
+    rs = np.random.default_rng(lo)
+    fb = rs.integers(lo, hi + 1, size=(w.nchan, w.nsamp), dtype=np.uint8)
+    ref = oracle_path(orc, w, fb, search=False)
+    for options in ({}, {"skew": 0}):
+        plan, dmt, _ = run_gpu(cuda, api, w, fb[None], options=options, search=False)
+        check_dmt_against_oracle(plan, dmt, ref)
+
+
 # ---- config 2 at reduced length -----------------------------------------------------------------------------------
 def test_cfg2_reduced(cuda, api, orc, synth):
     w = synth.workload(2, nsamp=16384)
