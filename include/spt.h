@@ -202,6 +202,30 @@ int spt_search_host(spt_plan* plan, const uint8_t* h_fb, int32_t nbeam, float th
 int spt_stream_push(spt_plan* plan, const uint8_t* h_fb /*HOST*/, int32_t nbeam, float threshold);
 int spt_stream_pop(spt_plan* plan, int64_t* ncand, int32_t* overflowed);
 
+/* -------------------------------------------------------------------------------------------------------
+ * The step before the hot path for a continuous stream (blocks arrive time-major, the band is flipped to
+ * highest frequency first; every segment is read with an overlap so that each DM trial has its full
+ * sweep; reading F).
+ *
+ * spt_corner_turn: d_out[b][c'][t] = d_in[b][t][c], c' = flip ? nchan-1-c : c.   d_in DEVICE uint8 [nbeam][nsamp][nchan]
+ *   (time-major), d_out DEVICE uint8 [nbeam][nchan][nsamp] (what spt_dedisperse takes).  Needs no plan.  Enqueues.
+ *
+ * spt_segment_push: overlap-save.  The plan's nsamp is the length of a library-owned working buffer per channel row =
+ *   history + new samples.  A push drops the oldest nnew samples of every row, appends the corner-turned new block
+ *   (d_new DEVICE uint8 [nbeam][nnew][nchan], time-major; flip as above) and computes the DM transform of the buffer
+ *   into d_dmt exactly as spt_dedisperse would (same layout).  The buffer starts as zeros.  With
+ *   nsamp - nnew >= min_history every trial d gains nnew/decim new outputs per push: the LAST nnew/decim of its nout[d]
+ *   samples; the ones before them repeat outputs of earlier pushes.  nnew must be a multiple of `granule` (16, or the
+ *   largest decimation factor if larger) so that the shift keeps the decimation phase and the row alignment.
+ *   SPT_ERR_SHAPE when the history is shorter than min_history.  Enqueues on cuda_stream.
+ * spt_segment_info: min_history = the longest sweep of the plan in raw samples, rounded up to the granule.
+ * ----------------------------------------------------------------------------------------------------- */
+int spt_corner_turn(const uint8_t* d_in /*DEVICE*/, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip,
+                    uint8_t* d_out /*DEVICE*/, void* cuda_stream);
+int spt_segment_info(const spt_plan* plan, int64_t* min_history, int64_t* granule);
+int spt_segment_push(spt_plan* plan, const uint8_t* d_new /*DEVICE*/, int32_t nbeam, int64_t nnew, int32_t flip,
+                     int32_t* d_dmt /*DEVICE*/, void* cuda_stream);
+
 /* With option "profile" = 1: device time (ms) of each kernel launched by the LAST spt_dedisperse and the LAST
  * spt_single_pulse_search, in launch order; kinds: 1 = decimate, 2 = dedisperse, 3 = single-pulse search; `range` is the
  * DM range the launch served (-1 for the search).  Synchronises.  Arrays (HOST) hold `cap` entries; n = entries written. */

@@ -203,6 +203,26 @@ def search_plane(dmt: np.ndarray, rowoff: np.ndarray, nout_: np.ndarray, widths:
     return PlaneSearch(s, q, cnt, candoff, ct, cw, cs)
 
 
+# ---- F. corner turn and overlap-save (PAPER.md:41, 47) -- plain definitions ---------------------------
+def corner_turn(x_time_major: np.ndarray, flip: bool = False) -> np.ndarray:
+    """[nsamp][nchan] (time-major block) -> [nchan][nsamp]; flip = the block has the lowest frequency first."""
+    y = np.ascontiguousarray(np.asarray(x_time_major, dtype=np.uint8).T)
+    return np.ascontiguousarray(y[::-1]) if flip else y
+
+
+def overlap_save_buffers(blocks_time_major: Sequence[np.ndarray], nsamp: int, flip: bool = False) -> List[np.ndarray]:
+    """The working buffer ([nchan][nsamp]) after each push of a stream that starts on a history of zeros: the last
+    nsamp samples of zeros ++ block 0 ++ block 1 ++ ... (every trial of a dedispersion of it has its full sweep when
+    nsamp - len(block) >= the longest sweep)."""
+    nchan = blocks_time_major[0].shape[1]
+    stream = np.zeros((nchan, nsamp), dtype=np.uint8)
+    out = []
+    for blk in blocks_time_major:
+        stream = np.concatenate([stream, corner_turn(blk, flip)], axis=1)
+        out.append(np.ascontiguousarray(stream[:, -nsamp:]))
+    return out
+
+
 # ---- E. peak filtering (PAPER.md:96) --------------------------------------------------------------------
 def peak_filter(beam: np.ndarray, trial: np.ndarray, t: np.ndarray, snr: np.ndarray, range_of_trial: np.ndarray,
                 windows: Sequence[int] = (3, 11)) -> np.ndarray:

@@ -57,6 +57,9 @@ SYMBOLS = {
     "spt_peak_filter": (ctypes.c_int, [_vp, _P(_i32), _i32, _vp]),
     "spt_peaks_count": (ctypes.c_int, [_vp, _P(_i64)]),
     "spt_peaks_read": (ctypes.c_int, [_vp, _vp, _i64, _P(_i64)]),
+    "spt_corner_turn": (ctypes.c_int, [_vp, _i32, _i64, _i32, _i32, _vp, _vp]),
+    "spt_segment_info": (ctypes.c_int, [_vp, _P(_i64), _P(_i64)]),
+    "spt_segment_push": (ctypes.c_int, [_vp, _vp, _i32, _i64, _i32, _vp, _vp]),
     "spt_stream_push": (ctypes.c_int, [_vp, _vp, _i32, _f32]),
     "spt_stream_pop": (ctypes.c_int, [_vp, _P(_i64), _P(_i32)]),
     "spt_plan_kernel_times": (ctypes.c_int, [_vp, _i32, _vp, _vp, _vp, _P(_i32)]),
@@ -257,6 +260,24 @@ class Plan:
         _check(lib().spt_peaks_read(self._h, out.ctypes.data, int(n.value), ctypes.byref(k)), "spt_peaks_read")
         return out[: int(k.value)]
 
+    def segment_info(self):
+        """(min_history, granule) in raw samples for spt_segment_push."""
+        h, g = ctypes.c_int64(), ctypes.c_int64()
+        _check(lib().spt_segment_info(self._h, ctypes.byref(h), ctypes.byref(g)), "spt_segment_info")
+        return int(h.value), int(g.value)
+
+    def segment_push(self, d_new, flip: bool = False, d_dmt=None, stream=None):
+        """Overlap-save push of a time-major CUDA uint8 block [nbeam][nnew][nchan]; returns the DM transform tensor."""
+        import torch
+        nbeam, nnew, nchan = d_new.shape
+        if nchan != self.nchan or d_new.dtype != torch.uint8:
+            raise ValueError("block must be uint8 [nbeam][nnew][nchan]")
+        if d_dmt is None:
+            d_dmt = torch.empty((nbeam, self.dmt_elems_per_beam), dtype=torch.int32, device=d_new.device)
+        _check(lib().spt_segment_push(self._h, _dev_ptr(d_new), nbeam, nnew, int(bool(flip)), _dev_ptr(d_dmt),
+                                      _stream_ptr(stream)), "spt_segment_push")
+        return d_dmt
+
     def stream_push(self, h_fb, threshold: float):
         """Enqueue one batch (HOST uint8 [nbeam][nchan][nsamp], pinned) into the two-deep pipeline; returns at once."""
         ptr, nbeam = _host_ptr_and_beams(h_fb, self.nchan, self.nsamp)
@@ -296,6 +317,16 @@ def _host_ptr_and_beams(h_fb, nchan, nsamp):
         shape = (1,) + tuple(shape)
     assert tuple(shape[1:]) == (nchan, nsamp)
     return ptr, shape[0]
+
+
+def corner_turn(d_in, flip: bool = False, stream=None):
+    """Time-major CUDA uint8 [nbeam][nsamp][nchan] -> channel-major [nbeam][nchan][nsamp] (optionally band-flipped)."""
+    import torch
+    nbeam, nsamp, nchan = d_in.shape
+    out = torch.empty((nbeam, nchan, nsamp), dtype=torch.uint8, device=d_in.device)
+    _check(lib().spt_corner_turn(_dev_ptr(d_in), nbeam, nsamp, nchan, int(bool(flip)), _dev_ptr(out), _stream_ptr(stream)),
+           "spt_corner_turn")
+    return out
 
 
 def probe(kind: int, reps: int = 5) -> Tuple[float, float]:

@@ -42,6 +42,10 @@ struct DeviceState {
     uint32_t* maxval = nullptr;     // [nranges][2] largest and smallest sample of the series each range read last
     int32_t* range_lo = nullptr;    // [ntrials] first / last trial of the trial's DM range (peak filter)
     int32_t* range_hi = nullptr;
+    // continuous stream (lazily allocated): two working buffers [max_beams][nchan][nsamp], the current one holds the last
+    // nsamp samples of every channel row
+    uint8_t* work[2] = {nullptr, nullptr};
+    int work_cur = 0;
     // peak filter (lazily allocated): lookup plane laid out like the DM transform, live flags, peak list
     uint32_t* plane = nullptr;
     uint8_t* alive[2] = {nullptr, nullptr};
@@ -122,6 +126,7 @@ static void free_device(Plan* p) {
         cudaFree(r.series);
     }
     cudaFree(d->maxval); cudaFree(d->nout); cudaFree(d->offset); cudaFree(d->range_lo); cudaFree(d->range_hi);
+    cudaFree(d->work[0]); cudaFree(d->work[1]);
     cudaFree(d->plane); cudaFree(d->alive[0]); cudaFree(d->alive[1]); cudaFree(d->peaks); cudaFree(d->peaks_count);
     for (auto& b : d->bufs) { cudaFree(b.sum); cudaFree(b.sumsq); cudaFree(b.cand); cudaFree(b.count); }
     for (auto& sl : d->slot) {
@@ -808,6 +813,67 @@ int spt_peaks_read(spt_plan* plan, spt_candidate* host_out, int64_t cap, int64_t
     if (n > 0) SPT_CUDA(cudaMemcpy(host_out, plan->p.dev->peaks, (size_t)n * sizeof(spt_candidate), cudaMemcpyDeviceToHost));
     if (nwritten) *nwritten = n;
     return SPT_OK;
+}
+
+int spt_corner_turn(const uint8_t* d_in, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip, uint8_t* d_out,
+                    void* cuda_stream) {
+    if (!d_in || !d_out || nbeam < 1 || nsamp < 1 || nchan < 1 || (flip != 0 && flip != 1)) return SPT_ERR_INVALID;
+    launch_corner_turn(d_in, nbeam, nsamp, nchan, flip, d_out, nsamp, (int64_t)nchan * nsamp, 0, (cudaStream_t)cuda_stream);
+    SPT_CUDA(cudaGetLastError());
+    return SPT_OK;
+}
+
+int spt_segment_info(const spt_plan* plan, int64_t* min_history, int64_t* granule) {
+    if (!plan) return SPT_ERR_INVALID;
+    const Plan& p = plan->p;
+    int64_t h = 0, g = 16;
+    for (const RangePlan& rp : p.ranges) {
+        int32_t dmax = 0;
+        for (int32_t i = 0; i < rp.ndm; ++i) dmax = std::max(dmax, rp.delay[(size_t)i * p.nchan + p.nchan - 1]);
+        h = std::max<int64_t>(h, (int64_t)dmax * rp.decim);
+        g = std::max<int64_t>(g, rp.decim);
+    }
+    if (min_history) *min_history = (h + g - 1) / g * g;
+    if (granule) *granule = g;
+    return SPT_OK;
+}
+
+int spt_segment_push(spt_plan* plan, const uint8_t* d_new, int32_t nbeam, int64_t nnew, int32_t flip, int32_t* d_dmt,
+                     void* cuda_stream) {
+    if (!plan || !d_new || !d_dmt || nbeam < 1 || nbeam > plan->p.max_beams || (flip != 0 && flip != 1)) return SPT_ERR_INVALID;
+    if ((reinterpret_cast<uintptr_t>(d_dmt) & 127) != 0) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    int64_t hmin = 0, gran = 16;
+    spt_segment_info(plan, &hmin, &gran);
+    // the shift must keep the phase of every decimation and the 16-byte alignment of the rows
+    if (nnew < 1 || nnew > p.nsamp || nnew % gran != 0 || p.nsamp % 16 != 0) return SPT_ERR_INVALID;
+    if (p.nsamp - nnew < hmin) return SPT_ERR_SHAPE;              // not every trial would have its full sweep
+    int rc;
+    try {
+        rc = ensure_device(&p);
+    } catch (const std::bad_alloc&) {
+        rc = SPT_ERR_NOMEM;
+    }
+    if (rc != SPT_OK) return rc;
+    DeviceState* d = p.dev;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t bytes = (size_t)p.max_beams * p.nchan * p.nsamp;
+    if (!d->work[0]) {
+        for (int i = 0; i < 2; ++i) {
+            SPT_CUDA(cudaMalloc((void**)&d->work[i], bytes));
+            SPT_CUDA(cudaMemset(d->work[i], 0, bytes));           // the stream starts on a history of zeros
+        }
+        d->work_cur = 0;
+    }
+    const uint8_t* prev = d->work[d->work_cur];
+    uint8_t* cur = d->work[d->work_cur ^ 1];
+    const int64_t keep = p.nsamp - nnew;
+    launch_keep_history(prev, cur, p.nsamp, nnew, keep, (int64_t)nbeam * p.nchan, st);
+    launch_corner_turn(d_new, nbeam, nnew, p.nchan, flip, cur, p.nsamp, (int64_t)p.nchan * p.nsamp, keep, st);
+    p.launches += keep > 0 ? 2 : 1;
+    SPT_CUDA(cudaGetLastError());
+    d->work_cur ^= 1;
+    return do_dedisperse(&p, cur, nbeam, d_dmt, st);
 }
 
 int spt_plan_kernel_times(spt_plan* plan, int32_t cap, int32_t* kind, int32_t* range, double* ms, int32_t* n) {

@@ -56,6 +56,11 @@ void launch_peaks_stencil(const PeakArgs& a, int32_t window, const uint8_t* aliv
 void launch_peaks_compact(const PeakArgs& a, const uint8_t* alive, spt_candidate* out, unsigned long long* out_count,
                           long long out_capacity, cudaStream_t st);
 
+void launch_corner_turn(const uint8_t* in, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip, uint8_t* out,
+                        int64_t out_row_stride, int64_t out_beam_stride, int64_t out_t0, cudaStream_t st);
+void launch_keep_history(const uint8_t* src, uint8_t* dst, int64_t row_bytes, int64_t shift_bytes, int64_t keep_bytes,
+                         int64_t nrows, cudaStream_t st);
+
 int run_probe(int kind, int reps, double* warp_instr_per_s, double* elapsed_ms);
 
 }  // namespace spt

@@ -1,0 +1,83 @@
+// stream.cu -- the step before the hot path for a continuous stream (reading F):
+//   corner turn   telescope blocks are time-major ([t][chan], SIGPROC order) and may have the lowest frequency first;
+//                 the search wants channel-major rows with the highest frequency first ("frequency flip")
+//   overlap-save  aamulti reads each segment with an overlap so that every DM trial has its full sweep:
+//                 the working buffer keeps the last `history` samples of every channel row and appends the new block.
+// Both are pure data movement, HBM bound.
+#include <cuda_runtime.h>
+
+#include "kernels.h"
+
+namespace spt {
+
+// out[b][c'][t0 + t] = in[b][t][c],  c' = flip ? nchan-1-c : c.  Tile: 64 samples x 128 channels through shared memory;
+// loads are 128-byte rows of channels, stores are 64-byte runs of samples.
+__global__ void __launch_bounds__(256) corner_turn_kernel(const uint8_t* __restrict__ in, int64_t nsamp, int32_t nchan,
+                                                          int32_t flip, uint8_t* __restrict__ out, int64_t out_row_stride,
+                                                          int64_t out_beam_stride, int64_t out_t0) {
+    __shared__ uint8_t tile[128][64 + 4];                 // [channel][sample], padded rows
+    const int b = blockIdx.z;
+    const int64_t t0 = (int64_t)blockIdx.x * 64;
+    const int c0 = blockIdx.y * 128;
+    const uint8_t* src = in + (int64_t)b * nsamp * nchan;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;          // 32 x 8
+    // load: one warp reads 128 consecutive channels of one sample (4 per lane)
+    for (int i = ty; i < 64; i += 8) {
+        const int64_t t = t0 + i;
+        const int c = c0 + 4 * tx;
+        uint32_t v = 0;
+        if (t < nsamp) {
+            const uint8_t* p = src + t * nchan + c;
+            if (c + 4 <= nchan && ((reinterpret_cast<uintptr_t>(p) & 3) == 0)) v = *reinterpret_cast<const uint32_t*>(p);
+            else
+                for (int k = 0; k < 4; ++k)
+                    if (c + k < nchan) v |= (uint32_t)p[k] << (8 * k);
+        }
+        tile[4 * tx + 0][i] = (uint8_t)v;
+        tile[4 * tx + 1][i] = (uint8_t)(v >> 8);
+        tile[4 * tx + 2][i] = (uint8_t)(v >> 16);
+        tile[4 * tx + 3][i] = (uint8_t)(v >> 24);
+    }
+    __syncthreads();
+    // store: 16 lanes write the 64 samples of one channel (4 per lane), two channels per warp pass
+    const int half = tx >> 4, l = tx & 15;
+    for (int i = ty * 2 + half; i < 128; i += 16) {
+        const int c = c0 + i;
+        if (c >= nchan) continue;
+        const int cc = flip ? nchan - 1 - c : c;
+        const int64_t t = t0 + 4 * l;
+        uint8_t* dst = out + (int64_t)b * out_beam_stride + (int64_t)cc * out_row_stride + out_t0 + t;
+        const uint32_t v = *reinterpret_cast<const uint32_t*>(&tile[i][4 * l]);
+        if (t + 4 <= nsamp && ((reinterpret_cast<uintptr_t>(dst) & 3) == 0)) *reinterpret_cast<uint32_t*>(dst) = v;
+        else
+            for (int k = 0; k < 4; ++k)
+                if (t + k < nsamp) dst[k] = (uint8_t)(v >> (8 * k));
+    }
+}
+
+void launch_corner_turn(const uint8_t* in, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip, uint8_t* out,
+                        int64_t out_row_stride, int64_t out_beam_stride, int64_t out_t0, cudaStream_t st) {
+    if (nbeam <= 0 || nsamp <= 0 || nchan <= 0) return;
+    dim3 grid((unsigned)((nsamp + 63) / 64), (unsigned)((nchan + 127) / 128), (unsigned)nbeam);
+    corner_turn_kernel<<<grid, 256, 0, st>>>(in, nsamp, nchan, flip, out, out_row_stride, out_beam_stride, out_t0);
+}
+
+// dst[row][0 .. nkeep) = src[row][shift .. shift + nkeep): the history of every channel row moves to the front of the
+// other working buffer (all counts are multiples of 16 bytes).
+__global__ void keep_history_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst, int64_t row16, int64_t shift16,
+                                    int64_t keep16, int64_t nrows) {
+    const int64_t n = keep16 * nrows;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t r = i / keep16, k = i - r * keep16;
+        dst[r * row16 + k] = __ldg(src + r * row16 + shift16 + k);
+    }
+}
+
+void launch_keep_history(const uint8_t* src, uint8_t* dst, int64_t row_bytes, int64_t shift_bytes, int64_t keep_bytes,
+                         int64_t nrows, cudaStream_t st) {
+    if (keep_bytes <= 0 || nrows <= 0) return;
+    keep_history_kernel<<<148 * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(src), reinterpret_cast<uint4*>(dst),
+                                                  row_bytes / 16, shift_bytes / 16, keep_bytes / 16, nrows);
+}
+
+}  // namespace spt

@@ -1,0 +1,54 @@
+"""NEXT-2 (reading F): corner turn of time-major blocks and overlap-save segments.  The DM transform after
+every push must be, bit for bit, the oracle's batch dedispersion of the last nsamp samples of the stream, so that the
+last nnew/decim outputs of every trial continue the previous push's."""
+import numpy as np
+import pytest
+
+from helpers import check_dmt_against_oracle, make_plan
+from test_gpu_parity import Shape, oracle_path
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("shape,flip", [((1, 1000, 71), False), ((2, 513, 256), True), ((1, 64, 4096), True), ((3, 7, 5), False)])
+def test_corner_turn(cuda, api, orc, shape, flip):
+    rs = np.random.default_rng(sum(shape))
+    x = rs.integers(0, 256, size=shape, dtype=np.uint8)
+    got = api.corner_turn(cuda.from_numpy(x).cuda(), flip).cpu().numpy()
+    for b in range(shape[0]):
+        assert np.array_equal(got[b], orc.corner_turn(x[b], flip))
+
+
+def test_overlap_save_segments(cuda, api, orc):
+    nchan, nnew = 256, 2048
+    w = Shape(500.0, -200.0 / nchan, nchan, 0, [(0.0, 0.2, 70, 1), (10.0, 0.5, 40, 2), (30.0, 1.0, 33, 4)], [1, 2, 4], 6.0, nbeam=2)
+    probe = api.Plan(w.fch1, w.foff, nchan, w.tsamp, 1 << 16, w.ranges, w.widths)
+    hmin, gran = probe.segment_info()
+    assert gran == 16 and hmin % 16 == 0 and hmin > 0
+    w.nsamp = hmin + nnew                                          # exactly the shortest legal history
+    rs = np.random.default_rng(9)
+    blocks = [rs.integers(0, 256, size=(2, nnew, nchan), dtype=np.uint8) for _ in range(4)]
+    plan = make_plan(api, w, nbeam=2)
+    refs = [orc.overlap_save_buffers([blk[b] for blk in blocks], w.nsamp, flip=True) for b in range(2)]
+    _, _, dec, nout, off = plan.trial_table()
+    prev = None
+    for i, blk in enumerate(blocks):
+        d_dmt = plan.segment_push(cuda.from_numpy(blk).cuda(), flip=True)
+        dmt = d_dmt.cpu().numpy()
+        for b in range(2):
+            ref = oracle_path(orc, w, refs[b][i], search=False)
+            check_dmt_against_oracle(plan, dmt, ref, beam=b)
+        if prev is not None:                                       # every row slid by nnew/decim: old outputs repeat, new ones follow
+            for d in (0, 69, 70, 109, 110, 142):
+                k, n = int(dec[d]), int(nout[d])
+                assert n >= nnew // k
+                assert np.array_equal(dmt[0][off[d]: off[d] + n - nnew // k], prev[0][off[d] + nnew // k: off[d] + n])
+        prev = dmt
+    # a history shorter than the longest sweep, or a shift that breaks the decimation phase, is refused
+    short = make_plan(api, w, nbeam=2, nsamp=hmin + nnew - 16)
+    with pytest.raises(api.SptError) as e:
+        short.segment_push(cuda.from_numpy(blocks[0]).cuda())
+    assert e.value.code == api.SPT_ERR_SHAPE
+    with pytest.raises(api.SptError) as e:
+        plan.segment_push(cuda.from_numpy(blocks[0][:, : nnew - 8]).cuda())
+    assert e.value.code == api.SPT_ERR_INVALID

@@ -1,0 +1,42 @@
+"""Pins of the oracle's stream definitions (reading F): worked examples written out by hand and the
+overlap-save identity -- the buffer after push i, dedispersed, continues the buffer after push i-1."""
+import numpy as np
+
+
+def test_corner_turn_worked_example(orc):
+    x = np.array([[1, 2, 3], [4, 5, 6]], dtype=np.uint8)                 # 2 samples x 3 channels, time-major
+    assert orc.corner_turn(x).tolist() == [[1, 4], [2, 5], [3, 6]]         # channel rows
+    assert orc.corner_turn(x, flip=True).tolist() == [[3, 6], [2, 5], [1, 4]]   # last channel (highest frequency) first
+
+
+def test_overlap_save_buffers_worked_example(orc):
+    b0 = np.array([[1, 10], [2, 20]], dtype=np.uint8)                    # 2 new samples x 2 channels per push
+    b1 = np.array([[3, 30], [4, 40]], dtype=np.uint8)
+    bufs = orc.overlap_save_buffers([b0, b1], nsamp=3)
+    assert bufs[0].tolist() == [[0, 1, 2], [0, 10, 20]]                   # one sample of zero history, then block 0
+    assert bufs[1].tolist() == [[2, 3, 4], [20, 30, 40]]                  # the last sample of block 0 is the history
+
+
+def test_overlap_save_continues_the_dm_transform(orc):
+    """With history >= the longest sweep, the DM transform of the buffer after push i, shifted by the new samples, is
+    the DM transform of one long observation: nothing is lost or doubled at segment borders."""
+    rs = np.random.default_rng(1)
+    nchan, nnew, npush = 16, 64, 4
+    fch1, foff, tsamp = 500.0, -12.5, 1.31072e-3
+    dly = orc.delay_table(fch1, foff, nchan, tsamp, 0.0, 1.0, 12, 1)
+    hist = int(dly.max())
+    hist += (-hist) % 16
+    nsamp = hist + nnew
+    blocks = [rs.integers(0, 256, size=(nnew, nchan), dtype=np.uint8) for _ in range(npush)]
+    bufs = orc.overlap_save_buffers(blocks, nsamp)
+    whole = np.concatenate([np.zeros((nchan, hist), dtype=np.uint8)] + [orc.corner_turn(b) for b in blocks], axis=1)
+    no_w = orc.nout(dly, whole.shape[1], 1)
+    full, off_w = orc.dedisperse(whole, dly, no_w)
+    no = orc.nout(dly, nsamp, 1)
+    for i, buf in enumerate(bufs):
+        out, off = orc.dedisperse(buf, dly, no)
+        for d in range(dly.shape[0]):
+            row = out[off[d]: off[d + 1]]
+            a = i * nnew                                                  # buffer start inside the long observation
+            assert np.array_equal(row, full[off_w[d] + a: off_w[d] + a + no[d]])
+            assert no[d] >= nnew                                          # every push yields nnew new outputs per trial
