@@ -6,6 +6,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstring>
+#include <cstdlib>
 #include <map>
 #include <utility>
 
@@ -276,8 +277,6 @@ int build_tiling(Plan& p) {
             td.ntrial = std::min(DT, rp.ndm - d0);
             td.stage0 = (int32_t)rp.sidx.size();
             std::vector<PendingGroup> open;
-            int64_t open_v = 0, open_r = 0;
-            int since_flush = 0;
             auto blob_words_of = [&](const std::vector<PendingGroup>& gs, const PendingGroup* extra) {
                 int64_t w = kBlobHdrWords + 4;
                 auto one = [&](const PendingGroup& g) {
@@ -288,13 +287,7 @@ int build_tiling(Plan& p) {
                 return w;
             };
             auto close_stage = [&](bool flush) {
-                if (open.empty()) {
-                    if (flush && (int32_t)rp.sidx.size() > td.stage0) {
-                        rp.blob[rp.sidx.back().blob_word0 + 1] |= 1u;
-                        since_flush = 0;
-                    }
-                    return;
-                }
+                if (open.empty()) return;
                 StageIndex si;
                 si.blob_word0 = (uint32_t)rp.blob.size();
                 si.row0 = (uint32_t)rp.rows.size();
@@ -379,25 +372,43 @@ int build_tiling(Plan& p) {
                 si.blob_words = (uint32_t)(rp.blob.size() - si.blob_word0);
                 si.nrows = (uint32_t)(rp.rows.size() - si.row0);
                 rp.sidx.push_back(si);
-                if (flush) since_flush = 0;
                 open.clear();
-                open_v = open_r = 0;
             };
+            // all groups of the tile first, then the cut into stages
+            std::vector<PendingGroup> all;
             for (int32_t c = 0; c < p.nchan;) {
                 PendingGroup g;
-                if (!make_group(p, rp, d0, td.ntrial, c, G, es, &rp.skew[(size_t)(d0 / DT) * DT], g)) return SPT_ERR_UNSUPPORTED;
+                if (!make_group(p, rp, d0, td.ntrial, c, std::min(G, lane_channels), es, &rp.skew[(size_t)(d0 / DT) * DT], g))
+                    return SPT_ERR_UNSUPPORTED;
                 c += g.nch;
                 if (g.vwords > rp.vcap_words || g.raw_bytes > rcap_bytes || blob_words_of({}, &g) * 4 > kBlobBytes)
                     return SPT_ERR_UNSUPPORTED;  // one group must fit a stage
-                if (since_flush + g.nch > lane_channels) close_stage(true);
-                else if (open_v + g.vwords > rp.vcap_words || open_r + g.raw_bytes > rcap_bytes ||
-                         (int)open.size() >= kMaxStageGroups || blob_words_of(open, &g) * 4 > kBlobBytes)
-                    close_stage(false);
-                open_v += g.vwords; open_r += g.raw_bytes;
-                since_flush += g.nch;
-                open.push_back(std::move(g));
+                all.push_back(std::move(g));
             }
-            close_stage(true);
+            // A stage costs ceil(tasks / warps) pre-sum rounds plus a fixed overhead (barriers, bulk-copy issue, tables) of
+            // about one round; its groups must fit shared memory and the table blob, and its channels one worst-case lane
+            // interval (the kernel widens the lanes between stages, never inside one).  Take, from every starting group,
+            // the feasible prefix with the lowest cost per channel: 15 tasks in two rounds beat 18 tasks in three.
+            constexpr int kWarps = kThreads / 32;
+            constexpr double kStageOverheadRounds = 1.0;
+            for (size_t i0 = 0; i0 < all.size();) {
+                int64_t v = 0, r = 0, words = kBlobHdrWords + 4;
+                int nch = 0, tasks = 0;
+                size_t best_n = 1;
+                double best_cost = 1e300;
+                for (size_t n = 1; i0 + n <= all.size() && n <= (size_t)kMaxStageGroups; ++n) {
+                    const PendingGroup& g = all[i0 + n - 1];
+                    v += g.vwords; r += g.raw_bytes; nch += g.nch;
+                    words += 4 + (g.vlen + kChunkU - 1) / kChunkU + 2 * kMaxG + kChainWords + 2 * g.ncorrected + 3 + DT / 2;
+                    tasks += (g.vlen + kChunkU - 1) / kChunkU;
+                    if (n > 1 && (v > rp.vcap_words || r > rcap_bytes || words * 4 > kBlobBytes || nch > lane_channels)) break;
+                    const double cost = ((tasks + kWarps - 1) / kWarps + kStageOverheadRounds) / nch;
+                    if (cost <= best_cost) { best_cost = cost; best_n = n; }
+                }
+                for (size_t n = 0; n < best_n; ++n) open.push_back(std::move(all[i0 + n]));
+                close_stage(false);
+                i0 += best_n;
+            }
             td.nstage = (int32_t)rp.sidx.size() - td.stage0;
             rp.tiles.push_back(td);
         }
