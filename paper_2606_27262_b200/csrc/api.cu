@@ -73,6 +73,9 @@ struct DeviceState {
     } slot[2];
     int push_next = 0, pop_next = 0;
     cudaStream_t copy_stream = nullptr;
+    // side streams for the DM ranges after the first (their grids fill the tail of the previous range's grid)
+    cudaStream_t side[2] = {nullptr, nullptr};
+    cudaEvent_t fork = nullptr, join[2] = {nullptr, nullptr};
     cudaEvent_t wait_event = nullptr;   // when set, read-out calls wait for this event instead of the whole stream
     uint8_t* fb_pad = nullptr;      // aligned copy of an input whose rows are not 16-byte multiples
     int64_t fb_pad_stride = 0;
@@ -138,6 +141,8 @@ static void free_device(Plan* p) {
     cudaFree(d->fb_pad); cudaFree(d->h_fb); cudaFree(d->h_dmt);
     if (d->own_stream) cudaStreamDestroy(d->own_stream);
     if (d->copy_stream) cudaStreamDestroy(d->copy_stream);
+    for (int i = 0; i < 2; ++i) { if (d->side[i]) cudaStreamDestroy(d->side[i]); if (d->join[i]) cudaEventDestroy(d->join[i]); }
+    if (d->fork) cudaEventDestroy(d->fork);
     timed_clear(d, 0); timed_clear(d, 1);
     for (cudaEvent_t e : d->event_pool) cudaEventDestroy(e);
     delete d;
@@ -250,10 +255,27 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
         launch_max_u16(d->r[i].series, (int64_t)nbeam * p->nchan * rp.stride_k, d->maxval + 2 * i, st);
         p->launches += 2;
     }
-    // a3: DM transform, range by range
+    // a3: DM transform, range by range.  Unless launches are being timed one by one, the ranges after the first go to
+    // side streams: they are independent, and a later grid then fills the last, partly empty wave of the grid before it.
+    const bool overlap = !p->opt_profile && p->ranges.size() > 1;
+    if (overlap) {
+        if (!d->fork) {
+            SPT_CUDA(cudaEventCreateWithFlags(&d->fork, cudaEventDisableTiming));
+            for (int i = 0; i < 2; ++i) {
+                SPT_CUDA(cudaStreamCreateWithFlags(&d->side[i], cudaStreamNonBlocking));
+                SPT_CUDA(cudaEventCreateWithFlags(&d->join[i], cudaEventDisableTiming));
+            }
+        }
+        SPT_CUDA(cudaEventRecord(d->fork, st));                  // after the decimation and the min/max passes
+        for (int i = 0; i < 2; ++i) SPT_CUDA(cudaStreamWaitEvent(d->side[i], d->fork, 0));
+    }
+    cudaStream_t const caller = st;
+    bool used_side[2] = {false, false};
     for (size_t i = 0; i < p->ranges.size(); ++i) {
         const RangePlan& rp = p->ranges[i];
         if (rp.max_nout <= 0) continue;
+        if (overlap && i > 0) { st = d->side[(i - 1) & 1]; used_side[(i - 1) & 1] = true; }
+        else st = caller;
         const RangeDev& rd = d->r[i];
         const bool u16 = rp.decim > 1;
         const void* src = u16 ? (const void*)rd.series : (const void*)in;
@@ -274,6 +296,12 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
         }
         p->launches++;
     }
+    st = caller;
+    for (int i = 0; i < 2; ++i)
+        if (used_side[i]) {                                      // the caller's stream continues when every range is done
+            SPT_CUDA(cudaEventRecord(d->join[i], d->side[i]));
+            SPT_CUDA(cudaStreamWaitEvent(st, d->join[i], 0));
+        }
     SPT_CUDA(cudaGetLastError());
     d->last_stream = st;
     d->nbeam_dedisp = nbeam;
