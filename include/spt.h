@@ -218,11 +218,22 @@ int spt_stream_pop(spt_plan* plan, int64_t* ncand, int32_t* overflowed);
  *   samples; the ones before them repeat outputs of earlier pushes.  nnew must be a multiple of `granule` (16, or the
  *   largest decimation factor if larger) so that the shift keeps the decimation phase and the row alignment.
  *   SPT_ERR_SHAPE when the history is shorter than min_history.  Enqueues on cuda_stream.
- * spt_segment_info: min_history = the longest sweep of the plan in raw samples, rounded up to the granule.
+ * spt_segment_info: min_history = the longest sweep of the plan in raw samples, rounded up to the granule;
+ *   min_history_search = the same plus (widest boxcar - 1) samples of the coarsest rate (what spt_segment_search needs).
+ *
+ * spt_segment_search: the single-pulse search of one pushed segment (readings C1-C5, D1 applied to a window).  For every
+ *   trial d (decimation k, row length n = nout[d]) the window is the last L = nnew/k + wmax - 1 samples of the row; the
+ *   statistics (N = L, Sx, Sxx) and S/N are those of the window; reported are the start positions in its first nnew/k
+ *   samples -- exactly those for which every boxcar width fits in the data seen so far and that no earlier segment has
+ *   reported -- so that consecutive segments report every start position of the stream exactly once.  Candidate t is
+ *   the index inside the row (add the row's stream offset for an absolute time).  d_dmt: what spt_segment_push wrote.
+ *   Needs nsamp - nnew >= min_history_search (else SPT_ERR_SHAPE).  Read-out calls as after spt_single_pulse_search.
  * ----------------------------------------------------------------------------------------------------- */
 int spt_corner_turn(const uint8_t* d_in /*DEVICE*/, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip,
                     uint8_t* d_out /*DEVICE*/, void* cuda_stream);
-int spt_segment_info(const spt_plan* plan, int64_t* min_history, int64_t* granule);
+int spt_segment_info(const spt_plan* plan, int64_t* min_history, int64_t* min_history_search, int64_t* granule);
+int spt_segment_search(spt_plan* plan, const int32_t* d_dmt /*DEVICE*/, int32_t nbeam, int64_t nnew, float threshold,
+                       void* cuda_stream);
 int spt_segment_push(spt_plan* plan, const uint8_t* d_new /*DEVICE*/, int32_t nbeam, int64_t nnew, int32_t flip,
                      int32_t* d_dmt /*DEVICE*/, void* cuda_stream);
 

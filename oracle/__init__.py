@@ -223,6 +223,20 @@ def overlap_save_buffers(blocks_time_major: Sequence[np.ndarray], nsamp: int, fl
     return out
 
 
+def search_segment(row: np.ndarray, widths: Sequence[int], threshold: float, nnew_k: int):
+    """Search of one pushed segment of one trial (reading F): the window is the last nnew_k + wmax - 1 samples of the row,
+    statistics and S/N are the window's (readings C1-C5 applied to it), and only the start positions in its first nnew_k
+    samples are reported.  Returns (sum, sumsq, t, width, snr) with t an index into the row."""
+    row = np.ascontiguousarray(row, dtype=np.int32)
+    L = int(nnew_k) + int(max(widths)) - 1
+    lo = max(0, row.size - L)
+    win = row[lo:]
+    sx, sxx = stats(win)
+    best, bw = best_width(win, widths)
+    tt = np.flatnonzero(best[: int(nnew_k)] >= threshold)
+    return sx, sxx, (tt + lo).astype(np.int32), bw[tt], best[tt]
+
+
 # ---- E. peak filtering (PAPER.md:96) --------------------------------------------------------------------
 def peak_filter(beam: np.ndarray, trial: np.ndarray, t: np.ndarray, snr: np.ndarray, range_of_trial: np.ndarray,
                 windows: Sequence[int] = (3, 11)) -> np.ndarray:

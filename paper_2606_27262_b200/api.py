@@ -58,7 +58,8 @@ SYMBOLS = {
     "spt_peaks_count": (ctypes.c_int, [_vp, _P(_i64)]),
     "spt_peaks_read": (ctypes.c_int, [_vp, _vp, _i64, _P(_i64)]),
     "spt_corner_turn": (ctypes.c_int, [_vp, _i32, _i64, _i32, _i32, _vp, _vp]),
-    "spt_segment_info": (ctypes.c_int, [_vp, _P(_i64), _P(_i64)]),
+    "spt_segment_info": (ctypes.c_int, [_vp, _P(_i64), _P(_i64), _P(_i64)]),
+    "spt_segment_search": (ctypes.c_int, [_vp, _vp, _i32, _i64, _f32, _vp]),
     "spt_segment_push": (ctypes.c_int, [_vp, _vp, _i32, _i64, _i32, _vp, _vp]),
     "spt_stream_push": (ctypes.c_int, [_vp, _vp, _i32, _f32]),
     "spt_stream_pop": (ctypes.c_int, [_vp, _P(_i64), _P(_i32)]),
@@ -261,10 +262,15 @@ class Plan:
         return out[: int(k.value)]
 
     def segment_info(self):
-        """(min_history, granule) in raw samples for spt_segment_push."""
-        h, g = ctypes.c_int64(), ctypes.c_int64()
-        _check(lib().spt_segment_info(self._h, ctypes.byref(h), ctypes.byref(g)), "spt_segment_info")
-        return int(h.value), int(g.value)
+        """(min_history, min_history_search, granule) in raw samples for spt_segment_push / spt_segment_search."""
+        h, hs, g = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_int64()
+        _check(lib().spt_segment_info(self._h, ctypes.byref(h), ctypes.byref(hs), ctypes.byref(g)), "spt_segment_info")
+        return int(h.value), int(hs.value), int(g.value)
+
+    def segment_search(self, d_dmt, nnew: int, threshold: float, stream=None):
+        """Search of the segment just pushed (window = last nnew/k + wmax - 1 samples of every row)."""
+        _check(lib().spt_segment_search(self._h, _dev_ptr(d_dmt), d_dmt.shape[0], int(nnew), float(threshold),
+                                        _stream_ptr(stream)), "spt_segment_search")
 
     def segment_push(self, d_new, flip: bool = False, d_dmt=None, stream=None):
         """Overlap-save push of a time-major CUDA uint8 block [nbeam][nnew][nchan]; returns the DM transform tensor."""

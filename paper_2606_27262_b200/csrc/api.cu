@@ -46,6 +46,9 @@ struct DeviceState {
     // nsamp samples of every channel row
     uint8_t* work[2] = {nullptr, nullptr};
     int work_cur = 0;
+    int32_t* win_len = nullptr;     // [ntrials] search window of a segment and the start positions it reports,
+    int32_t* win_starts = nullptr;  // for the segment length win_nnew
+    int64_t win_nnew = -1;
     // peak filter (lazily allocated): lookup plane laid out like the DM transform, live flags, peak list
     uint32_t* plane = nullptr;
     uint8_t* alive[2] = {nullptr, nullptr};
@@ -129,7 +132,7 @@ static void free_device(Plan* p) {
         cudaFree(r.series);
     }
     cudaFree(d->maxval); cudaFree(d->nout); cudaFree(d->offset); cudaFree(d->range_lo); cudaFree(d->range_hi);
-    cudaFree(d->work[0]); cudaFree(d->work[1]);
+    cudaFree(d->work[0]); cudaFree(d->work[1]); cudaFree(d->win_len); cudaFree(d->win_starts);
     cudaFree(d->plane); cudaFree(d->alive[0]); cudaFree(d->alive[1]); cudaFree(d->peaks); cudaFree(d->peaks_count);
     for (auto& b : d->bufs) { cudaFree(b.sum); cudaFree(b.sumsq); cudaFree(b.cand); cudaFree(b.count); }
     for (auto& sl : d->slot) {
@@ -308,7 +311,8 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
     return SPT_OK;
 }
 
-static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float threshold, cudaStream_t st, int set = 0) {
+static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float threshold, cudaStream_t st, int set = 0,
+                     bool windowed = false) {
     DeviceState* d = p->dev;
     const DeviceState::SearchBufs& bf = d->bufs[set];
     SPT_CUDA(cudaMemsetAsync(bf.count, 0, 8, st));
@@ -326,6 +330,8 @@ static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float thresho
     a.cand = bf.cand;
     a.count = bf.count;
     a.capacity = p->cand_capacity;
+    a.win_len = windowed ? d->win_len : nullptr;
+    a.win_starts = windowed ? d->win_starts : nullptr;
     timed_clear(d, 1);
     {
         ScopedTimer tm(p, st, 1, 3, -1);
@@ -851,19 +857,55 @@ int spt_corner_turn(const uint8_t* d_in, int32_t nbeam, int64_t nsamp, int32_t n
     return SPT_OK;
 }
 
-int spt_segment_info(const spt_plan* plan, int64_t* min_history, int64_t* granule) {
+int spt_segment_info(const spt_plan* plan, int64_t* min_history, int64_t* min_history_search, int64_t* granule) {
     if (!plan) return SPT_ERR_INVALID;
     const Plan& p = plan->p;
-    int64_t h = 0, g = 16;
+    int64_t h = 0, hs = 0, g = 16;
+    const int64_t wmax = p.widths.back();
     for (const RangePlan& rp : p.ranges) {
         int32_t dmax = 0;
         for (int32_t i = 0; i < rp.ndm; ++i) dmax = std::max(dmax, rp.delay[(size_t)i * p.nchan + p.nchan - 1]);
         h = std::max<int64_t>(h, (int64_t)dmax * rp.decim);
+        hs = std::max<int64_t>(hs, ((int64_t)dmax + wmax - 1) * rp.decim);   // the widest boxcar may start in the old part
         g = std::max<int64_t>(g, rp.decim);
     }
     if (min_history) *min_history = (h + g - 1) / g * g;
+    if (min_history_search) *min_history_search = (hs + g - 1) / g * g;
     if (granule) *granule = g;
     return SPT_OK;
+}
+
+int spt_segment_search(spt_plan* plan, const int32_t* d_dmt, int32_t nbeam, int64_t nnew, float threshold, void* cuda_stream) {
+    if (!plan || !d_dmt || nbeam < 1 || nbeam > plan->p.max_beams || !(threshold == threshold)) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    int64_t hmin = 0, hs = 0, gran = 16;
+    spt_segment_info(plan, &hmin, &hs, &gran);
+    if (nnew < 1 || nnew > p.nsamp || nnew % gran != 0) return SPT_ERR_INVALID;
+    if (p.nsamp - nnew < hs) return SPT_ERR_SHAPE;
+    int rc;
+    try {
+        rc = ensure_device(&p);
+    } catch (const std::bad_alloc&) {
+        rc = SPT_ERR_NOMEM;
+    }
+    if (rc != SPT_OK) return rc;
+    DeviceState* d = p.dev;
+    if (d->win_nnew != nnew) {
+        std::vector<int32_t> len, starts;
+        const int32_t wmax = p.widths.back();
+        for (const RangePlan& rp : p.ranges)
+            for (int32_t i = 0; i < rp.ndm; ++i) {
+                const int32_t ns = (int32_t)(nnew / rp.decim);
+                len.push_back(ns + wmax - 1);
+                starts.push_back(ns);
+            }
+        cudaFree(d->win_len); cudaFree(d->win_starts);
+        d->win_len = d->win_starts = nullptr;
+        if ((rc = upload(&d->win_len, len)) != SPT_OK) return rc;
+        if ((rc = upload(&d->win_starts, starts)) != SPT_OK) return rc;
+        d->win_nnew = nnew;
+    }
+    return do_search(&p, d_dmt, nbeam, threshold, (cudaStream_t)cuda_stream, 0, true);
 }
 
 int spt_segment_push(spt_plan* plan, const uint8_t* d_new, int32_t nbeam, int64_t nnew, int32_t flip, int32_t* d_dmt,
@@ -872,7 +914,7 @@ int spt_segment_push(spt_plan* plan, const uint8_t* d_new, int32_t nbeam, int64_
     if ((reinterpret_cast<uintptr_t>(d_dmt) & 127) != 0) return SPT_ERR_INVALID;
     Plan& p = plan->p;
     int64_t hmin = 0, gran = 16;
-    spt_segment_info(plan, &hmin, &gran);
+    spt_segment_info(plan, &hmin, nullptr, &gran);
     // the shift must keep the phase of every decimation and the 16-byte alignment of the rows
     if (nnew < 1 || nnew > p.nsamp || nnew % gran != 0 || p.nsamp % 16 != 0) return SPT_ERR_INVALID;
     if (p.nsamp - nnew < hmin) return SPT_ERR_SHAPE;              // not every trial would have its full sweep

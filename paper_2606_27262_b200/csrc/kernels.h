@@ -38,6 +38,8 @@ struct SpsArgs {
     spt_candidate* cand;
     unsigned long long* count;      // exact number found (may exceed capacity)
     long long capacity;
+    const int32_t* win_len;         // [ntrials] or NULL: search only the last win_len[d] samples of row d ...
+    const int32_t* win_starts;      // [ntrials] or NULL: ... and report only the first win_starts[d] start positions
 };
 void launch_sps(const SpsArgs& a, int32_t nbeam, cudaStream_t st);
 

@@ -86,8 +86,13 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
     __shared__ __align__(16) SpsShared sh;
     const int d = blockIdx.x, b = blockIdx.y;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int n = a.nout[d];
-    if (n <= 0) {
+    const int n = a.nout[d];                                  // end of the row
+    // Window of the row that is searched: the whole row, or -- for a segment of a stream -- its last win_len[d] samples,
+    // of which only the first win_starts[d] start positions are reported (the later ones belong to the next segment).
+    const int lo = a.win_len ? max(0, n - a.win_len[d]) : 0;
+    const int lim = a.win_starts ? a.win_starts[d] : 0x7fffffff;
+    const int nn = n - lo;                                    // N of readings C1-C5
+    if (nn <= 0) {
         if (tid == 0) { a.sum[(int64_t)b * a.ntrials + d] = 0; a.sumsq[(int64_t)b * a.ntrials + d] = 0ull; }
         return;
     }
@@ -98,9 +103,15 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
         long long sx = 0;
         unsigned long long sxx = 0;
         int mn = 0x7fffffff, mx = (int)0x80000000;
-        const int n4 = n >> 2;
+        const int n4 = n >> 2, l4 = (lo + 3) >> 2;            // whole 128-bit words inside [lo, n)
         const int4* x4 = reinterpret_cast<const int4*>(x);
-        for (int i = tid; i < n4; i += kSpsThreads) {
+        for (int i = lo + tid; i < min(n, l4 << 2); i += kSpsThreads) {   // head of a window that starts off a word
+            const int v = x[i];
+            sx += v;
+            sxx += (unsigned long long)(unsigned)v * (unsigned)v;
+            mn = min(mn, v); mx = max(mx, v);
+        }
+        for (int i = l4 + tid; i < n4; i += kSpsThreads) {
             const int4 v = x4[i];
             sx += (long long)v.x + v.y + v.z + v.w;
             sxx += (unsigned long long)(unsigned)v.x * (unsigned)v.x + (unsigned long long)(unsigned)v.y * (unsigned)v.y +
@@ -108,7 +119,7 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
             mn = min(min(mn, v.x), min(v.y, min(v.z, v.w)));
             mx = max(max(mx, v.x), max(v.y, max(v.z, v.w)));
         }
-        for (int i = (n4 << 2) + tid; i < n; i += kSpsThreads) {
+        for (int i = max(n4, l4) * 4 + tid; i < n; i += kSpsThreads) {
             const int v = x[i];
             sx += v;
             sxx += (unsigned long long)(unsigned)v * (unsigned)v;
@@ -131,35 +142,35 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
                 rmn = min(rmn, sh.redmin[w]); rmx = max(rmx, sh.redmax[w]);
             }
             // sigma^2 = (N*Sxx - Sx^2)/N^2 from 128-bit integers (N*Sxx reaches ~1e23)
-            const unsigned long long N = (unsigned long long)n, US = (unsigned long long)S;
+            const unsigned long long N = (unsigned long long)nn, US = (unsigned long long)S;
             const unsigned long long alo = N * Q, ahi = __umul64hi(N, Q);
             const unsigned long long blo = US * US, bhi = __umul64hi(US, US);
             unsigned long long dlo = alo - blo, dhi = ahi - bhi - (alo < blo ? 1ull : 0ull);
             if (ahi < bhi || (ahi == bhi && alo < blo)) { dlo = 0; dhi = 0; }  // cannot happen (Cauchy-Schwarz)
             const double num = (double)dhi * 18446744073709551616.0 + (double)dlo;
-            const double sigma = sqrt(num / ((double)n * (double)n));
-            const int live = (sigma > 0.0 && n >= 2) ? 1 : 0;
+            const double sigma = sqrt(num / ((double)nn * (double)nn));
+            const int live = (sigma > 0.0 && nn >= 2) ? 1 : 0;
             // integer mean and the fast-path test: every boxcar sum of x - m stays below 2^30 in magnitude
-            const long long m = (2 * S + (long long)n) / (2 * (long long)n);             // S >= 0: round half up
+            const long long m = (2 * S + (long long)nn) / (2 * (long long)nn);           // S >= 0: round half up
             const long long dev = max((long long)rmx - m, m - (long long)rmn);
             const int wmax = a.widths[a.nw - 1];
-            const int fast = (dev * (long long)min(wmax, n) < (1ll << 30)) ? 1 : 0;
-            const long long r = S - (long long)n * m;                                    // |r| <= N/2
+            const int fast = (dev * (long long)min(wmax, nn) < (1ll << 30)) ? 1 : 0;
+            const long long r = S - (long long)nn * m;                                   // |r| <= N/2
             if (tid == 0) {
                 a.sum[(int64_t)b * a.ntrials + d] = S;
                 a.sumsq[(int64_t)b * a.ntrials + d] = Q;
                 sh.S = S; sh.Q = Q; sh.live = live; sh.fast = fast; sh.m = (int)m;
                 int ne = 0;
-                while (ne < a.nw && a.widths[ne] <= n) ++ne;                             // widths > N never apply
+                while (ne < a.nw && a.widths[ne] <= nn) ++ne;                            // widths > N never apply
                 sh.nw_eff = ne;
             }
             if (tid < a.nw) {
                 const double w = (double)a.widths[tid];
-                const double nsig = ((double)n * sigma) * sqrt(w);
+                const double nsig = ((double)nn * sigma) * sqrt(w);
                 sh.scale[tid] = live ? 1.0 / nsig : 0.0;
                 sh.wsum[tid] = (long long)a.widths[tid] * (fast ? r : S);
                 // tau_w = (threshold*N*sigma*sqrt(w) + w*r)/N ; the integer test uses a floor that can only be too low
-                double tau = (a.threshold * nsig + (double)((long long)a.widths[tid] * r)) / (double)n;
+                double tau = (a.threshold * nsig + (double)((long long)a.widths[tid] * r)) / (double)nn;
                 tau = floor(tau - fabs(tau) * 1e-9 - 1e-6);
                 tau = fmin(fmax(tau, -1073741824.0), 1073741824.0);
                 sh.negT[tid] = -(int)tau;
@@ -170,10 +181,11 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
     if (!sh.live) return;  // sigma == 0 or N < 2: S/N == 0 everywhere, no candidates (reading C1)
 
     const int w0 = a.widths[0], wmax = a.widths[a.nw - 1];
-    const int nbest = n - w0 + 1;              // best[t] is defined for t in [0, N - wmin]  (reading C5)
-    if (nbest <= 0) return;
-    const int halo = min(wmax, n);             // widths > N never apply
-    const long long N64 = n;
+    const int lo_al = lo & ~3;                 // staging starts on a 128-bit word; slots before lo are not start positions
+    const int nbest = min(nn - w0 + 1, lim) + (lo - lo_al);   // best[t] is defined for t - lo in [0, N - wmin]  (reading C5)
+    if (nbest <= lo - lo_al) return;
+    const int halo = min(wmax, nn);            // widths > N never apply
+    const long long N64 = nn;
 
     if (sh.fast) {
         // ---- pass 2, fast path ---------------------------------------------------------------------------------------
@@ -187,15 +199,15 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
             int tot = 0;
 #pragma unroll
             for (int it = 0; it < kIters; ++it) {
-                const int e = tb + warp * kWarpSpan + it * 128 + lane * 4;
-                if (e + 4 <= n) {
+                const int e = lo_al + tb + warp * kWarpSpan + it * 128 + lane * 4;
+                if (e >= lo && e + 4 <= n) {
                     v[it] = *reinterpret_cast<const int4*>(x + e);
                     v[it].x -= m; v[it].y -= m; v[it].z -= m; v[it].w -= m;
-                } else {
-                    v[it].x = e < n ? x[e] - m : 0;
-                    v[it].y = e + 1 < n ? x[e + 1] - m : 0;
-                    v[it].z = e + 2 < n ? x[e + 2] - m : 0;
-                    v[it].w = 0;
+                } else {                                          // the ends of the window: zero outside [lo, n)
+                    v[it].x = (e >= lo && e < n) ? x[e] - m : 0;
+                    v[it].y = (e + 1 >= lo && e + 1 < n) ? x[e + 1] - m : 0;
+                    v[it].z = (e + 2 >= lo && e + 2 < n) ? x[e + 2] - m : 0;
+                    v[it].w = (e + 3 >= lo && e + 3 < n) ? x[e + 3] - m : 0;
                 }
                 tot += v[it].x + v[it].y + v[it].z + v[it].w;
             }
@@ -243,12 +255,12 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
 #pragma unroll
                 for (int e = 0; e < kEpt; ++e) {
                     const int i = i0 + e * kSpsThreads + tid;
-                    const bool pre = i < nthis && mxv[e] >= 0;
+                    const int t = lo_al + tb + i;
+                    const bool pre = i < nthis && t >= lo && mxv[e] >= 0;
                     if (!__any_sync(0xffffffffu, pre)) continue;
                     bool hit = false;
                     double best = 0.0;
                     int bw = w0;
-                    const int t = tb + i;
                     if (pre)
                         hit = best_of(sh, a, t, n, N64, [&](int, int w) { return (long long)(int)(sh.c[kCOff + i + w] - sh.c[kCOff + i]); },
                                       best, bw);
@@ -267,8 +279,8 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
             // load kXEpt consecutive samples per thread (coalesced via shared memory), zero beyond N
             __syncthreads();
             for (int i = tid; i < kXSeg; i += kSpsThreads) {
-                const int t = tb + i;
-                s_c[padi(i + 1)] = t < n ? (uint32_t)x[t] : 0u;
+                const int t = lo_al + tb + i;
+                s_c[padi(i + 1)] = (t >= lo && t < n) ? (uint32_t)x[t] : 0u;
             }
             __syncthreads();
             uint32_t v[kXEpt];
@@ -294,11 +306,11 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
             const int nthis = min(adv, nbest - tb);
             for (int i0 = 0; i0 < nthis; i0 += kSpsThreads) {
                 const int i = i0 + tid;
-                const int t = tb + i;
+                const int t = lo_al + tb + i;
                 bool hit = false;
                 double best = 0.0;
                 int bw = w0;
-                if (i < nthis)
+                if (i < nthis && t >= lo)
                     hit = best_of(sh, a, t, n, N64, [&](int, int w) { return (long long)(uint32_t)(s_c[padi(i + w)] - s_c[padi(i)]); },
                                   best, bw);                          // exact: S < 2^32 (plan check)
                 append(a, hit, b, d, t, bw, best, lane);

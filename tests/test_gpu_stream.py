@@ -23,7 +23,7 @@ def test_overlap_save_segments(cuda, api, orc):
     nchan, nnew = 256, 2048
     w = Shape(500.0, -200.0 / nchan, nchan, 0, [(0.0, 0.2, 70, 1), (10.0, 0.5, 40, 2), (30.0, 1.0, 33, 4)], [1, 2, 4], 6.0, nbeam=2)
     probe = api.Plan(w.fch1, w.foff, nchan, w.tsamp, 1 << 16, w.ranges, w.widths)
-    hmin, gran = probe.segment_info()
+    hmin, _, gran = probe.segment_info()
     assert gran == 16 and hmin % 16 == 0 and hmin > 0
     w.nsamp = hmin + nnew                                          # exactly the shortest legal history
     rs = np.random.default_rng(9)
@@ -52,3 +52,53 @@ def test_overlap_save_segments(cuda, api, orc):
     with pytest.raises(api.SptError) as e:
         plan.segment_push(cuda.from_numpy(blocks[0][:, : nnew - 8]).cuda())
     assert e.value.code == api.SPT_ERR_INVALID
+
+
+def test_segment_search_matches_the_oracle_window(cuda, api, orc):
+    """spt_segment_search after every push: per trial, statistics and candidates of the window (last nnew/k + wmax - 1
+    samples) restricted to its first nnew/k start positions, against the oracle's composition of C1-C5 on that window."""
+    nchan, nnew = 128, 4096
+    widths = [1, 2, 8, 32]
+    w = Shape(500.0, -200.0 / nchan, nchan, 0, [(0.0, 0.5, 40, 1), (20.0, 1.0, 24, 2), (50.0, 2.0, 17, 4)], widths, 3.5, nbeam=1)
+    probe = api.Plan(w.fch1, w.foff, nchan, w.tsamp, 1 << 16, w.ranges, w.widths)
+    hmin, hsearch, gran = probe.segment_info()
+    assert hsearch >= hmin + (max(widths) - 1) * 4 - gran
+    w.nsamp = hsearch + nnew
+    plan = make_plan(api, w, cand_capacity=1 << 22)
+    with pytest.raises(api.SptError) as e:                         # a history that covers the sweeps but not the widest boxcar
+        make_plan(api, w, nsamp=hmin + nnew).segment_search(cuda.zeros((1, 8), dtype=cuda.int32, device="cuda"), nnew, 5.0)
+    assert e.value.code == api.SPT_ERR_SHAPE
+    rs = np.random.default_rng(21)
+    _, _, dec, nout, off = plan.trial_table()
+    total = 0
+    for i in range(3):
+        blk = rs.normal(128, 12, size=(1, nnew, nchan)).round().clip(0, 255).astype(np.uint8)
+        blk[0, 1000 + 300 * i: 1003 + 300 * i, :] += 20            # a zero-DM spike per segment
+        d_dmt = plan.segment_push(cuda.from_numpy(blk).cuda())
+        plan.segment_search(d_dmt, nnew, w.threshold)
+        n, ovf = plan.candidates_count()
+        assert not ovf
+        cands = plan.candidates_read()
+        s_all, q_all = plan.trial_stats_all(1)
+        dmt = d_dmt.cpu().numpy()[0]
+        got = {}
+        for c in cands:
+            got.setdefault(int(c["trial"]), []).append((int(c["t"]), int(c["width"]), float(c["snr"])))
+        for d in range(plan.ntrials):
+            row = dmt[off[d]: off[d] + nout[d]]
+            sx, sxx, t, bw, snr = orc.search_segment(row, widths, w.threshold, nnew // int(dec[d]))
+            assert (int(s_all[0, d]), int(q_all[0, d])) == (sx, sxx), d
+            g = sorted(got.get(d, []))
+            exp = sorted(zip(t.tolist(), bw.tolist(), snr.tolist()))
+            near = [x for x in exp if abs(x[2] - w.threshold) <= 1e-3]
+            assert abs(len(g) - len(exp)) <= len(near), (d, len(g), len(exp))
+            ge = {x[0]: x for x in g}
+            for (tt, ww, ss) in exp:
+                if tt in ge:
+                    assert ge[tt][1] == ww and abs(ge[tt][2] - ss) <= 1e-3, (d, tt)
+                else:
+                    assert abs(ss - w.threshold) <= 1e-3
+            lo = nout[d] - (nnew // int(dec[d]) + max(widths) - 1)
+            assert all(lo <= x[0] < lo + nnew // int(dec[d]) for x in g)      # only this segment's start positions
+        total += n
+    assert total > 1000

@@ -40,3 +40,24 @@ def test_overlap_save_continues_the_dm_transform(orc):
             a = i * nnew                                                  # buffer start inside the long observation
             assert np.array_equal(row, full[off_w[d] + a: off_w[d] + a + no[d]])
             assert no[d] >= nnew                                          # every push yields nnew new outputs per trial
+
+
+def test_segment_windows_report_every_start_once(orc):
+    """Window arithmetic of the segment search (reading F): with row length n, segment length s and widest boxcar wmax,
+    segment i reports the row-relative starts [n - s - (wmax-1), n - (wmax-1)), i.e. the stream starts
+    [i*s + n - s - wmax + 1, (i+1)*s + n - s - wmax + 1): consecutive segments tile the stream, and every reported start
+    has all its boxcars inside the data seen so far."""
+    rs = np.random.default_rng(0)
+    n, s, widths = 300, 64, [1, 4, 16]
+    stream = rs.integers(0, 1000, size=n + 5 * s).astype(np.int32)
+    seen = []
+    for i in range(6):
+        row = stream[i * s: i * s + n]                              # what the push leaves in the row (it slid by s)
+        sx, sxx, t, bw, snr = orc.search_segment(row, widths, -1e9, s)      # threshold so low that every start is reported
+        assert t.size == s and t[0] == n - s - (max(widths) - 1) and np.all(np.diff(t) == 1)
+        assert np.all(t + max(widths) <= n)                         # the widest boxcar fits
+        seen.append(t + i * s)                                      # stream positions
+        win = row[n - (s + max(widths) - 1):]
+        assert sx == int(win.sum())                                 # statistics are the window's
+    allpos = np.concatenate(seen)
+    assert np.array_equal(allpos, np.arange(allpos[0], allpos[0] + 6 * s))   # contiguous, no gap, no repeat
