@@ -82,6 +82,8 @@ __device__ __forceinline__ void append(const SpsArgs& a, bool hit, int b, int d,
     }
 }
 
+// WIN = false: the whole row (the window logic folds away); WIN = true: a segment's window
+template <bool WIN>
 __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
     __shared__ __align__(16) SpsShared sh;
     const int d = blockIdx.x, b = blockIdx.y;
@@ -89,8 +91,8 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
     const int n = a.nout[d];                                  // end of the row
     // Window of the row that is searched: the whole row, or -- for a segment of a stream -- its last win_len[d] samples,
     // of which only the first win_starts[d] start positions are reported (the later ones belong to the next segment).
-    const int lo = a.win_len ? max(0, n - a.win_len[d]) : 0;
-    const int lim = a.win_starts ? a.win_starts[d] : 0x7fffffff;
+    const int lo = WIN ? max(0, n - a.win_len[d]) : 0;
+    const int lim = WIN ? a.win_starts[d] : 0x7fffffff;
     const int nn = n - lo;                                    // N of readings C1-C5
     if (nn <= 0) {
         if (tid == 0) { a.sum[(int64_t)b * a.ntrials + d] = 0; a.sumsq[(int64_t)b * a.ntrials + d] = 0ull; }
@@ -322,7 +324,8 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
 void launch_sps(const SpsArgs& a, int32_t nbeam, cudaStream_t st) {
     if (a.ntrials <= 0 || nbeam <= 0) return;
     dim3 grid((unsigned)a.ntrials, (unsigned)nbeam);
-    sps_kernel<<<grid, kSpsThreads, 0, st>>>(a);
+    if (a.win_len) sps_kernel<true><<<grid, kSpsThreads, 0, st>>>(a);
+    else sps_kernel<false><<<grid, kSpsThreads, 0, st>>>(a);
 }
 
 }  // namespace spt
