@@ -253,6 +253,90 @@ def peak_filter(beam: np.ndarray, trial: np.ndarray, t: np.ndarray, snr: np.ndar
     return alive.astype(bool)
 
 
+# ---- G. candidate sifting ---------------------------------------------------------------
+def dbscan(x: np.ndarray, y: np.ndarray, eps: float, min_pts: int) -> Tuple[np.ndarray, np.ndarray]:
+    """DBSCAN (Ester et al. 1996) written out: a point is a CORE point when at least min_pts points (itself included)
+    lie within eps of it; core points within eps of each other are in the same cluster (transitively); a non-core point
+    within eps of a core point is a BORDER point.  Returns (is_core, core_label) where core_label[i] for a core point is
+    the smallest index among the core points of its cluster (-1 for non-core points)."""
+    x = np.asarray(x, dtype=np.float64)
+    y = np.asarray(y, dtype=np.float64)
+    n = x.size
+    dx = x[:, None] - x[None, :]
+    dy = y[:, None] - y[None, :]
+    near = (dx * dx + dy * dy) <= eps * eps
+    core = near.sum(axis=1) >= min_pts
+    label = np.full(n, -1, dtype=np.int64)
+    for i in range(n):                                   # flood fill over core points, smallest index first
+        if not core[i] or label[i] >= 0:
+            continue
+        label[i] = i
+        stack = [i]
+        while stack:
+            a = stack.pop()
+            for b in np.flatnonzero(near[a] & core & (label < 0)):
+                label[b] = i
+                stack.append(int(b))
+    return core, label
+
+
+def sift(beam, trial, t, width, snr, dm_of_trial, decim_of_trial, tsamp: float, nbeam: int, eps: float = 0.5,
+         min_pts: int = 5, time_unit_s: float = 1.0, dm_unit: float = 1.0, snr_min: float = 10.0, dm_min: float = 10.0,
+         width_max_s: float = 0.1, coinc_window_s: float = 0.0, coinc_beam_fraction: float = 0.5):
+    """The candidate optimisation of PAPER.md:104/112 (reading G), stage by stage; returns the boolean masks after
+    (clustering, cuts, anti-coincidence) over the input list.
+      1 per beam: DBSCAN in the plane (arrival time / time_unit_s, DM / dm_unit); clusters need a core point (>= min_pts
+        points within eps); a border point joins the cluster of its strongest core neighbour (largest S/N, then smallest
+        (trial, t)); out of each cluster the member with the highest S/N (then smallest (trial, t)) is kept; points in no
+        cluster are rejected.
+      2 cuts: rejected when S/N < snr_min, DM < dm_min or width (seconds) > width_max_s.
+      3 anti-coincidence (coinc_window_s > 0): a survivor is rejected when survivors of MORE than coinc_beam_fraction * nbeam
+        distinct beams (its own included) arrive within coinc_window_s of it."""
+    beam = np.asarray(beam); trial = np.asarray(trial); t = np.asarray(t); width = np.asarray(width)
+    snr = np.asarray(snr, dtype=np.float64)
+    dm = np.asarray(dm_of_trial, dtype=np.float64)[trial]
+    k = np.asarray(decim_of_trial, dtype=np.int64)[trial]
+    arrival = (t.astype(np.float64) * k.astype(np.float64)) * tsamp            # seconds, at the top of the band
+    wsec = (width.astype(np.float64) * k.astype(np.float64)) * tsamp
+    n = beam.size
+    keep1 = np.zeros(n, dtype=bool)
+
+    def stronger(a, b):                                  # is candidate a stronger than b
+        return snr[a] > snr[b] or (snr[a] == snr[b] and (trial[a], t[a]) < (trial[b], t[b]))
+
+    for b in np.unique(beam):
+        idx = np.flatnonzero(beam == b)
+        xs, ys = arrival[idx] / time_unit_s, dm[idx] / dm_unit
+        core, label = dbscan(xs, ys, eps, min_pts)
+        member = label.copy()
+        dx = xs[:, None] - xs[None, :]
+        dy = ys[:, None] - ys[None, :]
+        near = (dx * dx + dy * dy) <= eps * eps
+        for i in np.flatnonzero(~core):
+            best = -1
+            for j in np.flatnonzero(near[i] & core):
+                if best < 0 or stronger(idx[j], idx[best]):
+                    best = int(j)
+            if best >= 0:
+                member[i] = label[best]
+        for c in np.unique(member[member >= 0]):
+            mem = np.flatnonzero(member == c)
+            top = mem[0]
+            for j in mem[1:]:
+                if stronger(idx[j], idx[top]):
+                    top = j
+            keep1[idx[top]] = True
+    keep2 = keep1 & (snr >= snr_min) & (dm >= dm_min) & (wsec <= width_max_s)
+    keep3 = keep2.copy()
+    if coinc_window_s > 0.0:
+        s = np.flatnonzero(keep2)
+        for i in s:
+            beams = set(int(beam[j]) for j in s if abs(arrival[j] - arrival[i]) <= coinc_window_s)
+            if len(beams) > coinc_beam_fraction * nbeam:
+                keep3[i] = False
+    return keep1, keep2, keep3
+
+
 # ---- whole path over a plan (one beam) ----------------------------------------------------------------
 @dataclass
 class RangeResult:
