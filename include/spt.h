@@ -237,6 +237,34 @@ int spt_segment_search(spt_plan* plan, const int32_t* d_dmt /*DEVICE*/, int32_t 
 int spt_segment_push(spt_plan* plan, const uint8_t* d_new /*DEVICE*/, int32_t nbeam, int64_t nnew, int32_t flip,
                      int32_t* d_dmt /*DEVICE*/, void* cuda_stream);
 
+/* -------------------------------------------------------------------------------------------------------
+ * spt_sift -- candidate optimisation after the search (reading G), on a HOST list (typically
+ * what spt_peaks_read returned for all beams of a batch):
+ *   1 per beam, DBSCAN (Ester et al. 1996) in the plane (arrival time / time_unit_s, DM / dm_unit) with radius eps and
+ *     min_pts points (the point itself included) for a core point (eps = 0.5, 5 points); a border point
+ *     joins the cluster of its strongest core neighbour; out of each cluster the member with the highest snr (then the
+ *     smaller (trial, t)) is kept, candidates in no cluster are rejected;
+ *   2 cuts: rejected when snr < snr_min, DM < dm_min or width*decim*tsamp > width_max_s (10, 10, 0.1 s);
+ *   3 anti-coincidence (off when coinc_window_s <= 0): rejected when survivors of more than
+ *     coinc_beam_fraction * nbeam distinct beams (its own included) arrive within coinc_window_s of it.
+ * Arrival time = t*decim*tsamp at the top of the band.  h_out (HOST, cap records) receives the survivors, order
+ * arbitrary; stage_counts (HOST, 3 entries, may be NULL) the number left after each stage.  Synchronous; the plan only
+ * supplies the trial table.  nbeam <= 1024.
+ * ----------------------------------------------------------------------------------------------------- */
+typedef struct {
+    double eps;                 /* neighbourhood radius in plane units (paper: 0.5) */
+    double time_unit_s;         /* seconds per plane unit of the time axis */
+    double dm_unit;             /* pc cm^-3 per plane unit of the DM axis */
+    int32_t min_pts;            /* paper: 5 */
+    float snr_min;              /* paper: 10 */
+    double dm_min;              /* paper: 10 pc cm^-3 */
+    double width_max_s;         /* paper: 0.1 s */
+    double coinc_window_s;      /* <= 0: no anti-coincidence stage */
+    double coinc_beam_fraction; /* "a majority of the beams": 0.5 */
+} spt_sift_params;
+int spt_sift(spt_plan* plan, const spt_candidate* h_in /*HOST*/, int64_t n, int32_t nbeam, const spt_sift_params* params,
+             spt_candidate* h_out /*HOST*/, int64_t cap, int64_t* nwritten, int64_t* stage_counts /*HOST[3]*/);
+
 /* With option "profile" = 1: device time (ms) of each kernel launched by the LAST spt_dedisperse and the LAST
  * spt_single_pulse_search, in launch order; kinds: 1 = decimate, 2 = dedisperse, 3 = single-pulse search; `range` is the
  * DM range the launch served (-1 for the search).  Synchronises.  Arrays (HOST) hold `cap` entries; n = entries written. */

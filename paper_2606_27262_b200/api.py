@@ -29,6 +29,13 @@ class spt_candidate(ctypes.Structure):
                 ("width", ctypes.c_int32), ("snr", ctypes.c_float)]
 
 
+class spt_sift_params(ctypes.Structure):
+    _fields_ = [("eps", ctypes.c_double), ("time_unit_s", ctypes.c_double), ("dm_unit", ctypes.c_double),
+                ("min_pts", ctypes.c_int32), ("snr_min", ctypes.c_float), ("dm_min", ctypes.c_double),
+                ("width_max_s", ctypes.c_double), ("coinc_window_s", ctypes.c_double),
+                ("coinc_beam_fraction", ctypes.c_double)]
+
+
 CAND_DTYPE = np.dtype([("beam", "<i4"), ("trial", "<i4"), ("t", "<i4"), ("width", "<i4"), ("snr", "<f4")])
 
 # every symbol include/spt.h declares: name -> (restype, argtypes)
@@ -61,6 +68,7 @@ SYMBOLS = {
     "spt_segment_info": (ctypes.c_int, [_vp, _P(_i64), _P(_i64), _P(_i64)]),
     "spt_segment_search": (ctypes.c_int, [_vp, _vp, _i32, _i64, _f32, _vp]),
     "spt_segment_push": (ctypes.c_int, [_vp, _vp, _i32, _i64, _i32, _vp, _vp]),
+    "spt_sift": (ctypes.c_int, [_vp, _vp, _i64, _i32, _P(spt_sift_params), _vp, _i64, _P(_i64), _P(_i64)]),
     "spt_stream_push": (ctypes.c_int, [_vp, _vp, _i32, _f32]),
     "spt_stream_pop": (ctypes.c_int, [_vp, _P(_i64), _P(_i32)]),
     "spt_plan_kernel_times": (ctypes.c_int, [_vp, _i32, _vp, _vp, _vp, _P(_i32)]),
@@ -283,6 +291,20 @@ class Plan:
         _check(lib().spt_segment_push(self._h, _dev_ptr(d_new), nbeam, nnew, int(bool(flip)), _dev_ptr(d_dmt),
                                       _stream_ptr(stream)), "spt_segment_push")
         return d_dmt
+
+    def sift(self, cands: np.ndarray, nbeam: int, eps: float = 0.5, min_pts: int = 5, time_unit_s: float = 1.0,
+             dm_unit: float = 1.0, snr_min: float = 10.0, dm_min: float = 10.0, width_max_s: float = 0.1,
+             coinc_window_s: float = 0.0, coinc_beam_fraction: float = 0.5):
+        """Candidate optimisation of a host list of records; returns (survivors, stage counts)."""
+        cands = np.ascontiguousarray(cands, dtype=CAND_DTYPE)
+        prm = spt_sift_params(eps, time_unit_s, dm_unit, min_pts, snr_min, dm_min, width_max_s, coinc_window_s,
+                              coinc_beam_fraction)
+        out = np.empty(max(cands.size, 1), dtype=CAND_DTYPE)
+        nw = ctypes.c_int64()
+        stages = (ctypes.c_int64 * 3)()
+        _check(lib().spt_sift(self._h, cands.ctypes.data, cands.size, nbeam, ctypes.byref(prm), out.ctypes.data, cands.size,
+                              ctypes.byref(nw), stages), "spt_sift")
+        return out[: int(nw.value)], [int(v) for v in stages]
 
     def stream_push(self, h_fb, threshold: float):
         """Enqueue one batch (HOST uint8 [nbeam][nchan][nsamp], pinned) into the two-deep pipeline; returns at once."""

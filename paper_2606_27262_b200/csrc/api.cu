@@ -946,6 +946,97 @@ int spt_segment_push(spt_plan* plan, const uint8_t* d_new, int32_t nbeam, int64_
     return do_dedisperse(&p, cur, nbeam, d_dmt, st);
 }
 
+int spt_sift(spt_plan* plan, const spt_candidate* h_in, int64_t n, int32_t nbeam, const spt_sift_params* prm,
+             spt_candidate* h_out, int64_t cap, int64_t* nwritten, int64_t* stage_counts) {
+    if (!plan || !prm || (!h_in && n > 0) || n < 0 || nbeam < 1 || cap < 0 || (!h_out && cap > 0)) return SPT_ERR_INVALID;
+    if (!(prm->eps > 0.0) || prm->min_pts < 1 || !(prm->time_unit_s > 0.0) || !(prm->dm_unit > 0.0)) return SPT_ERR_INVALID;
+    if (nbeam > kSiftMaxBeams || n >= (1ll << 31)) return SPT_ERR_UNSUPPORTED;
+    Plan& p = plan->p;
+    if (nwritten) *nwritten = 0;
+    if (stage_counts) stage_counts[0] = stage_counts[1] = stage_counts[2] = 0;
+    if (n == 0) return SPT_OK;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) { cudaGetLastError(); g_last_error = "no CUDA device"; return SPT_ERR_CUDA; }
+    // host: order by (beam, trial, t) -- the index then breaks S/N ties towards the smaller (trial, t) -- and the plane
+    std::vector<int64_t> order((size_t)n);
+    for (int64_t i = 0; i < n; ++i) {
+        if (h_in[i].beam < 0 || h_in[i].beam >= nbeam || h_in[i].trial < 0 || h_in[i].trial >= p.ntrials) return SPT_ERR_SHAPE;
+        order[(size_t)i] = i;
+    }
+    std::sort(order.begin(), order.end(), [&](int64_t a, int64_t b) {
+        const spt_candidate &u = h_in[a], &v = h_in[b];
+        if (u.beam != v.beam) return u.beam < v.beam;
+        if (u.trial != v.trial) return u.trial < v.trial;
+        return u.t < v.t;
+    });
+    std::vector<double> x((size_t)n), y((size_t)n), dm((size_t)n), wsec((size_t)n), arr((size_t)n);
+    std::vector<float> snr((size_t)n);
+    std::vector<int32_t> beam((size_t)n);
+    std::vector<int64_t> lo((size_t)n), hi((size_t)n);
+    for (int64_t i = 0; i < n; ++i) {
+        const spt_candidate& c = h_in[order[(size_t)i]];
+        int32_t loc = 0;
+        const RangePlan* rp = range_of_trial(p, c.trial, &loc);
+        const double k = (double)rp->decim;
+        dm[(size_t)i] = rp->dm_lo + (double)loc * rp->dm_step;
+        arr[(size_t)i] = ((double)c.t * k) * p.tsamp;                  // arrival at the top of the band, seconds
+        wsec[(size_t)i] = ((double)c.width * k) * p.tsamp;
+        x[(size_t)i] = arr[(size_t)i] / prm->time_unit_s;
+        y[(size_t)i] = dm[(size_t)i] / prm->dm_unit;
+        snr[(size_t)i] = c.snr;
+        beam[(size_t)i] = c.beam;
+    }
+    for (int64_t i = 0, s0 = 0; i <= n; ++i)
+        if (i == n || beam[(size_t)i] != beam[(size_t)s0]) {
+            for (int64_t j = s0; j < i; ++j) { lo[(size_t)j] = s0; hi[(size_t)j] = i; }
+            s0 = i;
+        }
+    // device: one allocation for everything
+    const size_t nn = (size_t)n;
+    const size_t bytes = nn * (5 * 8 + 4 + 4 + 2 * 8 + 3 * 4 + 8 + 4) + 256;
+    uint8_t* buf = nullptr;
+    SPT_CUDA(cudaMalloc((void**)&buf, bytes));
+    uint8_t* q = buf;
+    auto take = [&](size_t b) { uint8_t* r = q; q += (b + 15) / 16 * 16; return r; };
+    SiftArgs a{};
+    double *dx = (double*)take(nn * 8), *dy = (double*)take(nn * 8), *ddm = (double*)take(nn * 8), *dw = (double*)take(nn * 8),
+           *da = (double*)take(nn * 8);
+    int64_t *dlo = (int64_t*)take(nn * 8), *dhi = (int64_t*)take(nn * 8);
+    unsigned long long* drep = (unsigned long long*)take(nn * 8);
+    float* dsnr = (float*)take(nn * 4);
+    int32_t *dbeam = (int32_t*)take(nn * 4), *dcore = (int32_t*)take(nn * 4), *dpar = (int32_t*)take(nn * 4),
+            *dmem = (int32_t*)take(nn * 4), *dkeep = (int32_t*)take(nn * 4);
+    cudaError_t ce = cudaSuccess;
+    auto up = [&](void* d, const void* h, size_t b) { if (ce == cudaSuccess) ce = cudaMemcpy(d, h, b, cudaMemcpyHostToDevice); };
+    up(dx, x.data(), nn * 8); up(dy, y.data(), nn * 8); up(ddm, dm.data(), nn * 8); up(dw, wsec.data(), nn * 8);
+    up(da, arr.data(), nn * 8); up(dlo, lo.data(), nn * 8); up(dhi, hi.data(), nn * 8); up(dsnr, snr.data(), nn * 4);
+    up(dbeam, beam.data(), nn * 4);
+    if (ce == cudaSuccess) ce = cudaMemset(drep, 0, nn * 8);
+    if (ce == cudaSuccess) ce = cudaMemset(dkeep, 0, nn * 4);
+    a.n = n; a.nbeam = nbeam; a.min_pts = prm->min_pts;
+    a.eps2 = prm->eps * prm->eps; a.snr_min = (double)prm->snr_min; a.dm_min = prm->dm_min; a.width_max_s = prm->width_max_s;
+    a.coinc_window_s = prm->coinc_window_s; a.coinc_beam_fraction = prm->coinc_beam_fraction;
+    a.x = dx; a.y = dy; a.dm = ddm; a.wsec = dw; a.arrival = da; a.snr = dsnr; a.beam = dbeam; a.seg_lo = dlo; a.seg_hi = dhi;
+    a.core = dcore; a.parent = dpar; a.member = dmem; a.rep = drep; a.keep = dkeep;
+    std::vector<int32_t> keep(nn, 0);
+    if (ce == cudaSuccess) {
+        launch_sift(a, nullptr);
+        p.launches += 5;
+        ce = cudaGetLastError();
+    }
+    if (ce == cudaSuccess) ce = cudaMemcpy(keep.data(), dkeep, nn * 4, cudaMemcpyDeviceToHost);
+    cudaFree(buf);
+    if (ce != cudaSuccess) return cuda_fail(ce, "spt_sift");
+    int64_t w = 0;
+    for (int64_t i = 0; i < n; ++i) {
+        const int32_t kf = keep[(size_t)i];
+        if (stage_counts) { stage_counts[0] += kf & 1; stage_counts[1] += (kf >> 1) & 1; stage_counts[2] += (kf >> 2) & 1; }
+        if ((kf & 4) && w < cap) h_out[w++] = h_in[order[(size_t)i]];
+    }
+    if (nwritten) *nwritten = w;
+    return SPT_OK;
+}
+
 int spt_plan_kernel_times(spt_plan* plan, int32_t cap, int32_t* kind, int32_t* range, double* ms, int32_t* n) {
     if (!plan || !n || cap < 0) return SPT_ERR_INVALID;
     Plan& p = plan->p;

@@ -63,6 +63,28 @@ void launch_corner_turn(const uint8_t* in, int32_t nbeam, int64_t nsamp, int32_t
 void launch_keep_history(const uint8_t* src, uint8_t* dst, int64_t row_bytes, int64_t shift_bytes, int64_t keep_bytes,
                          int64_t nrows, cudaStream_t st);
 
+constexpr int kSiftMaxBeams = 1024;
+struct SiftArgs {                   // all arrays DEVICE, n entries sorted by (beam, trial, t)
+    int64_t n;
+    int32_t nbeam, min_pts;
+    double eps2, snr_min, dm_min, width_max_s, coinc_window_s, coinc_beam_fraction;
+    const double* x;                // arrival time / time unit
+    const double* y;                // DM / DM unit
+    const double* dm;
+    const double* wsec;             // width in seconds
+    const double* arrival;          // seconds
+    const float* snr;
+    const int32_t* beam;
+    const int64_t* seg_lo;          // [n] first / one-past-last candidate of the same beam
+    const int64_t* seg_hi;
+    int32_t* core;
+    int32_t* parent;
+    int32_t* member;
+    unsigned long long* rep;        // [n] zeroed: best (S/N, index) key of the cluster rooted here
+    int32_t* keep;                  // bit 0 after clustering, bit 1 after the cuts, bit 2 after anti-coincidence
+};
+void launch_sift(const SiftArgs& a, cudaStream_t st);
+
 int run_probe(int kind, int reps, double* warp_instr_per_s, double* elapsed_ms);
 
 }  // namespace spt
