@@ -52,6 +52,10 @@ def lib():
         L.orc_best_width.argtypes = [vp, i64, vp, i32, vp, vp]
         L.orc_snr_at.argtypes = [vp, i64, i32, i64, vp]
         L.orc_search_plane.argtypes = [vp, i32, vp, vp, vp, i32, f64, vp, vp, vp, vp, vp, vp, vp]
+        L.orc_cutout.argtypes = [vp, i32, i64, f64, f64, f64, f64, f64, i32, i64, i32, i32, i32, vp, vp]
+        L.orc_cutout.restype = ctypes.c_int
+        L.orc_delta_dm.argtypes = [f64, f64, f64, f64, f64]
+        L.orc_delta_dm.restype = f64
         L.orc_peak_filter.argtypes = [i64, vp, vp, vp, vp, vp, i32, i32, vp]
         L.orc_peak_filter.restype = ctypes.c_int
         for name in ("orc_delay_table", "orc_nout", "orc_decimate", "orc_dedisperse_u16", "orc_dedisperse_u8",
@@ -335,6 +339,23 @@ def sift(beam, trial, t, width, snr, dm_of_trial, decim_of_trial, tsamp: float, 
             if len(beams) > coinc_beam_fraction * nbeam:
                 keep3[i] = False
     return keep1, keep2, keep3
+
+
+# ---- H. candidate cut-outs (Eq. 4) -------------------------------------------------------
+def cutout(x: np.ndarray, fch1: float, foff: float, tsamp: float, dm0: float, ddm: float, ndm: int, ts: int, tbin: int,
+           nt: int, nf: int) -> Tuple[np.ndarray, np.ndarray]:
+    """(dedispersed dynamic spectrum [nf][nt], DM transform [ndm][nt]) of one candidate, integers."""
+    x = np.ascontiguousarray(x, dtype=np.uint8)
+    dds = np.zeros((nf, nt), dtype=np.int32)
+    dmt = np.zeros((ndm, nt), dtype=np.int32)
+    _check(lib().orc_cutout(_ptr(x), x.shape[0], x.shape[1], fch1, foff, tsamp, dm0, ddm, ndm, ts, tbin, nt, nf, _ptr(dds),
+                            _ptr(dmt)), "cutout")
+    return dds, dmt
+
+
+def delta_dm(width_s: float, nu_mhz: float, bw_mhz: float, snr_ratio: float = 0.1, constant: float = 1382.0) -> float:
+    """Eq. 4: half-width of the DM range over which the S/N drops to snr_ratio of its peak."""
+    return float(lib().orc_delta_dm(width_s, 1.0 / snr_ratio, nu_mhz, bw_mhz, constant))
 
 
 # ---- whole path over a plan (one beam) ----------------------------------------------------------------

@@ -377,4 +377,48 @@ int orc_peak_filter(int64_t n, const int32_t* beam, const int32_t* trial, const 
     return 0;
 }
 
+/* ------------------------------------------------------------------------------------------------
+ * H. Candidate cut-outs -- PAPER.md:116 ("candies ... extracts two features from this data: the dedispersed dynamic
+ * spectrum, and the DM transform.  The former is created at the candidate's detected DM, while the latter is created at
+ * a narrow DM range centred around that DM"), Eq. 4 for the half-width of that range.  Reading H: integers,
+ * no normalisation; time bins of tbin raw samples, nt of them, the window starting at raw sample ts (may lie partly
+ * outside the data: samples outside contribute 0); nf frequency bands of nchan/nf adjacent channels;
+ *   dds[f][j] = sum_{c in band f} sum_{m<tbin} x[c][ts + j*tbin + m + delay(dm0, c)]
+ *   dmt[i][j] = sum_c            sum_{m<tbin} x[c][ts + j*tbin + m + delay(DM_i, c)],  DM_i = (dm0 - ddm) + i*step,
+ *   step = (2*ddm)/(ndm-1) (ndm > 1), delays at full time resolution as in section A.
+ * ---------------------------------------------------------------------------------------------- */
+int orc_cutout(const uint8_t* x /* [nchan][nsamp] */, int32_t nchan, int64_t nsamp, double fch1, double foff, double tsamp,
+               double dm0, double ddm, int32_t ndm, int64_t ts, int32_t tbin, int32_t nt, int32_t nf,
+               int32_t* dds /* [nf][nt] */, int32_t* dmt /* [ndm][nt] */) {
+    if (!x || !dds || !dmt || nchan < 1 || ndm < 1 || tbin < 1 || nt < 1 || nf < 1 || nchan % nf != 0) return -1;
+    std::vector<int32_t> d0((size_t)nchan), di((size_t)nchan);
+    if (orc_delay_table(fch1, foff, nchan, tsamp, dm0, 1.0, 1, 1, d0.data()) != 0) return -1;
+    const int32_t per = nchan / nf;
+    auto at = [&](int32_t c, int64_t s) -> int32_t { return (s < 0 || s >= nsamp) ? 0 : (int32_t)x[(size_t)c * nsamp + s]; };
+    for (int32_t f = 0; f < nf; ++f)
+        for (int32_t j = 0; j < nt; ++j) {
+            int32_t acc = 0;
+            for (int32_t c = f * per; c < (f + 1) * per; ++c)
+                for (int32_t m = 0; m < tbin; ++m) acc += at(c, ts + (int64_t)j * tbin + m + d0[c]);
+            dds[(size_t)f * nt + j] = acc;
+        }
+    const double step = ndm > 1 ? (2.0 * ddm) / (double)(ndm - 1) : 0.0;
+    for (int32_t i = 0; i < ndm; ++i) {
+        if (orc_delay_table(fch1, foff, nchan, tsamp, (dm0 - ddm) + (double)i * step, 1.0, 1, 1, di.data()) != 0) return -1;
+        for (int32_t j = 0; j < nt; ++j) {
+            int32_t acc = 0;
+            for (int32_t c = 0; c < nchan; ++c)
+                for (int32_t m = 0; m < tbin; ++m) acc += at(c, ts + (int64_t)j * tbin + m + di[c]);
+            dmt[(size_t)i * nt + j] = acc;
+        }
+    }
+    return 0;
+}
+
+/* Eq. 4 (clean form at PAPER.md:244): dDM = sqrt(pi)/C * W_s * (S/S(dDM)) * nu_MHz^3 / dnu_MHz with the
+ * printed C = 1382.  (The derivation's own first line, from Eq. A3, gives C = 13820: DESIGN.md reading H.) */
+double orc_delta_dm(double width_s, double snr_ratio_inverse, double nu_mhz, double bw_mhz, double constant) {
+    return std::sqrt(3.14159265358979323846) / constant * width_s * snr_ratio_inverse * (nu_mhz * nu_mhz * nu_mhz) / bw_mhz;
+}
+
 }  // extern "C"
