@@ -265,6 +265,23 @@ typedef struct {
 int spt_sift(spt_plan* plan, const spt_candidate* h_in /*HOST*/, int64_t n, int32_t nbeam, const spt_sift_params* params,
              spt_candidate* h_out /*HOST*/, int64_t cap, int64_t* nwritten, int64_t* stage_counts /*HOST[3]*/);
 
+/* -------------------------------------------------------------------------------------------------------
+ * spt_cutout -- the two classifier features of one candidate ("the dedispersed dynamic spectrum, and the DM
+ * transform.  The former is created at the candidate's detected DM, while the latter is created at a narrow DM range
+ * centred around that DM"; reading H), as exact integers:
+ *   d_dds[f][j] = sum_{c in band f} sum_{m<tbin} x[c][ts + j*tbin + m + delay(dm0, c)]       int32 [nf][nt]
+ *   d_dmt[i][j] = sum_c            sum_{m<tbin} x[c][ts + j*tbin + m + delay(DM_i, c)]        int32 [ndm][nt]
+ *   DM_i = (dm0 - ddm) + i*(2*ddm)/(ndm-1); delay() as in spt_plan_create at full time resolution; band f = channels
+ *   [f*nchan/nf, (f+1)*nchan/nf) (nf must divide nchan); samples outside [0, nsamp) count as 0 (ts may be negative).
+ * d_fb: DEVICE uint8 [nchan][nsamp] of ONE beam.  Needs no plan.  Enqueues on cuda_stream.
+ * spt_delta_dm: Eq. 4: sqrt(pi)/1382 * width_s * (1/snr_ratio) * nu_mhz^3 / bw_mhz -- the half-width of
+ *   the DM range at which the S/N has dropped to snr_ratio (candies' default 0.1) of its peak.
+ * ----------------------------------------------------------------------------------------------------- */
+int spt_cutout(const uint8_t* d_fb /*DEVICE*/, int32_t nchan, int64_t nsamp, double fch1_mhz, double foff_mhz, double tsamp_s,
+               double dm0, double ddm, int32_t ndm, int64_t ts, int32_t tbin, int32_t nt, int32_t nf,
+               int32_t* d_dds /*DEVICE*/, int32_t* d_dmt /*DEVICE*/, void* cuda_stream);
+double spt_delta_dm(double width_s, double snr_ratio, double nu_mhz, double bw_mhz);
+
 /* With option "profile" = 1: device time (ms) of each kernel launched by the LAST spt_dedisperse and the LAST
  * spt_single_pulse_search, in launch order; kinds: 1 = decimate, 2 = dedisperse, 3 = single-pulse search; `range` is the
  * DM range the launch served (-1 for the search).  Synchronises.  Arrays (HOST) hold `cap` entries; n = entries written. */

@@ -68,6 +68,8 @@ SYMBOLS = {
     "spt_segment_info": (ctypes.c_int, [_vp, _P(_i64), _P(_i64), _P(_i64)]),
     "spt_segment_search": (ctypes.c_int, [_vp, _vp, _i32, _i64, _f32, _vp]),
     "spt_segment_push": (ctypes.c_int, [_vp, _vp, _i32, _i64, _i32, _vp, _vp]),
+    "spt_cutout": (ctypes.c_int, [_vp, _i32, _i64, _f64, _f64, _f64, _f64, _f64, _i32, _i64, _i32, _i32, _i32, _vp, _vp, _vp]),
+    "spt_delta_dm": (_f64, [_f64, _f64, _f64, _f64]),
     "spt_sift": (ctypes.c_int, [_vp, _vp, _i64, _i32, _P(spt_sift_params), _vp, _i64, _P(_i64), _P(_i64)]),
     "spt_stream_push": (ctypes.c_int, [_vp, _vp, _i32, _f32]),
     "spt_stream_pop": (ctypes.c_int, [_vp, _P(_i64), _P(_i32)]),
@@ -345,6 +347,22 @@ def _host_ptr_and_beams(h_fb, nchan, nsamp):
         shape = (1,) + tuple(shape)
     assert tuple(shape[1:]) == (nchan, nsamp)
     return ptr, shape[0]
+
+
+def cutout(d_fb, fch1: float, foff: float, tsamp: float, dm0: float, ddm: float, ndm: int, ts: int, tbin: int, nt: int, nf: int,
+           stream=None):
+    """(dedispersed dynamic spectrum [nf][nt], DM transform [ndm][nt]) of one candidate from a CUDA uint8 [nchan][nsamp] beam."""
+    import torch
+    nchan, nsamp = d_fb.shape
+    dds = torch.empty((nf, nt), dtype=torch.int32, device=d_fb.device)
+    dmt = torch.empty((ndm, nt), dtype=torch.int32, device=d_fb.device)
+    _check(lib().spt_cutout(_dev_ptr(d_fb), nchan, nsamp, fch1, foff, tsamp, dm0, ddm, ndm, ts, tbin, nt, nf, _dev_ptr(dds),
+                            _dev_ptr(dmt), _stream_ptr(stream)), "spt_cutout")
+    return dds, dmt
+
+
+def delta_dm(width_s: float, nu_mhz: float, bw_mhz: float, snr_ratio: float = 0.1) -> float:
+    return float(lib().spt_delta_dm(width_s, snr_ratio, nu_mhz, bw_mhz))
 
 
 def corner_turn(d_in, flip: bool = False, stream=None):

@@ -2,6 +2,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <new>
@@ -1035,6 +1036,29 @@ int spt_sift(spt_plan* plan, const spt_candidate* h_in, int64_t n, int32_t nbeam
     }
     if (nwritten) *nwritten = w;
     return SPT_OK;
+}
+
+int spt_cutout(const uint8_t* d_fb, int32_t nchan, int64_t nsamp, double fch1_mhz, double foff_mhz, double tsamp_s, double dm0,
+               double ddm, int32_t ndm, int64_t ts, int32_t tbin, int32_t nt, int32_t nf, int32_t* d_dds, int32_t* d_dmt,
+               void* cuda_stream) {
+    if (!d_fb || !d_dds || !d_dmt || nchan < 1 || nsamp < 1 || ndm < 1 || tbin < 1 || nt < 1 || nf < 1 || nchan % nf != 0 ||
+        !(tsamp_s > 0.0) || !(fch1_mhz > 0.0) || !(dm0 >= 0.0) || !(ddm >= 0.0))
+        return SPT_ERR_INVALID;
+    if (!(foff_mhz < 0.0)) return SPT_ERR_UNSUPPORTED;
+    if (!(fch1_mhz + (double)(nchan - 1) * foff_mhz > 0.0)) return SPT_ERR_INVALID;
+    if ((double)nchan * 255.0 * tbin >= 2147483648.0 || ndm + nf > 65535) return SPT_ERR_UNSUPPORTED;
+    if (launch_cutout(d_fb, nchan, nsamp, fch1_mhz, foff_mhz, tsamp_s, dm0, ddm, ndm, ts, tbin, nt, nf, d_dds, d_dmt,
+                      (cudaStream_t)cuda_stream) != 0) {
+        g_last_error = "spt_cutout: launch failed";
+        cudaGetLastError();
+        return SPT_ERR_CUDA;
+    }
+    return SPT_OK;
+}
+
+double spt_delta_dm(double width_s, double snr_ratio, double nu_mhz, double bw_mhz) {
+    // Eq. 4 as printed; reading H notes that the derivation's own first line implies 13820
+    return std::sqrt(3.14159265358979323846) / 1382.0 * width_s * (1.0 / snr_ratio) * (nu_mhz * nu_mhz * nu_mhz) / bw_mhz;
 }
 
 int spt_plan_kernel_times(spt_plan* plan, int32_t cap, int32_t* kind, int32_t* range, double* ms, int32_t* n) {

@@ -85,6 +85,10 @@ struct SiftArgs {                   // all arrays DEVICE, n entries sorted by (b
 };
 void launch_sift(const SiftArgs& a, cudaStream_t st);
 
+int launch_cutout(const uint8_t* x, int32_t nchan, int64_t nsamp, double fch1, double foff, double tsamp, double dm0,
+                  double ddm, int32_t ndm, int64_t ts, int32_t tbin, int32_t nt, int32_t nf, int32_t* dds, int32_t* dmt,
+                  cudaStream_t st);
+
 int run_probe(int kind, int reps, double* warp_instr_per_s, double* elapsed_ms);
 
 }  // namespace spt
