@@ -206,6 +206,9 @@ __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
     asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(addr));
     return v;
 }
+__device__ __forceinline__ void lds64(uint32_t addr, uint32_t& a, uint32_t& b) {
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "r"(addr));
+}
 __device__ __forceinline__ void sts128(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w) {
     asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(x), "r"(y), "r"(z), "r"(w) : "memory");
 }
@@ -219,7 +222,7 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
 // The five packed words w_i = y[u0+i] | y[u0+i+kH] << 16, i = 0..4, of one entry (a channel at one of its shifts).
 // addr: shared-memory byte address of the aligned 32-bit word holding the lane's first sample; c1: the entry's second
 // descriptor word (uint8: bits 0-4 = 8 * position of that sample inside the word, bits 8-23 = PRMT selector of sample 4;
-// uint16: bit 0 = position).
+// uint16: bits 0-1 = position inside the 8-byte unit the address points at).
 template <typename T>
 __device__ __forceinline__ void load_entry(uint32_t addr, uint32_t c1, uint32_t (&w)[5]) {
     if (sizeof(T) == 1) {
@@ -235,8 +238,12 @@ __device__ __forceinline__ void load_entry(uint32_t addr, uint32_t c1, uint32_t 
         w[3] = prmt(Lo, Ho, 0x7632u);
         w[4] = prmt(bL, bH, c1 >> 8) & 0x00FF00FFu;                    // sample 4 = byte a0 of the second word
     } else {
-        const uint32_t x0L = lds32(addr), x1L = lds32(addr + 4), x2L = lds32(addr + 8);
-        const uint32_t x0H = lds32(addr + 2 * kH), x1H = lds32(addr + 2 * kH + 4), x2H = lds32(addr + 2 * kH + 8);
+        // two 64-bit loads per half (a lane's samples start on an 8-byte boundary: conflict free), then the five samples
+        // from position c1 = 0..3 of the eight
+        uint32_t x0L, x1L, x2L, x3L, x0H, x1H, x2H, x3H;
+        lds64(addr, x0L, x1L); lds64(addr + 8, x2L, x3L);
+        lds64(addr + 2 * kH, x0H, x1H); lds64(addr + 2 * kH + 8, x2H, x3H);
+        if (c1 & 2u) { x0L = x1L; x1L = x2L; x2L = x3L; x0H = x1H; x1H = x2H; x2H = x3H; }
         const bool odd = (c1 & 1u) != 0u;
         const uint32_t s_even = odd ? 0x7632u : 0x5410u, s_odd = odd ? 0x5410u : 0x7632u;
         w[0] = prmt(x0L, x0H, s_even);

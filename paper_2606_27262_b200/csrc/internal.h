@@ -43,11 +43,11 @@ constexpr int kSmemDataBytes = kSmemBytes - kSmemCtrlBytes - 2 * kBlobBytes;  //
 //   cdesc         per group, kMaxG entries of 2 words (the first nent are real, the rest repeat the first one without
 //                 bit 26), in PREFIX ORDER (most-often-taken delta first; the first ntog have
 //                 a delta that some trial takes); an entry is a channel at one of its shifts: bits 0-17 byte offset
-//                 inside the raw region of the aligned 32-bit word that holds the entry's sample at u = 0, bits 24-25
-//                 position of that sample inside the word, bit 26 = the entry is the channel's smallest shift and adds
+//                 inside the raw region of the aligned 32-bit word (uint16 input: 8-byte unit) that holds the entry's sample
+//                 at u = 0, bits 24-25 position of that sample inside it, bit 26 = the entry is the channel's smallest shift and adds
 //                 it to the base sum.  The entry's delta (sample one later minus sample) moves its channel one later.
 //                 Second word: what the kernel's realignment needs (uint8: bits 0-4 funnel-shift amount, bits 8-23 PRMT
-//                 selector of the fifth sample; uint16: bit 0 = odd position).
+//                 selector of the fifth sample; uint16: bits 0-1 = that position).
 //   vdesc         per group: kChainWords chain words, word k <= ntog = offset in the variant region of the variant "base sum
 //                 + deltas of the first k entries" (0xffffffff: no trial uses it); then ncorr x { offset, mask } for the
 //                 variants off the chain: all ntog deltas minus those in mask.  Headers, cdesc and vdesc are 16-byte

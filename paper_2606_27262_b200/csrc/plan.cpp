@@ -313,8 +313,9 @@ int build_tiling(Plan& p) {
                         const RowDesc& r = g.rows[en.j];
                         const int32_t e0 = g.dmin + g.smin[en.j] + en.level - r.astart;   // element of the entry's u = 0 sample
                         const uint32_t byte = (uint32_t)(rbase + r.soff + e0 * es);
-                        const uint32_t a0 = es == 1 ? (byte & 3u) : (uint32_t)(e0 & 1);
-                        cdesc.push_back((byte & ~3u) | (a0 << 24) | (en.addbase ? kEntryAddBase : 0u));
+                        // uint8: aligned 32-bit word + byte position; uint16: aligned 8-byte unit + sample position in it
+                        const uint32_t a0 = es == 1 ? (byte & 3u) : ((byte >> 1) & 3u);
+                        cdesc.push_back((es == 1 ? (byte & ~3u) : (byte & ~7u)) | (a0 << 24) | (en.addbase ? kEntryAddBase : 0u));
                         // second word, ready for the kernel: uint8: funnel-shift amount and the PRMT selector of sample 4
                         cdesc.push_back(es == 1 ? (a0 * 8u) | ((a0 * 0x1111u + 0x4400u) << 8) : a0);
                     }
