@@ -193,7 +193,10 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
         // ---- pass 2, fast path ---------------------------------------------------------------------------------------
         const int m = sh.m;
         const int nw_eff = sh.nw_eff;
-        const int adv = (kSegLoad - halo) & ~3;                 // outputs per segment (launch_sps: wmax <= kXSeg - 32)
+        // outputs per segment (launch_sps: wmax <= kXSeg - 32): whole sub-blocks of kSpsThreads * kEpt start positions when
+        // the halo leaves room for them, so that no slot of the unrolled test below idles
+        const int room = kSegLoad - halo;
+        const int adv = room >= kSpsThreads * kEpt ? room / (kSpsThreads * kEpt) * (kSpsThreads * kEpt) : (room & ~3);
         for (int tb = 0; tb < nbest; tb += adv) {
             __syncthreads();                                    // the previous segment's readers are done
             // stage x - m: warp `warp` owns elements [warp*640, +640) of the segment; zero beyond N
@@ -240,19 +243,26 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
             // S'_w[i] = c[kCOff + i + w] - c[kCOff + i]   (i relative to the segment)
             const int nthis = min(adv, nbest - tb);
             for (int i0 = 0; i0 < nthis; i0 += kSpsThreads * kEpt) {
-                int idx[kEpt], mxv[kEpt];
-                uint32_t c0[kEpt];
+                // per slot: shared-memory address of c[i] and -c[i]; per (slot, width): one load, one add, one add-max
+                uint32_t adr[kEpt];
+                int nc0[kEpt], mxv[kEpt];
+                const uint32_t cbase = (uint32_t)__cvta_generic_to_shared(&sh.c[kCOff]);
 #pragma unroll
                 for (int e = 0; e < kEpt; ++e) {
-                    idx[e] = min(i0 + e * kSpsThreads + tid, nthis - 1);    // clamped: out-of-range slots repeat the last one
-                    c0[e] = sh.c[kCOff + idx[e]];
+                    const int idx = min(i0 + e * kSpsThreads + tid, nthis - 1);   // clamped: out-of-range slots repeat the last one
+                    adr[e] = cbase + 4u * (uint32_t)idx;
+                    nc0[e] = -(int)sh.c[kCOff + idx];
                     mxv[e] = (int)0x80000000;
                 }
                 for (int k = 0; k < nw_eff; ++k) {
-                    const int w = a.widths[k], nT = sh.negT[k];
+                    const uint32_t wb = 4u * (uint32_t)a.widths[k];
+                    const int nT = sh.negT[k];
 #pragma unroll
-                    for (int e = 0; e < kEpt; ++e)
-                        mxv[e] = max(mxv[e], (int)(sh.c[kCOff + idx[e] + w] - c0[e]) + nT);
+                    for (int e = 0; e < kEpt; ++e) {
+                        uint32_t v;
+                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(adr[e] + wb));
+                        mxv[e] = max(mxv[e], (int)v + (nc0[e] + nT));
+                    }
                 }
 #pragma unroll
                 for (int e = 0; e < kEpt; ++e) {
