@@ -147,19 +147,22 @@ template void launch_dedisp_naive<uint16_t>(const uint16_t*, int64_t, int64_t, c
 // ---------------------------------------------------------------------------------------------------------------
 // a3, the product kernel.  One block = DT trials x TT = 2*kH output samples of one beam; 8 warps, TPW = DT/8 trials
 // per warp, two blocks per SM; lane l of a warp owns the packed words q = l + 32*j (j < kH/32) of each of its
-// trials: the low 16 bits of word q accumulate output t0+q, the high 16 bits output t0+kH+q.  Because both halves
-// of a word move together, a read at ANY sample offset is one aligned 32-bit shared-memory load.
+// trials: the low 16 bits of word q accumulate output first+q, the high 16 bits output first+kH+q, where
+// first = t0 - skew[trial] (every trial of the tile has its own window start, which narrows what the tile reads).
+// Because both halves of a word move together, a read at ANY sample offset is one aligned 32-bit shared-memory load.
 //
 // Per stage (a run of channel groups that fits shared memory; tables built by plan.cpp):
-//   T  TMA    : one elected warp issues cp.async.bulk copies of the stage's table blob and raw channel rows
-//               (global -> shared, completion on an mbarrier); they land while the previous stage is gathered
+//   T  TMA    : every warp issues its share of the cp.async.bulk copies of the stage's raw channel rows, warp 0 also the
+//               table blob and the next stage's descriptors (global -> shared, completion on one mbarrier with one
+//               arrive.expect_tx per warp); they land while the previous stage is gathered
 //   B  presum : P_r[u] = sum_j y[c0+j][t0 + dmin + u + s_j + tau^r_j] | (same at +kH) << 16 for every variant r of
 //               every group.  A lane makes 4 consecutive u from aligned 32-bit words of the raw rows: per channel the
 //               five samples u..u+4 as packed words w0..w4, base += w_i, delta_i = w_{i+1} - w_i (the alternate shift
 //               is one sample later), then walks the prefix chain: variant k = base + delta of the first k channels.
 //   C  gather : acc[d][q] += P_{r(d)}[q + b(d)]       one LDS.32 + one add = 2*G algorithmic adds
-//   F  flush  : before a lane could exceed 65535 (every floor(65535 / largest sample of the launch) channels, at worst
-//               every 257/decim) the 16-bit lanes are widened into the int32 DM transform (first time a store, then RED).
+//   F  flush  : a lane sums (sample - smallest sample of the launch); before it could exceed 65535 (every
+//               floor(65535 / (largest - smallest sample)) channels, at worst every 257/decim) the 16-bit lanes are widened
+//               into the int32 DM transform, the floor added back (first time a store, then RED).
 // ---------------------------------------------------------------------------------------------------------------
 struct TiledArgs {
     const void* in;            // series of beam 0
