@@ -125,6 +125,9 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out);
  *   d_dmt: DEVICE, int32, at least nbeam*dmt_elems_per_beam elements, 128-byte aligned; beam b's row d starts at
  *          b*dmt_elems_per_beam + offset[d].  Every element t < nout[d] of every row is written.
  * Enqueues on cuda_stream and returns.
+ * SPT_ERR_UNSUPPORTED (from the first call, when the kernel tables are built): a tile of 64 consecutive trials whose
+ * delays at one channel spread over more samples than the shared-memory tile holds (DM steps of several pc cm^-3 over a
+ * wide, low band).  Options "dm_tile" = 32 halves the spread; "dedisp_kernel" = 1 takes any plan (slowly).
  * ----------------------------------------------------------------------------------------------------- */
 int spt_dedisperse(spt_plan* plan, const uint8_t* d_fb, int32_t nbeam, int32_t* d_dmt, void* cuda_stream);
 

@@ -577,7 +577,8 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
 }
 
 int spt_dedisperse(spt_plan* plan, const uint8_t* d_fb, int32_t nbeam, int32_t* d_dmt, void* cuda_stream) {
-    if (!plan || !d_fb || !d_dmt || nbeam < 1) return SPT_ERR_INVALID;
+    if (!plan || !d_fb || nbeam < 1) return SPT_ERR_INVALID;
+    if (!d_dmt && plan->p.dmt_elems > 0) return SPT_ERR_INVALID;   // a plan whose trials are all empty has no output
     if (nbeam > plan->p.max_beams) return SPT_ERR_INVALID;
     if ((reinterpret_cast<uintptr_t>(d_dmt) & 127) != 0) return SPT_ERR_INVALID;
     int rc;
@@ -627,7 +628,8 @@ int spt_decimated_read(spt_plan* plan, int32_t range, int32_t beam, uint16_t* ho
 }
 
 int spt_single_pulse_search(spt_plan* plan, const int32_t* d_dmt, int32_t nbeam, float threshold, void* cuda_stream) {
-    if (!plan || !d_dmt || nbeam < 1 || nbeam > plan->p.max_beams || !(threshold == threshold)) return SPT_ERR_INVALID;
+    if (!plan || nbeam < 1 || nbeam > plan->p.max_beams || !(threshold == threshold)) return SPT_ERR_INVALID;
+    if (!d_dmt && plan->p.dmt_elems > 0) return SPT_ERR_INVALID;
     int rc;
     try {
         rc = ensure_device(&plan->p);

@@ -282,6 +282,29 @@ def test_stream_pipeline_matches_search_host(cuda, api, synth):
             plan.stream_push(batches[i + 2], w.threshold)            # reuses the buffers of the batch just read out
 
 
+def test_plan_with_no_valid_output_at_all(cuda, api):
+    """Every sweep longer than the data: nothing to compute, nothing found, no error."""
+    w = Shape(500.0, -400.0 / 17, 17, 2314, [(32.6, 0.05, 93, 8), (37.3, 1.0, 88, 8)], [1, 3, 100], 5.0)
+    plan = api.Plan(w.fch1, w.foff, w.nchan, w.tsamp, w.nsamp, w.ranges, w.widths)
+    assert plan.dmt_elems_per_beam == 0
+    fb = cuda.zeros((1, w.nchan, w.nsamp), dtype=cuda.uint8, device="cuda")
+    d_dmt = plan.dedisperse(fb)
+    plan.single_pulse_search(d_dmt, w.threshold)
+    assert plan.candidates_count() == (0, False)
+
+
+def test_wide_delay_spread_is_refused_not_miscomputed(cuda, api, orc):
+    """DM steps of 3 pc cm^-3 over a band that reaches down to 100 MHz: the 64-trial tile does not fit shared memory ->
+    UNSUPPORTED; the cross-check kernel takes the same plan."""
+    w = Shape(500.0, -400.0 / 1024, 1024, 17003, [(4.4, 0.5, 125, 1), (66.9, 3.0, 139, 1)], [2, 100], 5.0)
+    fb = np.random.default_rng(0).integers(0, 256, size=(1, w.nchan, w.nsamp), dtype=np.uint8)
+    with pytest.raises(api.SptError) as e:
+        run_gpu(cuda, api, w, fb, search=False)
+    assert e.value.code == api.SPT_ERR_UNSUPPORTED
+    plan, dmt, _ = run_gpu(cuda, api, w, fb, options={"dedisp_kernel": 1}, search=False)
+    check_dmt_against_oracle(plan, dmt, oracle_path(orc, w, fb[0], search=False))
+
+
 def test_candidate_overflow_is_reported(cuda, api, synth):
     w = synth.workload(1)
     fb = synth.generate(w)
