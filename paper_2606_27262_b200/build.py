@@ -6,6 +6,7 @@ nvcc cross-compiles without a GPU, so this also is the "does it build" check on 
 """
 from __future__ import annotations
 
+import fcntl
 import os
 import subprocess
 import sys
@@ -31,14 +32,27 @@ def _stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not _stale():
         return LIB
-    cmd = [NVCC, *FLAGS, "-o", LIB, *[os.path.join(CSRC, s) for s in SOURCES]]
-    r = subprocess.run(cmd, capture_output=True, text=True)
-    if verbose or r.returncode != 0:
-        sys.stderr.write(r.stdout + r.stderr)
-    if r.returncode != 0:
-        raise RuntimeError("nvcc failed building libspt.so")
-    with open(os.path.join(HERE, "build.log"), "w") as f:
-        f.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
+    # several ranks of one node may get here together (torchrun): one builds, the others wait on the lock and find the
+    # library fresh; the library appears under its name only when complete (rename)
+    with open(os.path.join(HERE, ".build.lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            if not force and not _stale():
+                return LIB
+            tmp = LIB + ".tmp.%d" % os.getpid()
+            cmd = [NVCC, *FLAGS, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
+            r = subprocess.run(cmd, capture_output=True, text=True)
+            if verbose or r.returncode != 0:
+                sys.stderr.write(r.stdout + r.stderr)
+            if r.returncode != 0:
+                if os.path.exists(tmp):
+                    os.unlink(tmp)
+                raise RuntimeError("nvcc failed building libspt.so")
+            os.replace(tmp, LIB)
+            with open(os.path.join(HERE, "build.log"), "w") as f:
+                f.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
     return LIB
 
 
