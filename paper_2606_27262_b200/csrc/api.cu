@@ -244,23 +244,10 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
         SPT_CUDA(cudaMemsetAsync(d->maxval + 2 * i, 0, 4, st));
         SPT_CUDA(cudaMemsetAsync(d->maxval + 2 * i + 1, 0xff, 4, st));
     }
-    for (size_t i = 0; i < p->ranges.size(); ++i)
-        if (p->ranges[i].decim == 1 && p->ranges[i].max_nout > 0) {
-            launch_max_u8(in, (int64_t)nbeam * p->nchan * in_stride, d->maxval + 2 * i, st);
-            p->launches++;
-        }
-    // a2: decimated series of every range that needs one
-    for (size_t i = 0; i < p->ranges.size(); ++i) {
-        const RangePlan& rp = p->ranges[i];
-        if (rp.decim == 1 || rp.nsamp_k <= 0) continue;
-        ScopedTimer tm(p, st, 0, 1, (int)i);
-        launch_decimate(in, in_stride, (int64_t)p->nchan * in_stride, d->r[i].series, rp.stride_k,
-                        (int64_t)p->nchan * rp.stride_k, p->nchan, nbeam, rp.nsamp_k, rp.decim, st);
-        launch_max_u16(d->r[i].series, (int64_t)nbeam * p->nchan * rp.stride_k, d->maxval + 2 * i, st);
-        p->launches += 2;
-    }
-    // a3: DM transform, range by range.  Unless launches are being timed one by one, the ranges after the first go to
-    // side streams: they are independent, and a later grid then fills the last, partly empty wave of the grid before it.
+    // Every range has a pre-pass (the bounds of a raw range, or its decimated series and their bounds: a2) and its
+    // dedispersion (a3).  Unless launches are being timed one by one, the ranges after the first run on side streams:
+    // they are independent, their HBM-bound pre-passes run beside the first range's dedispersion, and their
+    // dedispersion grids fill the last, partly empty wave of the grid launched before them.
     const bool overlap = !p->opt_profile && p->ranges.size() > 1;
     if (overlap) {
         if (!d->fork) {
@@ -270,16 +257,39 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
                 SPT_CUDA(cudaEventCreateWithFlags(&d->join[i], cudaEventDisableTiming));
             }
         }
-        SPT_CUDA(cudaEventRecord(d->fork, st));                  // after the decimation and the min/max passes
+        SPT_CUDA(cudaEventRecord(d->fork, st));                  // after the input staging and the resets above
         for (int i = 0; i < 2; ++i) SPT_CUDA(cudaStreamWaitEvent(d->side[i], d->fork, 0));
     }
     cudaStream_t const caller = st;
     bool used_side[2] = {false, false};
+    auto stream_of = [&](size_t i) {
+        if (overlap && i > 0) { used_side[(i - 1) & 1] = true; return d->side[(i - 1) & 1]; }
+        return caller;
+    };
+    auto prepass = [&](size_t i) -> int {
+        const RangePlan& rp = p->ranges[i];
+        cudaStream_t s = stream_of(i);
+        if (rp.decim == 1) {
+            if (rp.max_nout <= 0) return SPT_OK;
+            launch_max_u8(in, (int64_t)nbeam * p->nchan * in_stride, d->maxval + 2 * i, s);
+            p->launches++;
+            return SPT_OK;
+        }
+        if (rp.nsamp_k <= 0) return SPT_OK;
+        ScopedTimer tm(p, s, 0, 1, (int)i);
+        launch_decimate(in, in_stride, (int64_t)p->nchan * in_stride, d->r[i].series, rp.stride_k,
+                        (int64_t)p->nchan * rp.stride_k, p->nchan, nbeam, rp.nsamp_k, rp.decim, s);
+        launch_max_u16(d->r[i].series, (int64_t)nbeam * p->nchan * rp.stride_k, d->maxval + 2 * i, s);
+        p->launches += 2;
+        return SPT_OK;
+    };
+    // launch order: the side streams' pre-passes, then the first range (pre-pass and grid), then the other grids
+    for (size_t i = 1; i < p->ranges.size(); ++i) prepass(i);
+    if (!p->ranges.empty()) prepass(0);
     for (size_t i = 0; i < p->ranges.size(); ++i) {
         const RangePlan& rp = p->ranges[i];
         if (rp.max_nout <= 0) continue;
-        if (overlap && i > 0) { st = d->side[(i - 1) & 1]; used_side[(i - 1) & 1] = true; }
-        else st = caller;
+        st = stream_of(i);
         const RangeDev& rd = d->r[i];
         const bool u16 = rp.decim > 1;
         const void* src = u16 ? (const void*)rd.series : (const void*)in;
