@@ -173,8 +173,11 @@ def run_ours(args, rank, world, local_rank):
     stream = torch.cuda.current_stream()
 
     def step():
-        plan.dedisperse(d_fb, d_dmt, stream)
-        plan.single_pulse_search(d_dmt, w.threshold, stream)
+        if args.two_calls:                  # spt_dedisperse, then spt_single_pulse_search
+            plan.dedisperse(d_fb, d_dmt, stream)
+            plan.single_pulse_search(d_dmt, w.threshold, stream)
+        else:                               # spt_search: the same two steps enqueued by one call
+            plan.search(d_fb, w.threshold, d_dmt, stream)
         return plan.candidates_count()      # a5: stream sync + 8-byte readback
 
     def barrier():
@@ -311,7 +314,9 @@ def run_ours(args, rank, world, local_rank):
                        "parallelism": f"beams sharded over {world} GPU(s), no collective",
                        "l2": "inputs larger than L2 (filterbank %.0f MiB, DM transform %.0f MiB per beam)" %
                              (w.nchan * w.nsamp / 2**20, plan.dmt_elems_per_beam * 4 / 2**20),
-                       "group": args.group or 8, "dm_tile": args.dm_tile or 64},
+                       "group": args.group or 8, "dm_tile": args.dm_tile or 64,
+                       "step_api": "spt_dedisperse + spt_single_pulse_search + spt_candidates_count" if args.two_calls
+                                   else "spt_search + spt_candidates_count"},
             "rtf": rtf, "realtime_beams": rtf, "candidates": ncand, "overflowed": ovf,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h_fb.numel()),
                     "d2h_bytes_per_step": 8, "ms_per_step": 1e3 * e2e_s / steps,
@@ -334,6 +339,7 @@ def main():
     ap.add_argument("--group", type=int, default=0)
     ap.add_argument("--dm-tile", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--two-calls", action="store_true", help="step = spt_dedisperse + spt_single_pulse_search instead of spt_search")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

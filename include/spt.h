@@ -153,6 +153,17 @@ int spt_decimated_read(spt_plan* plan, int32_t range, int32_t beam, uint16_t* ho
 int spt_single_pulse_search(spt_plan* plan, const int32_t* d_dmt /*DEVICE*/, int32_t nbeam, float threshold,
                             void* cuda_stream);
 
+/* -------------------------------------------------------------------------------------------------------
+ * spt_search -- a2 + a3 + a4 in one call: exactly spt_dedisperse(plan, d_fb, nbeam, d_dmt, stream) followed by
+ * spt_single_pulse_search(plan, d_dmt, nbeam, threshold, stream) -- same arguments, same results (DM transform,
+ * decimated series, statistics, candidate list up to its order) -- but enqueued so that a DM range is searched as soon
+ * as its own rows of the DM transform are complete, while later ranges are still being dedispersed.  Work on
+ * cuda_stream after this call sees everything finished.  The host-buffer calls (spt_search_host, spt_stream_push) use
+ * the same schedule.
+ * ----------------------------------------------------------------------------------------------------- */
+int spt_search(spt_plan* plan, const uint8_t* d_fb /*DEVICE*/, int32_t nbeam, int32_t* d_dmt /*DEVICE*/, float threshold,
+               void* cuda_stream);
+
 /* Exact statistics of one (beam, trial) from the last search (synchronises).  n = nout. */
 int spt_trial_stats(spt_plan* plan, int32_t beam, int32_t trial, int64_t* n, int64_t* sum, uint64_t* sumsq);
 /* All of them at once: host arrays [nbeam*ntrials] (beam major), any may be NULL. */

@@ -56,6 +56,7 @@ SYMBOLS = {
     "spt_decimated_stride": (ctypes.c_int, [_vp, _i32, _P(_i64)]),
     "spt_decimated_read": (ctypes.c_int, [_vp, _i32, _i32, _vp]),
     "spt_single_pulse_search": (ctypes.c_int, [_vp, _vp, _i32, _f32, _vp]),
+    "spt_search": (ctypes.c_int, [_vp, _vp, _i32, _vp, _f32, _vp]),
     "spt_trial_stats": (ctypes.c_int, [_vp, _i32, _i32, _P(_i64), _P(_i64), _P(ctypes.c_uint64)]),
     "spt_trial_stats_all": (ctypes.c_int, [_vp, _i32, _vp, _vp]),
     "spt_candidates_count": (ctypes.c_int, [_vp, _P(_i64), _P(_i32)]),
@@ -223,6 +224,20 @@ class Plan:
         nbeam = d_dmt.shape[0] if d_dmt.dim() == 2 else 1
         _check(lib().spt_single_pulse_search(self._h, _dev_ptr(d_dmt), nbeam, float(threshold), _stream_ptr(stream)),
                "spt_single_pulse_search")
+
+    def search(self, d_fb, threshold: float, d_dmt=None, stream=None):
+        """dedisperse + single_pulse_search in one call (spt_search): every DM range is searched as soon as its rows are
+        done.  Returns the DM transform tensor."""
+        import torch
+        if d_fb.dim() == 2:
+            d_fb = d_fb.unsqueeze(0)
+        nbeam = d_fb.shape[0]
+        assert d_fb.dtype == torch.uint8 and tuple(d_fb.shape[1:]) == (self.nchan, self.nsamp)
+        if d_dmt is None:
+            d_dmt = torch.empty((nbeam, self.dmt_elems_per_beam), dtype=torch.int32, device=d_fb.device)
+        _check(lib().spt_search(self._h, _dev_ptr(d_fb), nbeam, _dev_ptr(d_dmt), float(threshold), _stream_ptr(stream)),
+               "spt_search")
+        return d_dmt
 
     def trial_stats(self, beam: int, trial: int):
         n, s, q = ctypes.c_int64(), ctypes.c_int64(), ctypes.c_uint64()

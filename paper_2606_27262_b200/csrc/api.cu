@@ -80,6 +80,7 @@ struct DeviceState {
     // side streams for the DM ranges after the first (their grids fill the tail of the previous range's grid)
     cudaStream_t side[2] = {nullptr, nullptr};
     cudaEvent_t fork = nullptr, join[2] = {nullptr, nullptr};
+    bool side_pending[2] = {false, false};   // side streams left un-joined by do_dedisperse(defer_join) for do_search
     cudaEvent_t wait_event = nullptr;   // when set, read-out calls wait for this event instead of the whole stream
     uint8_t* fb_pad = nullptr;      // aligned copy of an input whose rows are not 16-byte multiples
     int64_t fb_pad_stride = 0;
@@ -220,7 +221,10 @@ static int ensure_device(Plan* p) {
     return rc;
 }
 
-static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d_dmt, cudaStream_t st) {
+// defer_join: leave the side streams un-joined (d->side_pending says which carry work); the caller -- do_search with
+// per_range = true, directly afterwards -- enqueues every range's search behind its dedispersion and joins then.
+static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d_dmt, cudaStream_t st,
+                         bool defer_join = false) {
     DeviceState* d = p->dev;
     const uint8_t* in = d_fb;
     int64_t in_stride = p->nsamp;
@@ -311,22 +315,32 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
         p->launches++;
     }
     st = caller;
-    for (int i = 0; i < 2; ++i)
-        if (used_side[i]) {                                      // the caller's stream continues when every range is done
+    for (int i = 0; i < 2; ++i) {
+        d->side_pending[i] = defer_join && used_side[i];
+        if (used_side[i] && !defer_join) {                       // the caller's stream continues when every range is done
             SPT_CUDA(cudaEventRecord(d->join[i], d->side[i]));
             SPT_CUDA(cudaStreamWaitEvent(st, d->join[i], 0));
         }
+    }
     SPT_CUDA(cudaGetLastError());
     d->last_stream = st;
     d->nbeam_dedisp = nbeam;
     return SPT_OK;
 }
 
+// The counter of the result set is reset on the caller's stream: before do_dedisperse forks when the two are fused.
+static int reset_count(Plan* p, cudaStream_t st, int set) {
+    SPT_CUDA(cudaMemsetAsync(p->dev->bufs[set].count, 0, 8, st));
+    return SPT_OK;
+}
+
+// per_range (only right after do_dedisperse(..., defer_join = true), counter already reset): one launch per DM range on
+// the stream that range was dedispersed on, so a range is searched while later ranges are still being dedispersed.
 static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float threshold, cudaStream_t st, int set = 0,
-                     bool windowed = false) {
+                     bool windowed = false, bool per_range = false) {
     DeviceState* d = p->dev;
     const DeviceState::SearchBufs& bf = d->bufs[set];
-    SPT_CUDA(cudaMemsetAsync(bf.count, 0, 8, st));
+    if (!per_range) { const int rc0 = reset_count(p, st, set); if (rc0 != SPT_OK) return rc0; }
     SpsArgs a{};
     a.dmt = d_dmt;
     a.beam_stride = p->dmt_elems;
@@ -344,11 +358,28 @@ static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float thresho
     a.win_len = windowed ? d->win_len : nullptr;
     a.win_starts = windowed ? d->win_starts : nullptr;
     timed_clear(d, 1);
-    {
+    if (per_range && (d->side_pending[0] || d->side_pending[1])) {
+        for (size_t i = 0; i < p->ranges.size(); ++i) {
+            const RangePlan& rp = p->ranges[i];
+            cudaStream_t s = (i > 0 && d->side_pending[(i - 1) & 1]) ? d->side[(i - 1) & 1] : st;
+            a.trial0 = rp.trial0;
+            a.nlaunch = rp.ndm;
+            launch_sps(a, nbeam, s);
+            p->launches++;
+        }
+        for (int i = 0; i < 2; ++i)
+            if (d->side_pending[i]) {
+                SPT_CUDA(cudaEventRecord(d->join[i], d->side[i]));
+                SPT_CUDA(cudaStreamWaitEvent(st, d->join[i], 0));
+                d->side_pending[i] = false;
+            }
+    } else {
+        a.trial0 = 0;
+        a.nlaunch = p->ntrials;
         ScopedTimer tm(p, st, 1, 3, -1);
         launch_sps(a, nbeam, st);
+        p->launches++;
     }
-    p->launches++;
     SPT_CUDA(cudaGetLastError());
     d->last_stream = st;
     d->nbeam_search = nbeam;
@@ -357,6 +388,14 @@ static int do_search(Plan* p, const int32_t* d_dmt, int32_t nbeam, float thresho
     d->wait_event = nullptr;
     d->peaks_valid = false;
     return SPT_OK;
+}
+
+// a2-a4 in one go: every range's search follows its own dedispersion on that range's stream.
+static int do_path(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d_dmt, float threshold, cudaStream_t st, int set) {
+    int rc;
+    if ((rc = reset_count(p, st, set)) != SPT_OK) return rc;
+    if ((rc = do_dedisperse(p, d_fb, nbeam, d_dmt, st, true)) != SPT_OK) return rc;
+    return do_search(p, d_dmt, nbeam, threshold, st, set, false, true);
 }
 
 // Read-out calls wait for the results they look at: the whole stream of the last plain call, or the completion event of the
@@ -650,6 +689,21 @@ int spt_single_pulse_search(spt_plan* plan, const int32_t* d_dmt, int32_t nbeam,
     return do_search(&plan->p, d_dmt, nbeam, threshold, (cudaStream_t)cuda_stream);
 }
 
+int spt_search(spt_plan* plan, const uint8_t* d_fb, int32_t nbeam, int32_t* d_dmt, float threshold, void* cuda_stream) {
+    if (!plan || !d_fb || nbeam < 1 || !(threshold == threshold)) return SPT_ERR_INVALID;
+    if (!d_dmt && plan->p.dmt_elems > 0) return SPT_ERR_INVALID;
+    if (nbeam > plan->p.max_beams) return SPT_ERR_INVALID;
+    if ((reinterpret_cast<uintptr_t>(d_dmt) & 127) != 0) return SPT_ERR_INVALID;
+    int rc;
+    try {
+        rc = ensure_device(&plan->p);
+    } catch (const std::bad_alloc&) {
+        rc = SPT_ERR_NOMEM;
+    }
+    if (rc != SPT_OK) return rc;
+    return do_path(&plan->p, d_fb, nbeam, d_dmt, threshold, (cudaStream_t)cuda_stream, 0);
+}
+
 int spt_trial_stats(spt_plan* plan, int32_t beam, int32_t trial, int64_t* n, int64_t* sum, uint64_t* sumsq) {
     if (!plan) return SPT_ERR_INVALID;
     Plan& p = plan->p;
@@ -720,8 +774,7 @@ int spt_search_host(spt_plan* plan, const uint8_t* h_fb, int32_t nbeam, float th
     if (!d->h_dmt) SPT_CUDA(cudaMalloc((void**)&d->h_dmt, (size_t)p.dmt_elems * 4 * p.max_beams + 128));
     cudaStream_t st = d->own_stream;
     SPT_CUDA(cudaMemcpyAsync(d->h_fb, h_fb, fb_bytes * nbeam, cudaMemcpyHostToDevice, st));
-    if ((rc = do_dedisperse(&p, d->h_fb, nbeam, d->h_dmt, st)) != SPT_OK) return rc;
-    if ((rc = do_search(&p, d->h_dmt, nbeam, threshold, st)) != SPT_OK) return rc;
+    if ((rc = do_path(&p, d->h_fb, nbeam, d->h_dmt, threshold, st, 0)) != SPT_OK) return rc;
     if (h_dmt) SPT_CUDA(cudaMemcpyAsync(h_dmt, d->h_dmt, (size_t)p.dmt_elems * 4 * nbeam, cudaMemcpyDeviceToHost, st));
     int64_t total = 0;
     int32_t ovf = 0;
@@ -763,8 +816,7 @@ int spt_stream_push(spt_plan* plan, const uint8_t* h_fb, int32_t nbeam, float th
     const cudaEvent_t keep = d->wait_event;                     // the read-out calls keep looking at the batch popped last
     const int keep_cur = d->cur;
     const bool keep_searched = d->searched;
-    if ((rc = do_dedisperse(&p, sl.fb, nbeam, d->h_dmt, st)) != SPT_OK) return rc;
-    if ((rc = do_search(&p, d->h_dmt, nbeam, threshold, st, k)) != SPT_OK) return rc;
+    if ((rc = do_path(&p, sl.fb, nbeam, d->h_dmt, threshold, st, k)) != SPT_OK) return rc;
     SPT_CUDA(cudaMemcpyAsync(sl.h_count, d->bufs[k].count, 8, cudaMemcpyDeviceToHost, st));
     SPT_CUDA(cudaEventRecord(sl.done, st));
     d->wait_event = keep; d->cur = keep_cur; d->searched = keep_searched;

@@ -30,6 +30,7 @@ struct SpsArgs {
     const int32_t* nout;            // [ntrials] global trial index
     const int64_t* offset;          // [ntrials]
     int32_t ntrials;
+    int32_t trial0, nlaunch;        // the launch searches the trials [trial0, trial0 + nlaunch)
     int32_t nw;
     int32_t widths[kMaxWidths];
     double threshold;

@@ -86,7 +86,7 @@ __device__ __forceinline__ void append(const SpsArgs& a, bool hit, int b, int d,
 template <bool WIN>
 __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
     __shared__ __align__(16) SpsShared sh;
-    const int d = blockIdx.x, b = blockIdx.y;
+    const int d = a.trial0 + blockIdx.x, b = blockIdx.y;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n = a.nout[d];                                  // end of the row
     // Window of the row that is searched: the whole row, or -- for a segment of a stream -- its last win_len[d] samples,
@@ -332,8 +332,8 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
 }
 
 void launch_sps(const SpsArgs& a, int32_t nbeam, cudaStream_t st) {
-    if (a.ntrials <= 0 || nbeam <= 0) return;
-    dim3 grid((unsigned)a.ntrials, (unsigned)nbeam);
+    if (a.nlaunch <= 0 || nbeam <= 0) return;
+    dim3 grid((unsigned)a.nlaunch, (unsigned)nbeam);
     if (a.win_len) sps_kernel<true><<<grid, kSpsThreads, 0, st>>>(a);
     else sps_kernel<false><<<grid, kSpsThreads, 0, st>>>(a);
 }

@@ -243,6 +243,54 @@ def test_search_host_matches_device_path(cuda, api, orc, synth):
     assert plan.launches() >= 2
 
 
+# ---- spt_search: both steps in one call, every range searched behind its own dedispersion --------------------------
+@pytest.mark.parametrize("profile", [0, 1])
+def test_fused_search_call_matches_oracle_and_two_call_path(cuda, api, orc, synth, profile):
+    w = mini3(synth, 12)
+    w.nbeam = 2
+    fb = np.stack([synth.generate(w, beam=b) for b in range(2)])
+    plan = make_plan(api, w, nbeam=2, options={"profile": profile})
+    d_fb = cuda.from_numpy(fb).cuda()
+    d_dmt = cuda.full((2, plan.dmt_elems_per_beam), -7, dtype=cuda.int32, device="cuda")
+    for _ in range(2):                                   # twice: the second pass reuses side streams and events
+        plan.search(d_fb, w.threshold, d_dmt)
+    total, ovf = plan.candidates_count()
+    assert not ovf
+    cands = plan.candidates_read()
+    assert cands.size == total
+    dmt = d_dmt.cpu().numpy()
+    for b in range(2):
+        ref = oracle_path(orc, w, fb[b])
+        check_dmt_against_oracle(plan, dmt, ref, beam=b)
+        check_stats_against_oracle(plan, ref, beam=b, nbeam=2)
+        st = check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold, beam=b)
+        assert st["oracle"] > 100, st
+    # the two separate calls give the same list (up to its order)
+    plan.dedisperse(d_fb, d_dmt)
+    plan.single_pulse_search(d_dmt, w.threshold)
+    two = plan.candidates_read()
+    key = lambda c: np.lexsort((c["t"], c["trial"], c["beam"]))
+    a, b2 = cands[key(cands)], two[key(two)]
+    assert a.size == b2.size
+    for f in ("beam", "trial", "t", "width", "snr"):
+        assert np.array_equal(a[f], b2[f]), f
+
+
+def test_search_host_multirange(cuda, api, orc, synth):
+    w = mini3(synth, 13)
+    fb = synth.generate(w)
+    ref = oracle_path(orc, w, fb)
+    plan = make_plan(api, w)
+    h_dmt = np.full((1, plan.dmt_elems_per_beam), -7, dtype=np.int32)
+    ncand, ovf = plan.search_host(fb[None], w.threshold, h_dmt)
+    assert not ovf
+    check_dmt_against_oracle(plan, h_dmt, ref)
+    check_stats_against_oracle(plan, ref)
+    cands = plan.candidates_read()
+    assert cands.size == ncand
+    check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+
+
 def test_stream_pipeline_matches_search_host(cuda, api, synth):
     """Two batches in flight (H2D of one overlapping the kernels of the other): every pop gives what the synchronous call
     gives for that batch, and the read-out calls follow the popped batch."""
