@@ -159,7 +159,7 @@ def run_ours(args, rank, world, local_rank):
     hv = h_fb.numpy()
     for b, gb in enumerate(shard.beams_of_rank(rank, world, nbeam)):   # every rank brings its own beams (weak scaling)
         synth.generate(w, beam=gb, out=hv[b])
-    cap = {1: 1 << 20, 2: 1 << 24, 3: 1 << 26, 4: 1 << 27, 5: 1 << 29}[w.index]
+    cap = {1: 1 << 20, 2: 1 << 24, 3: 1 << 26, 4: 1 << 27, 5: 1 << 29, 6: 1 << 26}[w.index]
     opts = {"profile": 1}
     if args.group:
         opts["group"] = args.group
@@ -335,7 +335,7 @@ def main():
     ap.add_argument("--steps", type=int, default=30)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5, 6])
     ap.add_argument("--group", type=int, default=0)
     ap.add_argument("--dm-tile", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -146,7 +146,8 @@ def _draw_bursts(rng, n, nchan, nsamp, fch1, foff, tsamp, std, dm_lo, dm_hi, wid
 
 
 def workload(index: int, nsamp: Optional[int] = None, nbeam: Optional[int] = None) -> Workload:
-    """BASELINE.json configs[index-1].  `nsamp`/`nbeam` override the length (reduced-size parity cases)."""
+    """BASELINE.json configs[index-1] (index 6: the Band-5 workload of SURVEY.md NEXT-4).  `nsamp`/`nbeam` override the
+    length (reduced-size parity cases)."""
     if index == 1:
         w = Workload("cfg1-tiny", 1, 1, 64, 4096, 500.0, -3.125, TSAMP, 128.0, 16.0,
                      [(0.0, 1.0, 101, 1)], _pow2_widths(64), 6.0, 0)
@@ -210,7 +211,23 @@ def workload(index: int, nsamp: Optional[int] = None, nbeam: Optional[int] = Non
         for _ in range(200):
             w.spikes.append((int(rng.integers(0, w.nsamp)), int(rng.integers(1, 9)), 30.0))
         return w
-    raise ValueError("config index must be 1..5")
+    if index == 6:
+        # Not a BASELINE.json config: SURVEY.md section 8(f) NEXT-4's second workload, the SPOTLIGHT beam of config 3 observed
+        # in uGMRT Band 5 (1060-1460 MHz), 400 MHz over 4096 channels.  Sweeps are about ten times shorter
+        # (DM 2000: 2666 samples instead of 44996), so tiles see few distinct delays per channel group.
+        w = Workload("cfg6-band5", 6, 1, 4096, 1 << 17, 1460.0, -0.09765625, TSAMP, 128.0, 10.0,
+                     list(_PLAN3), _pow2_widths(512), 7.0, 6)
+        if nsamp:
+            w.nsamp = nsamp
+        rng = np.random.default_rng(w.seed)
+
+        def wfn(r):
+            wms = math.exp(r.uniform(math.log(0.5), math.log(40.0)))
+            return max(1, int(round(wms * 1e-3 / TSAMP)))
+        w.bursts = [_draw_bursts(rng, 20, w.nchan, w.nsamp, w.fch1, w.foff, w.tsamp, w.std, 10.0, 2000.0,
+                                 wfn, 7.0, 50.0)]
+        return w
+    raise ValueError("config index must be 1..6")
 
 
 def generate(w: Workload, beam: int = 0, out: Optional[np.ndarray] = None, nthreads: int = 0) -> np.ndarray:

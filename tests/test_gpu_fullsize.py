@@ -139,6 +139,24 @@ def test_cfg3_full_injected_bursts_found(cuda, api, orc, synth):
     assert peaks.size * 5 < cands.size            # "an order-of-magnitude reduction"
 
 
+def test_cfg6_band5_full(cuda, api, orc, synth):
+    """SURVEY.md NEXT-4's second workload: the same beam in Band 5 (1060-1460 MHz), where sweeps are ~10x shorter, whole DM
+    tiles share their delays at most channels and groups have one or two variants."""
+    w, plan, cands, rep = run_full(cuda, api, orc, synth, 6, cap=1 << 26, trials_per_range=3)
+    _, _, _, nout, _ = plan.trial_table()
+    assert int(nout.min()) > 0 and plan.delays(plan.ntrials - 1)[-1] == 666       # DM 2000 at k = 4: 2666 raw samples
+    found = 0
+    dm, rg, dec, _, _ = plan.trial_table()
+    strong = [b for b in w.bursts[0] if not b.truncated and b.snr >= 20.0 and b.width <= 8]
+    for b in strong:
+        sel = cands[(np.abs(dm[cands["trial"]] - b.dm) <= 5.0)]
+        tt = sel["t"].astype(np.int64) * dec[sel["trial"]]
+        near = sel[np.abs(tt - b.t0) <= 4 * max(b.width, 4)]
+        if near.size and near["snr"].max() >= max(w.threshold, 0.3 * b.snr):
+            found += 1
+    assert found == len(strong), (found, len(strong))
+
+
 def test_cfg5_full_rfi_volume(cuda, api, orc, synth):
     """Candidate-list volume and the widest boxcars (w = 1024)."""
     w, plan, cands, rep = run_full(cuda, api, orc, synth, 5, cap=1 << 29, trials_per_range=1)

@@ -54,6 +54,9 @@ def test_config_shapes_match_baseline_json(synth):
         assert w.tsamp == 1.31072e-3 and w.foff < 0
         assert abs((w.fch1 + w.nchan * w.foff) - {1: 300, 2: 550, 3: 300, 4: 300, 5: 300}[i]) < 1e-9
         assert len(w.bursts) == nb
+    w6 = synth.workload(6)                          # NEXT-4's Band-5 workload: cfg 3's shape at 1060-1460 MHz
+    assert (w6.nbeam, w6.nchan, w6.nsamp, w6.ntrials, w6.fch1) == (1, 4096, 1 << 17, 4501, 1460.0)
+    assert abs(w6.fch1 + w6.nchan * w6.foff - 1060.0) < 1e-9 and len(w6.bursts[0]) == 20
     w3, w4, w5 = synth.workload(3), synth.workload(4), synth.workload(5)
     assert len(w3.bursts[0]) == 20 and all(1 <= b.width <= 31 for b in w3.bursts[0])
     assert all(0 <= len(bl) <= 3 for bl in w4.bursts) and any(b.truncated for bl in w4.bursts for b in bl)
