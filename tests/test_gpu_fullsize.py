@@ -5,7 +5,7 @@ sampled rows)."""
 import numpy as np
 import pytest
 
-from helpers import SNR_TOL, check_plan_against_oracle, make_plan
+from helpers import SNR_TOL, check_dmt_against_oracle, check_plan_against_oracle, check_stats_against_oracle, make_plan
 
 pytestmark = pytest.mark.gpu
 
@@ -137,6 +137,28 @@ def test_cfg3_full_injected_bursts_found(cuda, api, orc, synth):
     key = lambda c: set(zip(c["trial"].tolist(), c["t"].tolist(), c["width"].tolist(), c["snr"].tolist()))
     assert key(peaks) == key(cands[keep])
     assert peaks.size * 5 < cands.size            # "an order-of-magnitude reduction"
+
+
+def test_cfg3_full_every_output(cuda, api, orc, synth):
+    """The bench workload through the call bench.py times (spt_search), EVERY one of its 3.95e8 outputs and every trial's
+    exact statistics against the oracle (about 40 s of the oracle's plain loops on the host cores)."""
+    w = synth.workload(3)
+    fb = synth.generate(w)
+    plan = make_plan(api, w, cand_capacity=1 << 26)
+    d_dmt = plan.search(cuda.from_numpy(fb[None]).cuda(), w.threshold)
+    total, ovf = plan.candidates_count()
+    assert not ovf
+    ref = orc.run_path(fb, w.fch1, w.foff, w.tsamp, w.ranges, w.widths, w.threshold, do_search=False)
+    check_dmt_against_oracle(plan, d_dmt.cpu().numpy(), ref)
+    _, _, _, nout, _ = plan.trial_table()
+    s_all, q_all = plan.trial_stats_all(1)
+    d = 0
+    for rr in ref:                                   # exact integer statistics of all 4501 trials
+        for i in range(len(rr.nout)):
+            row = rr.dmt[rr.rowoff[i]: rr.rowoff[i + 1]].astype(np.int64)
+            assert int(s_all[0, d]) == int(row.sum()) and int(q_all[0, d]) == int((row * row).sum()), d
+            d += 1
+    assert d == plan.ntrials == 4501
 
 
 def test_cfg6_band5_full(cuda, api, orc, synth):
