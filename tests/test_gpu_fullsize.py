@@ -5,7 +5,7 @@ sampled rows)."""
 import numpy as np
 import pytest
 
-from helpers import SNR_TOL, check_dmt_against_oracle, check_plan_against_oracle, check_stats_against_oracle, make_plan
+from helpers import SNR_TOL, check_candidates_against_oracle, check_dmt_against_oracle, check_plan_against_oracle, check_stats_against_oracle, make_plan
 
 pytestmark = pytest.mark.gpu
 
@@ -140,16 +140,21 @@ def test_cfg3_full_injected_bursts_found(cuda, api, orc, synth):
 
 
 def test_cfg3_full_every_output(cuda, api, orc, synth):
-    """The bench workload through the call bench.py times (spt_search), EVERY one of its 3.95e8 outputs and every trial's
-    exact statistics against the oracle (about 40 s of the oracle's plain loops on the host cores)."""
+    """The bench workload through the call bench.py times (spt_search): EVERY one of its 3.95e8 outputs, every trial's
+    exact statistics and the complete candidate list against the oracle (about 40 s of the oracle's plain loops on the
+    host cores)."""
     w = synth.workload(3)
     fb = synth.generate(w)
     plan = make_plan(api, w, cand_capacity=1 << 26)
     d_dmt = plan.search(cuda.from_numpy(fb[None]).cuda(), w.threshold)
     total, ovf = plan.candidates_count()
     assert not ovf
-    ref = orc.run_path(fb, w.fch1, w.foff, w.tsamp, w.ranges, w.widths, w.threshold, do_search=False)
+    cands = plan.candidates_read()
+    assert cands.size == total
+    ref = orc.run_path(fb, w.fch1, w.foff, w.tsamp, w.ranges, w.widths, w.threshold, do_search=True)
     check_dmt_against_oracle(plan, d_dmt.cpu().numpy(), ref)
+    st = check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+    assert st["oracle"] > 20000 and st["near_threshold_only_oracle"] + st["near_threshold_only_gpu"] <= 25, st
     _, _, _, nout, _ = plan.trial_table()
     s_all, q_all = plan.trial_stats_all(1)
     d = 0
