@@ -116,6 +116,22 @@ def test_cfg2_full(cuda, api, orc, synth):
     assert rep[0]["oracle"] == rep[0]["gpu"] + 0 or rep[0]["near"] > 0
 
 
+def test_cfg2_full_every_output(cuda, api, orc, synth):
+    """Config 2 complete: all 1.3e8 outputs, all statistics, the whole candidate list (threshold 6: 1.1e5 records)."""
+    w = synth.workload(2)
+    fb = synth.generate(w)
+    plan = make_plan(api, w, cand_capacity=1 << 24)
+    d_dmt = plan.search(cuda.from_numpy(fb[None]).cuda(), w.threshold)
+    total, ovf = plan.candidates_count()
+    assert not ovf
+    cands = plan.candidates_read()
+    ref = orc.run_path(fb, w.fch1, w.foff, w.tsamp, w.ranges, w.widths, w.threshold, do_search=True)
+    check_dmt_against_oracle(plan, d_dmt.cpu().numpy(), ref)
+    check_stats_against_oracle(plan, ref)
+    st = check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+    assert st["oracle"] > 100000 and st["near_threshold_only_oracle"] + st["near_threshold_only_gpu"] <= 100, st
+
+
 def test_cfg3_full_injected_bursts_found(cuda, api, orc, synth):
     """The bench workload.  Besides parity: the strong injected bursts are in the CUDA path's candidate list."""
     w, plan, cands, rep = run_full(cuda, api, orc, synth, 3, cap=1 << 26)
