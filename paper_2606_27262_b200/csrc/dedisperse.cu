@@ -202,6 +202,19 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
                  "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+// L2 policy of the DM-transform lines: a tile adds to its 64 x 512 outputs about once per 450 channels, eight or nine
+// times in all; between two passes the lines should stay in L2 rather than go to HBM half summed and come back.
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void st_hint(int32_t* addr, int32_t v, uint64_t pol) {
+    asm volatile("st.global.L2::cache_hint.b32 [%0], %1, %2;" ::"l"(addr), "r"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void red_hint(int32_t* addr, int32_t v, uint64_t pol) {
+    asm volatile("red.global.add.L2::cache_hint.s32 [%0], %1, %2;" ::"l"(addr), "r"(v), "l"(pol) : "memory");
+}
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
@@ -434,6 +447,7 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     const int lane_cap = (int)(65535u / max(1u, vmax - floor1));
     int since = 0;
     auto flush_lanes = [&]() {
+        const uint64_t pol_out = policy_evict_last();
         const uint32_t back = (uint32_t)since * floor1;   // the floor of the channels summed since the last pass
 #pragma unroll
         for (int q = 0; q < TPW; ++q) {
@@ -446,11 +460,11 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
                 const int32_t lo = (int32_t)((acc[q][j] & 0xFFFFu) + back), hi = (int32_t)((acc[q][j] >> 16) + back);
                 const bool ok_lo = i >= ok.x && i < ok.y, ok_hi = i + kH >= ok.x && i + kH < ok.y;
                 if (first_flush) {
-                    if (ok_lo) row[i] = lo;
-                    if (ok_hi) row[i + kH] = hi;
+                    if (ok_lo) st_hint(row + i, lo, pol_out);
+                    if (ok_hi) st_hint(row + i + kH, hi, pol_out);
                 } else {
-                    if (ok_lo) atomicAdd(row + i, lo);          // result unused: a fire-and-forget RED in L2
-                    if (ok_hi) atomicAdd(row + i + kH, hi);
+                    if (ok_lo) red_hint(row + i, lo, pol_out);  // fire-and-forget RED in L2
+                    if (ok_hi) red_hint(row + i + kH, hi, pol_out);
                 }
                 acc[q][j] = 0u;
             }

@@ -28,6 +28,19 @@ constexpr int kEpt = 8;                             // outputs per thread per su
 constexpr int kXEpt = 8;
 constexpr int kXSeg = kSpsThreads * kXEpt;
 
+// L2 policies of a row: the statistics pass asks L2 to keep it, the search pass, its last reader, lets it go first.
+__device__ __forceinline__ uint64_t l2_policy(bool keep) {
+    uint64_t p;
+    if (keep) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    else asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ int4 ld4_hint(const int4* a, uint64_t pol) {
+    int4 v;
+    asm volatile("ld.global.L2::cache_hint.v4.s32 {%0, %1, %2, %3}, [%4], %5;" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(a), "l"(pol));
+    return v;
+}
+
 __device__ __forceinline__ int padi(int i) { return i + (i >> 5); }  // bank-conflict-free stride-8 access (exact path)
 
 __device__ __forceinline__ long long shfl_down_ll(long long v, int d) {
@@ -113,8 +126,9 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
             sxx += (unsigned long long)(unsigned)v * (unsigned)v;
             mn = min(mn, v); mx = max(mx, v);
         }
+        const uint64_t keep = l2_policy(true);
         for (int i = l4 + tid; i < n4; i += kSpsThreads) {
-            const int4 v = x4[i];
+            const int4 v = ld4_hint(x4 + i, keep);
             sx += (long long)v.x + v.y + v.z + v.w;
             sxx += (unsigned long long)(unsigned)v.x * (unsigned)v.x + (unsigned long long)(unsigned)v.y * (unsigned)v.y +
                    (unsigned long long)(unsigned)v.z * (unsigned)v.z + (unsigned long long)(unsigned)v.w * (unsigned)v.w;
@@ -206,7 +220,7 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
             for (int it = 0; it < kIters; ++it) {
                 const int e = lo_al + tb + warp * kWarpSpan + it * 128 + lane * 4;
                 if (e >= lo && e + 4 <= n) {
-                    v[it] = *reinterpret_cast<const int4*>(x + e);
+                    v[it] = ld4_hint(reinterpret_cast<const int4*>(x + e), l2_policy(false));
                     v[it].x -= m; v[it].y -= m; v[it].z -= m; v[it].w -= m;
                 } else {                                          // the ends of the window: zero outside [lo, n)
                     v[it].x = (e >= lo && e < n) ? x[e] - m : 0;
