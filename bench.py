@@ -29,7 +29,7 @@ UNIT = "DM-trial*chan*samples/s"
 
 # DRAM bytes per launch of the dominant kernel (dedisp_tiled, range 0 of config 3) from the committed
 # `ncu --set full` capture (profiles/): dram__bytes_read.sum + dram__bytes_write.sum.
-NCU_TRAFFIC_BYTES = {3: 2579948000}   # profiles/r01_final_summary.md: 1.04 GB read + 1.54 GB written
+NCU_TRAFFIC_BYTES = {3: 2257476000}   # profiles/r01_final_summary.md: 0.83 GB read + 1.43 GB written
 
 
 def algorithmic_adds(plan, nchan):

@@ -357,9 +357,9 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     int bid = blockIdx.x;
     const int dmt = bid % a.ntile_dm; bid /= a.ntile_dm;
-    const int tt = bid % a.ntile_t;
     const int beam = bid / a.ntile_t;
     const TileDesc td = a.tiles[dmt];
+    const int tt = (bid % a.ntile_t + a.ntile_t - td.tshift % a.ntile_t) % a.ntile_t;
     const int64_t t0 = (int64_t)tt * kTT;   // trial i of the tile computes the outputs t0 - skew[i] + [0, kTT)
 
     const T* in = reinterpret_cast<const T*>(a.in) + (int64_t)beam * a.beam_stride;

@@ -275,6 +275,7 @@ int build_tiling(Plan& p) {
             td.skew0 = (d0 / DT) * DT;
             td.trial0 = d0;
             td.ntrial = std::min(DT, rp.ndm - d0);
+            td.tshift = rp.delay[(size_t)(d0 + td.ntrial / 2) * p.nchan + p.nchan / 2] / kTT;   // median delay over the channels
             td.stage0 = (int32_t)rp.sidx.size();
             std::vector<PendingGroup> open;
             auto blob_words_of = [&](const std::vector<PendingGroup>& gs, const PendingGroup* extra) {
