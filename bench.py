@@ -302,7 +302,7 @@ def run_ours(args, rank, world, local_rank):
     kernels = {f"kind{k}_range{r}": sum(v) / len(v) for (k, r), v in sorted(ktimes.items())}
 
     cpu = None
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and world == 1:      # rank 0 at N = 1 only
         rate, cores, sample, _, _ = oracle_sample(w, hv[0])
         cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample}
 
