@@ -145,9 +145,17 @@ def run_ours(args, rank, world, local_rank):
     build.build()
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the path has no CPU fallback")
+    # SPT_BENCH_BACKEND=gloo exists for one purpose: running the N > 1 plumbing (sharding, barriers, reductions, rank-0
+    # output) on a box with fewer GPUs than ranks; numbers from such a run mean nothing.
+    backend = os.environ.get("SPT_BENCH_BACKEND", "nccl")
+    if backend != "nccl":
+        local_rank %= torch.cuda.device_count()
     torch.cuda.set_device(local_rank)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        if backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+        else:
+            dist.init_process_group(backend)
 
     w = synth.workload(args.config)
     nbeam = w.nbeam                        # beams per GPU (weak scaling: every rank gets its own beams)
