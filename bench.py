@@ -308,6 +308,22 @@ def run_ours(args, rank, world, local_rank):
                 "algorithmic_hbm_bytes": hbm_bytes,
                 "traffic": NCU_TRAFFIC_BYTES.get(w.index)}
     kernels = {f"kind{k}_range{r}": sum(v) / len(v) for (k, r), v in sorted(ktimes.items())}
+    # SURVEY.md 8(d), metric (3): the HBM-bound kernels against the copy bandwidth (a2: bytes = raw in + uint16 out per
+    # decimated range, its timed span includes the pass that finds the bounds of the series; a4: the DM transform read once)
+    hbm_gbs = float(peaks.get("hbm_gbs", 6650.0))
+    other = {}
+    _, rg_all, dec_all, nout_all, _ = plan.trial_table()
+    for (k, r), v in sorted(ktimes.items()):
+        ms = sum(v) / len(v)
+        if k == 1:
+            kdec = int(dec_all[rg_all == r][0])
+            nbytes = (w.nchan * w.nsamp + 2 * w.nchan * (w.nsamp // kdec)) * nbeam
+            other[f"decimate_range{r}"] = {"bound": "hbm", "bytes": nbytes, "ms": ms, "achieved_gbs": nbytes / ms / 1e6,
+                                           "frac": nbytes / ms / 1e6 / hbm_gbs}
+        elif k == 3:
+            nbytes = 4 * int(nout_all.astype("int64").sum()) * nbeam
+            other["single_pulse_search"] = {"bound": "hbm", "bytes": nbytes, "ms": ms, "achieved_gbs": nbytes / ms / 1e6,
+                                            "frac": nbytes / ms / 1e6 / hbm_gbs}
 
     cpu = None
     if not args.no_cpu_baseline and world == 1:      # rank 0 at N = 1 only
@@ -331,7 +347,7 @@ def run_ours(args, rank, world, local_rank):
                     "rtf": data_s * world * steps / e2e_s, "api": "spt_stream_push/spt_stream_pop (two batches in flight)",
                     "ms_per_step_synchronous_call": e2e_sync_ms},
             "peak_filter": peak_info, "gpu_launches": launches, "clocks": clocks, "kernel_ms": kernels, "probe": probe,
-            "roofline": roof, "cpu_baseline": cpu}
+            "roofline": roof, "roofline_other": other, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
