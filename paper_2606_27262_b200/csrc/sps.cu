@@ -37,7 +37,7 @@ __device__ __forceinline__ uint64_t l2_policy(bool keep) {
 }
 __device__ __forceinline__ int4 ld4_hint(const int4* a, uint64_t pol) {
     int4 v;
-    asm volatile("ld.global.L2::cache_hint.v4.s32 {%0, %1, %2, %3}, [%4], %5;" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(a), "l"(pol));
+    asm("ld.global.L2::cache_hint.v4.s32 {%0, %1, %2, %3}, [%4], %5;" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(a), "l"(pol));
     return v;
 }
 
@@ -127,14 +127,20 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
             mn = min(mn, v); mx = max(mx, v);
         }
         const uint64_t keep = l2_policy(true);
-        for (int i = l4 + tid; i < n4; i += kSpsThreads) {
-            const int4 v = ld4_hint(x4 + i, keep);
+        auto take = [&](const int4 v) {
             sx += (long long)v.x + v.y + v.z + v.w;
             sxx += (unsigned long long)(unsigned)v.x * (unsigned)v.x + (unsigned long long)(unsigned)v.y * (unsigned)v.y +
                    (unsigned long long)(unsigned)v.z * (unsigned)v.z + (unsigned long long)(unsigned)v.w * (unsigned)v.w;
             mn = min(min(mn, v.x), min(v.y, min(v.z, v.w)));
             mx = max(max(mx, v.x), max(v.y, max(v.z, v.w)));
+        };
+        int i = l4 + tid;
+        for (; i + 3 * kSpsThreads < n4; i += 4 * kSpsThreads) {          // four loads in flight per thread
+            const int4 v0 = ld4_hint(x4 + i, keep), v1 = ld4_hint(x4 + i + kSpsThreads, keep);
+            const int4 v2 = ld4_hint(x4 + i + 2 * kSpsThreads, keep), v3 = ld4_hint(x4 + i + 3 * kSpsThreads, keep);
+            take(v0); take(v1); take(v2); take(v3);
         }
+        for (; i < n4; i += kSpsThreads) take(ld4_hint(x4 + i, keep));
         for (int i = max(n4, l4) * 4 + tid; i < n; i += kSpsThreads) {
             const int v = x[i];
             sx += v;
@@ -254,28 +260,47 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
             if (tid == 0) sh.c[kCOff] = 0u;
             __syncthreads();
 
+            // the next segment's samples are fetched into L1 while this one is tested (one 128-byte line per thread)
+            {
+                const int e = lo_al + tb + adv + tid * 32;
+                if (tb + adv < nbest && tid * 32 < kSegLoad && e >= 0 && e < n)
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(x + e));
+            }
             // S'_w[i] = c[kCOff + i + w] - c[kCOff + i]   (i relative to the segment)
             const int nthis = min(adv, nbest - tb);
             for (int i0 = 0; i0 < nthis; i0 += kSpsThreads * kEpt) {
                 // per slot: shared-memory address of c[i] and -c[i]; per (slot, width): one load, one add, one add-max
-                uint32_t adr[kEpt];
+                // (The prefix sums may wrap; c[i+w] - c[i] is exact all the same, so c[i] is subtracted before anything is compared.)
+                // Slots past the end of the segment are not clamped: i + w stays inside sh.c (i < i0 + 4096 <= the staged
+                // length minus the halo, or < 4096 with w <= 4064), they read stale words and are dropped by `pre` below.
+                // So slot e sits at a fixed distance from slot 0 and its loads take an immediate offset.
                 int nc0[kEpt], mxv[kEpt];
-                const uint32_t cbase = (uint32_t)__cvta_generic_to_shared(&sh.c[kCOff]);
+                const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(&sh.c[kCOff]) + 4u * (uint32_t)(i0 + tid);
 #pragma unroll
                 for (int e = 0; e < kEpt; ++e) {
-                    const int idx = min(i0 + e * kSpsThreads + tid, nthis - 1);   // clamped: out-of-range slots repeat the last one
-                    adr[e] = cbase + 4u * (uint32_t)idx;
-                    nc0[e] = -(int)sh.c[kCOff + idx];
+                    nc0[e] = -(int)sh.c[kCOff + i0 + e * kSpsThreads + tid];
                     mxv[e] = (int)0x80000000;
                 }
-                for (int k = 0; k < nw_eff; ++k) {
-                    const uint32_t wb = 4u * (uint32_t)a.widths[k];
+                int k = 0;
+                for (; k + 2 <= nw_eff; k += 2) {                          // two widths per pass: one 3-input max for both
+                    const uint32_t aw0 = a0 + 4u * (uint32_t)a.widths[k], aw1 = a0 + 4u * (uint32_t)a.widths[k + 1];
+                    const int nT0 = sh.negT[k], nT1 = sh.negT[k + 1];
+#pragma unroll
+                    for (int e = 0; e < kEpt; ++e) {
+                        uint32_t v0, v1;
+                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v0) : "r"(aw0 + (uint32_t)(e * kSpsThreads * 4)));   // [R + imm]
+                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v1) : "r"(aw1 + (uint32_t)(e * kSpsThreads * 4)));
+                        mxv[e] = max(mxv[e], max((int)v0 + nc0[e] + nT0, (int)v1 + nc0[e] + nT1));
+                    }
+                }
+                if (k < nw_eff) {
+                    const uint32_t aw = a0 + 4u * (uint32_t)a.widths[k];
                     const int nT = sh.negT[k];
 #pragma unroll
                     for (int e = 0; e < kEpt; ++e) {
                         uint32_t v;
-                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(adr[e] + wb));
-                        mxv[e] = max(mxv[e], (int)v + (nc0[e] + nT));
+                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(aw + (uint32_t)(e * kSpsThreads * 4)));
+                        mxv[e] = max(mxv[e], (int)v + nc0[e] + nT);
                     }
                 }
 #pragma unroll
