@@ -12,8 +12,9 @@
  *   - plain pointers and sizes only; every pointer argument says HOST or DEVICE.
  *   - every call returns SPT_OK (0) or a negative spt_status; nothing throws, aborts or prints.
  *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
- *   - spt_dedisperse / spt_single_pulse_search only ENQUEUE work on that stream; spt_candidates_*,
- *     spt_trial_stats and the *_host calls synchronise it.  One plan is used by one thread at a time.
+ *   - spt_dedisperse / spt_single_pulse_search / spt_search only ENQUEUE work on that stream (internal side streams are
+ *     forked from it and joined back into it before the call returns, so stream order holds for the caller);
+ *     spt_candidates_*, spt_trial_stats and the *_host calls synchronise it.  One plan is used by one thread at a time.
  *   - the caller owns the filterbank and DM-transform device buffers; the library owns everything
  *     reachable from the plan (tables, decimated series, statistics, candidate list) until spt_plan_destroy.
  *   - there is no CPU fallback: a call that needs the GPU fails with SPT_ERR_CUDA when none is usable.
