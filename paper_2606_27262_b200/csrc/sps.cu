@@ -29,9 +29,10 @@ constexpr int kXEpt = 8;
 constexpr int kXSeg = kSpsThreads * kXEpt;
 
 // L2 policies of a row: the statistics pass asks L2 to keep it, the search pass, its last reader, lets it go first.
-__device__ __forceinline__ uint64_t l2_policy(bool keep) {
+__device__ __forceinline__ uint64_t l2_policy(int mode) {   // 0: evict first, 1: evict last, 2: normal
     uint64_t p;
-    if (keep) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    if (mode == 1) asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    else if (mode == 2) asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
     else asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
     return p;
 }
@@ -126,7 +127,7 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
             sxx += (unsigned long long)(unsigned)v * (unsigned)v;
             mn = min(mn, v); mx = max(mx, v);
         }
-        const uint64_t keep = l2_policy(true);
+        const uint64_t keep = l2_policy(1);
         auto take = [&](const int4 v) {
             sx += (long long)v.x + v.y + v.z + v.w;
             sxx += (unsigned long long)(unsigned)v.x * (unsigned)v.x + (unsigned long long)(unsigned)v.y * (unsigned)v.y +
@@ -217,7 +218,9 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
         // the halo leaves room for them, so that no slot of the unrolled test below idles
         const int room = kSegLoad - halo;
         const int adv = room >= kSpsThreads * kEpt ? room / (kSpsThreads * kEpt) * (kSpsThreads * kEpt) : (room & ~3);
-        for (int tb = 0; tb < nbest; tb += adv) {
+        // Segments are taken from the end of the row backwards: the statistics pass has just read the row front to back,
+        // so its tail is what L1 and L2 still hold.
+        for (int tb = (nbest - 1) / adv * adv; tb >= 0; tb -= adv) {
             __syncthreads();                                    // the previous segment's readers are done
             // stage x - m: warp `warp` owns elements [warp*640, +640) of the segment; zero beyond N
             int4 v[kIters];
@@ -226,7 +229,7 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
             for (int it = 0; it < kIters; ++it) {
                 const int e = lo_al + tb + warp * kWarpSpan + it * 128 + lane * 4;
                 if (e >= lo && e + 4 <= n) {
-                    v[it] = ld4_hint(reinterpret_cast<const int4*>(x + e), l2_policy(false));
+                    v[it] = ld4_hint(reinterpret_cast<const int4*>(x + e), l2_policy(0));
                     v[it].x -= m; v[it].y -= m; v[it].z -= m; v[it].w -= m;
                 } else {                                          // the ends of the window: zero outside [lo, n)
                     v[it].x = (e >= lo && e < n) ? x[e] - m : 0;
@@ -262,8 +265,8 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
 
             // the next segment's samples are fetched into L1 while this one is tested (one 128-byte line per thread)
             {
-                const int e = lo_al + tb + adv + tid * 32;
-                if (tb + adv < nbest && tid * 32 < kSegLoad && e >= 0 && e < n)
+                const int e = lo_al + tb - adv + tid * 32;
+                if (tb >= adv && tid * 32 < kSegLoad && e >= 0 && e < n)
                     asm volatile("prefetch.global.L1 [%0];" ::"l"(x + e));
             }
             // S'_w[i] = c[kCOff + i + w] - c[kCOff + i]   (i relative to the segment)
