@@ -6,7 +6,7 @@
  *   ->  boxcar single-pulse search  ->  candidate readback
  *
  * What each call computes is fixed by the paper (PAPER.md line numbers below) and, where the paper is
- * silent, by the readings listed in DESIGN.md section 3 (same letters as SURVEY.md section 8(c)).
+ * silent, by the readings listed in DESIGN.md section 2 (same letters as SURVEY.md section 8(c)).
  *
  * Conventions
  *   - plain pointers and sizes only; every pointer argument says HOST or DEVICE.
@@ -79,7 +79,8 @@ typedef struct {
  * trial widths").  max_beams bounds nbeam of later calls.  cand_capacity = records the device candidate list
  * can hold (overflow is reported, not an error).
  * Unsupported (SPT_ERR_UNSUPPORTED): foff >= 0; decim not a power of two <= 64; nchan*255*decim >= 2^31 (int32
- * DM transform); widths[last]*nchan*255*decim >= 2^32 (boxcar sums are formed modulo 2^32).
+ * DM transform); widths[last]*nchan*255*decim >= 2^32 (boxcar sums are formed modulo 2^32);
+ * floor(nsamp/decim)*(nchan*255*decim)^2 >= 2^64 for any range (the exact sum of squares of a row is kept in 64 bits).
  * ----------------------------------------------------------------------------------------------------- */
 int spt_plan_create(double fch1_mhz, double foff_mhz, int32_t nchan, double tsamp_s, int64_t nsamp,
                     const spt_dm_range* ranges /*HOST*/, int32_t nranges,
@@ -103,7 +104,10 @@ int spt_plan_delays(const spt_plan* plan, int32_t trial, int32_t* host_out);
  *   "skew":          1 (default) = every trial of a DM tile computes an output window shifted by its own delay at a
  *                    reference channel, which narrows the windows the tile reads; 0 = one window start per tile
  *   "profile":       1 = bracket every kernel launch with CUDA events on the caller's stream (see
- *                    spt_plan_kernel_times); may be switched at any time
+ *                    spt_plan_kernel_times); may be switched at any time.  NOTE: it also changes the schedule -- with
+ *                    profile = 1 the DM ranges run one after the other on the caller's stream (so that each launch can
+ *                    be timed alone) instead of side by side on the library's side streams; results are identical, the
+ *                    step is about 3 % slower.  Leave it 0 for production and for end-to-end timing.
  * Unknown names / values -> SPT_ERR_INVALID. */
 int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value);
 

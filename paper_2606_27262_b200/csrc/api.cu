@@ -87,7 +87,8 @@ struct DeviceState {
     uint8_t* h_fb = nullptr;        // spt_search_host: device copy of the host filterbank
     int32_t* h_dmt = nullptr;       // spt_search_host: library-owned DM transform
     cudaStream_t own_stream = nullptr;
-    cudaStream_t last_stream = nullptr;
+    cudaStream_t last_stream = nullptr;     // stream of the last search / peak filter: what the read-out calls wait for
+    cudaStream_t dedisp_stream = nullptr;   // stream of the last dedispersion (decimated series, launch timings)
     int32_t nbeam_dedisp = 0, nbeam_search = 0;
     bool searched = false;
     // option "profile": events around every launch of the last dedisperse [0] / search [1]
@@ -96,10 +97,10 @@ struct DeviceState {
     std::vector<cudaEvent_t> event_pool;
 };
 
-static cudaEvent_t get_event(DeviceState* d) {
+static cudaEvent_t get_event(DeviceState* d) {   // nullptr when the driver cannot make another event
     cudaEvent_t e = nullptr;
     if (!d->event_pool.empty()) { e = d->event_pool.back(); d->event_pool.pop_back(); }
-    else cudaEventCreate(&e);
+    else if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); e = nullptr; }
     return e;
 }
 static void timed_clear(DeviceState* d, int slot) {
@@ -111,6 +112,12 @@ struct ScopedTimer {  // records e0 at construction and e1 at destruction when p
     ScopedTimer(Plan* p, cudaStream_t s, int slot_, int kind, int range) : d(p->dev), st(s), slot(slot_), on(p->opt_profile != 0) {
         if (!on) return;
         DeviceState::Timed t{kind, range, get_event(d), get_event(d)};
+        if (!t.e0 || !t.e1) {          // no event to be had: this launch goes untimed (it still runs)
+            if (t.e0) d->event_pool.push_back(t.e0);
+            if (t.e1) d->event_pool.push_back(t.e1);
+            on = false;
+            return;
+        }
         cudaEventRecord(t.e0, st);
         d->timed[slot].push_back(t);
     }
@@ -324,6 +331,7 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
     }
     SPT_CUDA(cudaGetLastError());
     d->last_stream = st;
+    d->dedisp_stream = st;
     d->nbeam_dedisp = nbeam;
     return SPT_OK;
 }
@@ -437,6 +445,12 @@ int spt_plan_create(double fch1_mhz, double foff_mhz, int32_t nchan, double tsam
     }
     if ((double)nchan * 255.0 * maxdec >= 2147483648.0) return SPT_ERR_UNSUPPORTED;
     if ((double)widths[nwidths - 1] * nchan * 255.0 * maxdec >= 4294967296.0) return SPT_ERR_UNSUPPORTED;
+    // Sxx = sum x^2 of a row is kept in 64 bits: a row of floor(nsamp/decim) samples of at most nchan*255*decim must fit
+    for (int32_t r = 0; r < nranges; ++r) {
+        const unsigned __int128 xmax = (unsigned __int128)nchan * 255u * (unsigned)ranges[r].decim;
+        const unsigned __int128 worst = (unsigned __int128)(nsamp / ranges[r].decim) * xmax * xmax;
+        if (worst >> 64) return SPT_ERR_UNSUPPORTED;
+    }
     if (widths[nwidths - 1] > 4096 - 32) return SPT_ERR_UNSUPPORTED;
     if (nsamp >= (1ll << 31)) return SPT_ERR_UNSUPPORTED;
     spt_plan* h = new (std::nothrow) spt_plan();
@@ -668,7 +682,7 @@ int spt_decimated_read(spt_plan* plan, int32_t range, int32_t beam, uint16_t* ho
     if (rp.decim == 1) return SPT_ERR_INVALID;
     if (!p.dev || p.dev->nbeam_dedisp == 0) return SPT_ERR_STATE;
     if (beam < 0 || beam >= p.dev->nbeam_dedisp) return SPT_ERR_SHAPE;
-    SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
+    SPT_CUDA(cudaStreamSynchronize(p.dev->dedisp_stream));
     if (rp.nsamp_k <= 0) return SPT_OK;
     const uint16_t* src = p.dev->r[range].series + (size_t)beam * p.nchan * rp.stride_k;
     SPT_CUDA(cudaMemcpy2D(host_out, (size_t)rp.nsamp_k * 2, src, (size_t)rp.stride_k * 2, (size_t)rp.nsamp_k * 2,
@@ -813,13 +827,21 @@ int spt_stream_push(spt_plan* plan, const uint8_t* h_fb, int32_t nbeam, float th
     SPT_CUDA(cudaEventRecord(sl.copied, d->copy_stream));
     cudaStream_t st = d->own_stream;
     SPT_CUDA(cudaStreamWaitEvent(st, sl.copied, 0));
-    const cudaEvent_t keep = d->wait_event;                     // the read-out calls keep looking at the batch popped last
+    // the read-out calls keep looking at the batch popped last: everything do_search changes for them is put back,
+    // also when the push fails half way
+    const cudaEvent_t keep = d->wait_event;
     const int keep_cur = d->cur;
-    const bool keep_searched = d->searched;
-    if ((rc = do_path(&p, sl.fb, nbeam, d->h_dmt, threshold, st, k)) != SPT_OK) return rc;
+    const bool keep_searched = d->searched, keep_peaks = d->peaks_valid;
+    const int32_t keep_nbeam = d->nbeam_search;
+    cudaStream_t const keep_stream = d->last_stream;
+    rc = do_path(&p, sl.fb, nbeam, d->h_dmt, threshold, st, k);
+    d->wait_event = keep; d->cur = keep_cur; d->searched = keep_searched; d->peaks_valid = keep_peaks;
+    d->nbeam_search = keep_nbeam;
+    // a read-out without an event (after spt_peak_filter, or of a plain call) synchronises the stream it ran on, not ours
+    if (keep_stream || keep_searched) d->last_stream = keep_stream;
+    if (rc != SPT_OK) return rc;
     SPT_CUDA(cudaMemcpyAsync(sl.h_count, d->bufs[k].count, 8, cudaMemcpyDeviceToHost, st));
     SPT_CUDA(cudaEventRecord(sl.done, st));
-    d->wait_event = keep; d->cur = keep_cur; d->searched = keep_searched;
     sl.nbeam = nbeam;
     sl.pending = true;
     d->push_next = k ^ 1;
@@ -1130,7 +1152,8 @@ int spt_plan_kernel_times(spt_plan* plan, int32_t cap, int32_t* kind, int32_t* r
     Plan& p = plan->p;
     *n = 0;
     if (!p.dev) return SPT_ERR_STATE;
-    if (p.dev->last_stream || p.dev->nbeam_dedisp) SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
+    if (p.dev->nbeam_dedisp) SPT_CUDA(cudaStreamSynchronize(p.dev->dedisp_stream));
+    if (p.dev->searched) SPT_CUDA(cudaStreamSynchronize(p.dev->last_stream));
     for (int slot = 0; slot < 2; ++slot)
         for (auto& t : p.dev->timed[slot]) {
             if (*n >= cap) return SPT_OK;

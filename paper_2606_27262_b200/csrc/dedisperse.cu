@@ -7,6 +7,8 @@
 // shared-memory load pipe and the integer ALUs, not a dense contraction.
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include "internal.h"
 #include "kernels.h"
 
@@ -88,16 +90,29 @@ __global__ void max_u16_kernel(const uint4* __restrict__ x, int64_t n16, uint32_
     }
 }
 
+// SM count of the current device (grid-stride kernels launch 8 blocks per SM); looked up once per device.
+int sm_count() {
+    constexpr int kMaxDev = 64;
+    static std::atomic<int> cached[kMaxDev];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kMaxDev) return 148;
+    int n = cached[dev].load(std::memory_order_relaxed);
+    if (n > 0) return n;
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) { cudaGetLastError(); n = 148; }
+    cached[dev].store(n, std::memory_order_relaxed);
+    return n;
+}
+
 void launch_max_u16(const uint16_t* x, int64_t nelem, uint32_t* maxval, cudaStream_t st) {
     const int64_t n16 = nelem / 8;            // rows are 16-element multiples
     if (n16 <= 0) return;
-    max_u16_kernel<<<148 * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(x), n16, maxval);
+    max_u16_kernel<<<sm_count() * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(x), n16, maxval);
 }
 
 void launch_max_u8(const uint8_t* x, int64_t nbytes, uint32_t* maxval, cudaStream_t st) {
     const int64_t n16 = nbytes / 16;          // rows are 16-byte multiples
     if (n16 <= 0) return;
-    max_u8_kernel<<<148 * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(x), n16, maxval);
+    max_u8_kernel<<<sm_count() * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(x), n16, maxval);
 }
 
 void launch_decimate(const uint8_t* x, int64_t in_row_stride, int64_t in_beam_stride, uint16_t* y,
@@ -532,11 +547,15 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
 
 template <typename T, int DT>
 static int launch_tiled_inst(const TiledArgs& a, cudaStream_t st) {
-    static bool attr_set = false;
+    // the opt-in to 113 KB of dynamic shared memory is a per-device attribute of the function: one flag per device
+    constexpr int kMaxDev = 64;
+    static std::atomic<bool> attr_set[kMaxDev];
     auto kern = dedisp_tiled_kernel<T, DT>;
-    if (!attr_set) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return -1;
+    if (dev < 0 || dev >= kMaxDev || !attr_set[dev].load(std::memory_order_acquire)) {
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes) != cudaSuccess) return -1;
-        attr_set = true;
+        if (dev >= 0 && dev < kMaxDev) attr_set[dev].store(true, std::memory_order_release);
     }
     const int64_t nblocks = (int64_t)a.ntile_dm * a.ntile_t * a.nbeam;
     if (nblocks <= 0) return 0;

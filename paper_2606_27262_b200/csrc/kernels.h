@@ -7,6 +7,8 @@
 
 namespace spt {
 
+int sm_count();   // SMs of the current device (dedisperse.cu)
+
 void launch_decimate(const uint8_t* x, int64_t in_row_stride, int64_t in_beam_stride, uint16_t* y,
                      int64_t out_row_stride, int64_t out_beam_stride, int32_t nchan, int32_t nbeam, int64_t nsamp_k,
                      int32_t k, cudaStream_t st);

@@ -76,7 +76,7 @@ __global__ void keep_history_kernel(const uint4* __restrict__ src, uint4* __rest
 void launch_keep_history(const uint8_t* src, uint8_t* dst, int64_t row_bytes, int64_t shift_bytes, int64_t keep_bytes,
                          int64_t nrows, cudaStream_t st) {
     if (keep_bytes <= 0 || nrows <= 0) return;
-    keep_history_kernel<<<148 * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(src), reinterpret_cast<uint4*>(dst),
+    keep_history_kernel<<<sm_count() * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(src), reinterpret_cast<uint4*>(dst),
                                                   row_bytes / 16, shift_bytes / 16, keep_bytes / 16, nrows);
 }
 

@@ -59,6 +59,22 @@ def test_strerror_and_argument_validation(api):
         assert e.value.code == code, (change, e.value.code)
 
 
+def test_sum_of_squares_bound(api):
+    """Sxx of a row is a 64-bit integer: a plan whose worst row floor(nsamp/k) * (nchan*255*k)^2 reaches 2^64 is refused at
+    creation (it would wrap silently on both sides of the parity test), the largest one below the bound is accepted."""
+    nchan, k = 4096, 64
+    xmax = nchan * 255 * k                                     # largest sample of the decimated DM transform
+    n_ok = (2**64 - 1) // (xmax * xmax)                        # longest row whose worst-case Sxx still fits
+    assert n_ok * xmax * xmax < 2**64 <= (n_ok + 1) * xmax * xmax
+    kw = dict(fch1=500.0, foff=-0.048828125, nchan=nchan, tsamp=1.31072e-3, ranges=[(0.0, 1.0, 2, k)], widths=[1, 2, 4])
+    api.Plan(nsamp=n_ok * k + k - 1, **kw).close()             # floor(nsamp/k) == n_ok
+    with pytest.raises(api.SptError) as e:
+        api.Plan(nsamp=(n_ok + 1) * k, **kw)
+    assert e.value.code == api.SPT_ERR_UNSUPPORTED
+    # the BASELINE configs are far below it (config 5, decimation 4: 2^16 * (4096*255*4)^2 = 1.1e18)
+    assert (2**18 // 4) * (4096 * 255 * 4) ** 2 < 2**60
+
+
 def test_options_and_state_errors(api):
     p = api.Plan(500.0, -3.125, 64, 1.31072e-3, 4096, [(0.0, 1.0, 101, 1)], [1, 2, 4])
     p.set_option("group", 8)

@@ -3,11 +3,11 @@ points, noise and the partition of the core points are unique in DBSCAN, so they
 for the cluster representative, the cuts and the anti-coincidence rule."""
 import numpy as np
 import pytest
+import sklearn.cluster as sk   # a hard import: without it the oracle's DBSCAN would have no external pin
 
 
 @pytest.mark.parametrize("seed", range(5))
 def test_dbscan_agrees_with_scikit_learn(orc, seed):
-    sk = pytest.importorskip("sklearn.cluster")
     rs = np.random.default_rng(seed)
     centres = rs.uniform(0, 20, size=(6, 2))
     pts = np.concatenate([c + rs.normal(0, 0.25, size=(40, 2)) for c in centres] + [rs.uniform(0, 20, size=(80, 2))])
