@@ -254,6 +254,12 @@ def generate(w: Workload, beam: int = 0, out: Optional[np.ndarray] = None, nthre
     return out
 
 
+def uniform_bytes(nchan: int, nsamp: int, seed: int) -> np.ndarray:
+    """uint8 [nchan][nsamp] of i.i.d. uniform bytes 0..255 (numpy PCG64, seeded): the full-range input of the worst-case
+    legs (8-bit telescope data with unmitigated RFI can span the whole range); no signal in it."""
+    return np.random.default_rng(seed).integers(0, 256, size=(nchan, nsamp), dtype=np.uint8)
+
+
 def checksum(buf: np.ndarray) -> int:
     buf = np.ascontiguousarray(buf).view(np.uint8).reshape(-1)
     return int(_load().synth_checksum(buf.ctypes.data, buf.size))

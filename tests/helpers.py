@@ -118,3 +118,64 @@ def check_candidates_against_oracle(orc, plan, cands, oracle_ranges, widths, thr
                         stats["near_threshold_only_gpu"] += 1
             d += 1
     return stats
+
+
+def check_candidates_dense(orc, plan, cands, oracle_ranges, widths, threshold, beam=None):
+    """Rules D2 at any volume: instead of sorting 1e8 records, the CUDA path's records of one DM
+    range are scattered into dense rows laid out like the oracle's packed DM transform and read back at the oracle's
+    (sorted) candidate positions.  cands: the records of ONE beam (beam=None: all of them are)."""
+    mine = cands if beam is None else cands[cands["beam"] == beam]
+    stats = dict(oracle=0, gpu=int(mine.size), matched=0, near_threshold_only_oracle=0, near_threshold_only_gpu=0,
+                 width_near_ties=0, max_dsnr=0.0)
+    d0 = 0
+    seen = 0
+    for rr in oracle_ranges:
+        ndm = len(rr.nout)
+        sr = rr.search
+        g = mine[(mine["trial"] >= d0) & (mine["trial"] < d0 + ndm)]
+        seen += int(g.size)
+        nelem = int(rr.rowoff[-1])
+        tl = g["trial"].astype(np.int64) - d0
+        assert np.all((g["t"] >= 0) & (g["t"] < rr.nout[tl])), "candidate outside its row"
+        dense_s = np.full(nelem, np.nan, dtype=np.float32)
+        dense_w = np.zeros(nelem, dtype=np.int16)
+        gkey = rr.rowoff[tl] + g["t"]
+        dense_s[gkey] = g["snr"]
+        dense_w[gkey] = g["width"]
+        assert int(np.count_nonzero(~np.isnan(dense_s))) == g.size, "duplicate (trial, t) in the candidate list"
+        del gkey, tl
+        okey = sr.t.astype(np.int64) + np.repeat(rr.rowoff[:-1], sr.count)
+        stats["oracle"] += int(okey.size)
+        gs, gw = dense_s[okey], dense_w[okey]
+        have = ~np.isnan(gs)
+        # (ii) an event only the oracle has must sit within the tolerance of the threshold
+        only_o = np.flatnonzero(~have)
+        assert np.all(np.abs(sr.snr[only_o] - threshold) <= SNR_TOL), "oracle-only candidate away from the threshold"
+        stats["near_threshold_only_oracle"] += int(only_o.size)
+        # (iii) matched events
+        ds = np.abs(sr.snr[have] - gs[have].astype(np.float64))
+        if ds.size:
+            stats["max_dsnr"] = max(stats["max_dsnr"], float(ds.max()))
+            assert ds.max() <= SNR_TOL, f"range of trial {d0}: |dSNR| = {ds.max()}"
+        stats["matched"] += int(ds.size)
+        # (iv) widths, up to near ties
+        for j in np.flatnonzero(have & (gw != sr.w)):
+            i = int(np.searchsorted(rr.rowoff, okey[j], side="right")) - 1
+            row = rr.dmt[rr.rowoff[i]: rr.rowoff[i + 1]]
+            alt = orc.snr_at(row, int(gw[j]), int(sr.t[j]))
+            assert abs(alt - sr.snr[j]) <= SNR_TOL, f"trial {d0 + i} t {sr.t[j]}: width {gw[j]} vs {sr.w[j]}"
+            stats["width_near_ties"] += 1
+        # (ii) again: what is left after taking the oracle's positions out exists on the CUDA side only
+        dense_s[okey] = np.nan
+        best_cache = {}
+        for key in np.flatnonzero(~np.isnan(dense_s)):
+            i = int(np.searchsorted(rr.rowoff, key, side="right")) - 1
+            if i not in best_cache:
+                best_cache[i] = orc.best_width(rr.dmt[rr.rowoff[i]: rr.rowoff[i + 1]], widths)[0]
+            b = best_cache[i][int(key - rr.rowoff[i])]
+            assert abs(b - threshold) <= SNR_TOL, f"trial {d0 + i} t {key - rr.rowoff[i]}: GPU-only candidate, oracle best {b}"
+            stats["near_threshold_only_gpu"] += 1
+        del dense_s, dense_w, okey, gs, gw
+        d0 += ndm
+    assert seen == mine.size, "candidate with a trial index outside the plan"
+    return stats

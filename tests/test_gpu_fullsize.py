@@ -5,7 +5,7 @@ sampled rows)."""
 import numpy as np
 import pytest
 
-from helpers import SNR_TOL, check_candidates_against_oracle, check_dmt_against_oracle, check_plan_against_oracle, check_stats_against_oracle, make_plan
+from helpers import SNR_TOL, check_candidates_against_oracle, check_candidates_dense, check_dmt_against_oracle, check_plan_against_oracle, check_stats_against_oracle, make_plan
 
 pytestmark = pytest.mark.gpu
 
@@ -200,16 +200,113 @@ def test_cfg6_band5_full(cuda, api, orc, synth):
     assert found == len(strong), (found, len(strong))
 
 
-def test_cfg5_full_rfi_volume(cuda, api, orc, synth):
-    """Candidate-list volume and the widest boxcars (w = 1024)."""
-    w, plan, cands, rep = run_full(cuda, api, orc, synth, 5, cap=1 << 29, trials_per_range=1)
-    assert rep["candidates"] > 1_000_000          # zero-DM spikes smear into every trial (SURVEY.md 8(c)-D4)
+def full_beam_parity(orc, plan, w, fb, d_dmt_beam, cands_beam, s_row, q_row, dense=False):
+    """One beam complete: every output, every trial's exact statistics, the whole candidate list (rules D2)."""
+    ref = orc.run_path(fb, w.fch1, w.foff, w.tsamp, w.ranges, w.widths, w.threshold, do_search=True)
+    check_dmt_against_oracle(plan, d_dmt_beam.cpu().numpy()[None], ref)
+    d = 0
+    for rr in ref:
+        for i in range(len(rr.nout)):
+            assert int(s_row[d]) == int(rr.search.sum[i]), ("sum", d)
+            assert int(q_row[d]) == int(rr.search.sumsq[i]), ("sumsq", d)
+            d += 1
+    if dense:
+        return check_candidates_dense(orc, plan, cands_beam, ref, w.widths, w.threshold)
+    return check_candidates_against_oracle(orc, plan, cands_beam, ref, w.widths, w.threshold, beam=int(cands_beam["beam"][0]) if cands_beam.size else 0)
+
+
+def test_cfg5_full_every_output(cuda, api, orc, synth):
+    """Config 5 (RFI-stressed, 4096 ch x 2^18, widths to 1024, threshold 6) complete, through the call bench.py times: all
+    8.2e8 outputs, the exact statistics of all 4501 trials, and the whole candidate list -- about 2.5e8 records -- compared
+    trial by trial through dense rows.  This config runs a different schedule from config 3: a wider
+    data range (more widening passes), a third of the samples taking the full S/N evaluation, the widest boxcars."""
+    w = synth.workload(5)
+    fb = synth.generate(w)
+    plan = make_plan(api, w, cand_capacity=1 << 29)
+    check_plan_against_oracle(orc, plan, w, stride=499)
+    d_dmt = plan.search(cuda.from_numpy(fb[None]).cuda(), w.threshold)
+    total, ovf = plan.candidates_count()
+    assert not ovf, total
+    assert total > 1_000_000                      # zero-DM spikes smear into every trial (SURVEY.md 8(c)-D4)
+    cands = plan.candidates_read()
+    assert cands.size == total and np.all(cands["beam"] == 0)
     assert (cands["width"] == 1024).any()
+    s_all, q_all = plan.trial_stats_all(1)
+    st = full_beam_parity(orc, plan, w, fb, d_dmt[0], cands, s_all[0], q_all[0], dense=True)
+    assert st["oracle"] > 1_000_000
+    assert st["near_threshold_only_oracle"] + st["near_threshold_only_gpu"] <= 1e-4 * st["oracle"], st
+
+
+def test_cfg3_shape_uniform_bytes_full_every_output(cuda, api, orc, synth):
+    """The bench plan on the data the 16-bit lanes like least: i.i.d. uniform bytes 0..255 (what unmitigated 8-bit
+    telescope data can look like), so that every launch runs with its lane capacity at the floor 257/k and the stages cut
+    for the worst case -- every output, statistic and candidate of the 4501 trials."""
+    w = synth.workload(3)
+    fb = synth.uniform_bytes(w.nchan, w.nsamp, seed=33)
+    assert fb.min() == 0 and fb.max() == 255
+    plan = make_plan(api, w, cand_capacity=1 << 24)
+    d_dmt = plan.search(cuda.from_numpy(fb[None]).cuda(), w.threshold)
+    total, ovf = plan.candidates_count()
+    assert not ovf
+    cands = plan.candidates_read()
+    s_all, q_all = plan.trial_stats_all(1)
+    st = full_beam_parity(orc, plan, w, fb, d_dmt[0], cands, s_all[0], q_all[0], dense=True)
+    assert st["gpu"] == total
+
+
+CFG4_BEAMS_CHECKED = (0, 1, 7, 8, 15, 27, 28, 29, 31, 32, 40, 47, 48, 56, 62, 63)   # incl. both sides of the 2^31-byte
+                                                                                   # (7|8) and 2^31-element (28|29) offsets
 
 
 def test_cfg4_multibeam_batch_full(cuda, api, orc, synth):
-    """64 beams in one launch (64-bit offsets: 18 GiB of DM transform); two beams checked against the oracle."""
-    w, plan, cands, rep = run_full(cuda, api, orc, synth, 4, cap=1 << 27, beams_to_check=(0, 63), trials_per_range=1)
-    _, _, _, nout, _ = plan.trial_table()
+    """Config 4: 64 beams in one launch (64-bit offsets: 18 GiB of DM transform).  16 beams complete against the oracle
+    (every output, statistic, candidate); on ALL 64 beams the sum of every row against the prefix-sum identity
+    sum_t out[d][t] = sum_c (P_c[delay + nout] - P_c[delay]) evaluated from the raw input with the oracle's delay table, and
+    the kernel's sum of squares against the DM transform it was computed from."""
+    w = synth.workload(4)
+    nb = w.nbeam
+    h_fb = np.empty((nb, w.nchan, w.nsamp), dtype=np.uint8)
+    for b in range(nb):
+        synth.generate(w, beam=b, out=h_fb[b])
+    plan = make_plan(api, w, nbeam=nb, cand_capacity=1 << 27)
+    check_plan_against_oracle(orc, plan, w, stride=499)
+    _, rg, dec, nout, off = plan.trial_table()
     assert int((nout == 0).sum()) == 544
-    assert set(np.unique(cands["beam"])) <= set(range(64))
+    d_dmt = plan.search(cuda.from_numpy(h_fb).cuda(), w.threshold)
+    total, ovf = plan.candidates_count()
+    assert not ovf, total
+    cands = plan.candidates_read()
+    assert cands.size == total and set(np.unique(cands["beam"])) <= set(range(nb))
+    s_all, q_all = plan.trial_stats_all(nb)
+    order = np.argsort(cands["beam"], kind="stable")
+    cands = cands[order]
+    starts = np.searchsorted(cands["beam"], np.arange(nb + 1))
+    ncheck = 0
+    for b in CFG4_BEAMS_CHECKED:
+        st = full_beam_parity(orc, plan, w, h_fb[b], d_dmt[b], cands[starts[b]: starts[b + 1]], s_all[b], q_all[b])
+        assert st["gpu"] == starts[b + 1] - starts[b]
+        ncheck += 1
+    assert ncheck == 16
+    # all 64 beams: row sums from channel prefix sums of the input (independent of any dedispersion code)
+    delays = [orc.delay_table(w.fch1, w.foff, w.nchan, w.tsamp, lo, step, ndm, k) for (lo, step, ndm, k) in w.ranges]
+    offs = cuda.from_numpy(off).cuda()
+    nouts = cuda.from_numpy(nout.astype(np.int64)).cuda()
+    live = nouts > 0
+    for b in range(nb):
+        d0 = 0
+        for (lo, step, ndm, k), dly in zip(w.ranges, delays):
+            y = h_fb[b].astype(np.int64) if k == 1 else h_fb[b][:, : (w.nsamp // k) * k].reshape(w.nchan, -1, k).sum(-1, dtype=np.int64)
+            P = np.zeros((w.nchan, y.shape[1] + 1), dtype=np.int64)
+            np.cumsum(y, axis=1, out=P[:, 1:])
+            no = nout[d0: d0 + ndm].astype(np.int64)
+            cidx = np.arange(w.nchan)[None, :]
+            dl = np.where(no[:, None] > 0, dly, 0)       # empty trials: the sweep is longer than the data
+            expect = (P[cidx, dl + no[:, None]] - P[cidx, dl]).sum(axis=1)
+            assert np.array_equal(s_all[b, d0: d0 + ndm], expect), ("row sums", b, lo)
+            d0 += ndm
+        v = d_dmt[b].to(cuda.int64)
+        cs = cuda.cumsum(v * v, 0)                       # modulo 2^64: differences are exact
+        hi = cs[(offs + nouts - 1).clamp(min=0)]
+        lo_ = cuda.where(offs > 0, cs[(offs - 1).clamp(min=0)], cuda.zeros_like(hi))
+        qq = cuda.where(live, hi - lo_, cuda.zeros_like(hi)).cpu().numpy().astype(np.uint64)
+        assert np.array_equal(q_all[b], qq), ("row sums of squares", b)
