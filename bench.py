@@ -262,6 +262,8 @@ class Measurement:
             opts["group"] = args.group
         if args.dm_tile:
             opts["dm_tile"] = args.dm_tile
+        if args.max_entries:
+            opts["max_entries"] = args.max_entries
         self.plan = api.Plan(w.fch1, w.foff, w.nchan, w.tsamp, w.nsamp, w.ranges, w.widths, max_beams=nbeam,
                              cand_capacity=CAND_CAPACITY[w.index], options=opts)
         self.adds_step = algorithmic_adds(self.plan, w.nchan) * nbeam
@@ -652,6 +654,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5, 6])
     ap.add_argument("--group", type=int, default=0)
     ap.add_argument("--dm-tile", type=int, default=0)
+    ap.add_argument("--max-entries", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-worst-case", action="store_true")
     ap.add_argument("--all-configs", action="store_true")

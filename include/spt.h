@@ -116,6 +116,11 @@ int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value);
  * tiles, and the largest shared-memory footprint (32-bit words) of a stage.  Any out pointer may be NULL. */
 int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int64_t* nstages, int64_t* ngroups,
                          int64_t* nvariants, int64_t* ntiles_t, int64_t* max_stage_words);
+/* Work of the kernel's pre-sum phase over all DM tiles of a range (one time tile each): warp tasks, entries processed by
+ * them (the straight-line class size of each task's group), variants stored, and rounds of eight tasks -- what the entry
+ * cap is chosen by, for reports.  Any out pointer may be NULL. */
+int spt_plan_tiling_cost(spt_plan* plan, int32_t range, int64_t* ntasks, int64_t* task_entries, int64_t* task_variants,
+                         int64_t* presum_rounds);
 /* The delay row of one trial as the tiled kernel will apply it, reconstructed from those tables alone:
  * host_out[nchan] (HOST).  Must equal spt_plan_delays for every trial (checked by the CPU tests). */
 int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out);

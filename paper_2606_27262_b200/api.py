@@ -50,6 +50,7 @@ SYMBOLS = {
     "spt_plan_delays": (ctypes.c_int, [_vp, _i32, _vp]),
     "spt_plan_set_option": (ctypes.c_int, [_vp, ctypes.c_char_p, _i64]),
     "spt_plan_tiling_info": (ctypes.c_int, [_vp, _i32, _P(_i64), _P(_i64), _P(_i64), _P(_i64), _P(_i64), _P(_i64)]),
+    "spt_plan_tiling_cost": (ctypes.c_int, [_vp, _i32, _P(_i64), _P(_i64), _P(_i64), _P(_i64)]),
     "spt_plan_tiling_delays": (ctypes.c_int, [_vp, _i32, _vp]),
     "spt_dedisperse": (ctypes.c_int, [_vp, _vp, _i32, _vp, _vp]),
     "spt_decimated": (ctypes.c_int, [_vp, _i32, _P(_vp), _P(_i64)]),
@@ -190,6 +191,11 @@ class Plan:
         _check(lib().spt_plan_tiling_info(self._h, rng, *[ctypes.byref(x) for x in v]), "spt_plan_tiling_info")
         keys = ("ntiles_dm", "nstages", "ngroups", "nvariants", "ntiles_t", "max_stage_words")
         return {k: int(x.value) for k, x in zip(keys, v)}
+
+    def tiling_cost(self, rng: int) -> dict:
+        v = [ctypes.c_int64() for _ in range(4)]
+        _check(lib().spt_plan_tiling_cost(self._h, rng, *[ctypes.byref(x) for x in v]), "spt_plan_tiling_cost")
+        return {k: int(x.value) for k, x in zip(("ntasks", "task_entries", "task_variants", "presum_rounds"), v)}
 
     def tiling_delays(self, d: int) -> np.ndarray:
         out = np.empty(self.nchan, dtype=np.int32)

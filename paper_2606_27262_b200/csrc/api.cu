@@ -314,7 +314,7 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
             else launch_dedisp_naive<uint8_t>((const uint8_t*)src, rs, (int64_t)p->nchan * rs, rd.delay, nout, off,
                                               p->nchan, rp.ndm, nbeam, rp.max_nout, d_dmt, p->dmt_elems, st);
         } else {
-            const int rc = launch_dedisp_tiled(u16, p->opt_dm_tile, src, rs, (int64_t)p->nchan * rs, d_dmt, p->dmt_elems,
+            const int rc = launch_dedisp_tiled(u16, p->opt_dm_tile, rp.max_ent, src, rs, (int64_t)p->nchan * rs, d_dmt, p->dmt_elems,
                                                rd.tiles, rd.sidx, rd.rows, rd.blob, d->maxval + 2 * i, rd.skew, rp.skew_max, rp.vcap_words, nout, off,
                                                (int32_t)rp.tiles.size(), rp.ntile_t, nbeam, st);
             if (rc != 0) { g_last_error = "dedisp_tiled: launch configuration rejected"; return SPT_ERR_CUDA; }
@@ -520,8 +520,11 @@ int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value) {
         if (value != 0 && value != 1) return SPT_ERR_INVALID;
         p.opt_kernel = (int32_t)value;
     } else if (!std::strcmp(name, "group")) {
-        if (value != 1 && value != 2 && value != 4 && value != 8) return SPT_ERR_INVALID;
+        if (value != 1 && value != 2 && value != 4 && value != 8 && value != 12 && value != 16) return SPT_ERR_INVALID;
         p.opt_group = (int32_t)value; p.tiling_built = false;
+    } else if (!std::strcmp(name, "max_entries")) {
+        if (value != 8 && value != 12 && value != 16) return SPT_ERR_INVALID;
+        p.opt_max_ent = (int32_t)value; p.tiling_built = false;
     } else if (!std::strcmp(name, "skew")) {
         if (value != 0 && value != 1) return SPT_ERR_INVALID;
         p.opt_skew = (int32_t)value; p.tiling_built = false;
@@ -575,6 +578,21 @@ int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int6
     return SPT_OK;
 }
 
+int spt_plan_tiling_cost(spt_plan* plan, int32_t range, int64_t* ntasks, int64_t* task_entries, int64_t* task_variants,
+                         int64_t* presum_rounds) {
+    if (!plan) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (range < 0 || range >= (int32_t)p.ranges.size()) return SPT_ERR_SHAPE;
+    const int rc = ensure_tiling(p);
+    if (rc != SPT_OK) return rc;
+    const RangePlan& rp = p.ranges[range];
+    if (ntasks) *ntasks = rp.ntasks;
+    if (task_entries) *task_entries = rp.task_entries;
+    if (task_variants) *task_variants = rp.task_variants;
+    if (presum_rounds) *presum_rounds = rp.presum_rounds;
+    return SPT_OK;
+}
+
 int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
     if (!plan || !host_out) return SPT_ERR_INVALID;
     Plan& p = plan->p;
@@ -609,7 +627,8 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
             for (int32_t k = 0; k <= ntog; ++k)
                 if (vd[k] == (uint32_t)(vbase + r * vlen)) bits = (1u << k) - 1u;
             for (int32_t c = 0; c < ncorr; ++c)
-                if (vd[kChainWords + 2 * c] == (uint32_t)(vbase + r * vlen)) bits = ((1u << ntog) - 1u) & ~vd[kChainWords + 1 + 2 * c];
+                if (vd[chain_words(ent_class(nch)) + 2 * c] == (uint32_t)(vbase + r * vlen))
+                    bits = ((1u << ntog) - 1u) & ~vd[chain_words(ent_class(nch)) + 1 + 2 * c];
             if (bits == 0xffffffffu) return SPT_ERR_STATE;
             for (int pass = 0; pass < 2; ++pass)       // pass 0: base shifts; pass 1: one sample later per delta taken
                 for (int32_t q = 0; q < nch; ++q) {

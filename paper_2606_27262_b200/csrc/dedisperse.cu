@@ -286,12 +286,11 @@ __device__ __forceinline__ void load_entry(uint32_t addr, uint32_t c1, uint32_t 
 }
 
 // B: one warp task = kChunkU variant words (4 per lane) of every variant of one group.  All control flow is warp
-// uniform and the eight entries are straight-line code (unused entries repeat the first one; their deltas are never
+// uniform and the NE entries are straight-line code (unused entries repeat the first one; their deltas are never
 // taken): a lane past the end of the variants works on the last four words and does not store.
-template <typename T>
+template <typename T, int NE>
 __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uint32_t task, uint32_t var_addr,
-                                            uint32_t raw_addr, int lane, uint32_t floor2) {
-    const uint4 gh = *reinterpret_cast<const uint4*>(tb + kBlobHdrWords + 4 * (task & 0xffu));   // 128-bit broadcast loads
+                                            uint32_t raw_addr, int lane, uint32_t floor2, const uint4 gh) {
     const int vlen = (int)gh.y;
     const uint32_t meta = gh.z;
     const int ntog = (int)((meta >> 8) & 0xffu), ncorr = (int)((meta >> 16) & 0xffu);
@@ -305,9 +304,9 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
     // every channel of the group enters the base sum once: take the launch's smallest sample off each (both lanes)
     const uint32_t bias = 0u - (gh.x >> 16) * floor2;
     uint32_t cur[4] = {bias, bias, bias, bias};
-    uint32_t dl[kMaxG][4];
+    uint32_t dl[NE][4];
 #pragma unroll
-    for (int q2 = 0; q2 < kMaxG / 2; ++q2) {
+    for (int q2 = 0; q2 < NE / 2; ++q2) {
         const uint4 c2 = cd[q2];                  // two entries per load
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
@@ -326,7 +325,7 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
     // prefix chain: after step k, cur = base sum + deltas of the first k entries
     uint4 v4 = vd[0];
 #pragma unroll
-    for (int k = 0; k <= kMaxG; ++k) {
+    for (int k = 0; k <= NE; ++k) {
         if (k <= ntog) {
             if (k > 0) {
 #pragma unroll
@@ -339,11 +338,11 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
     }
     // variants off the chain (few): all deltas, minus those the variant does not take
     for (int c = 0; c < ncorr; ++c) {
-        const uint32_t* vc = reinterpret_cast<const uint32_t*>(vd) + kChainWords + 2 * c;
+        const uint32_t* vc = reinterpret_cast<const uint32_t*>(vd) + (NE + 4) + 2 * c;   // chain_words(NE)
         const uint32_t dst = vc[0], mask = vc[1];
         uint32_t o[4] = {cur[0], cur[1], cur[2], cur[3]};
 #pragma unroll
-        for (int q = 0; q < kMaxG; ++q)
+        for (int q = 0; q < NE; ++q)
             if (mask & (1u << q)) {
 #pragma unroll
                 for (int i = 0; i < 4; ++i) o[i] -= dl[q][i];
@@ -352,7 +351,9 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
     }
 }
 
-template <typename T, int DT>
+// NEMAX: the largest entry class the plan's tables hold (8, 12 or 16): the kernel carries only the pre-sum instances it
+// needs, so that a plan of small groups does not pay for the registers of the large ones.
+template <typename T, int DT, int NEMAX>
 __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledArgs a) {
     constexpr int NW = kThreads / 32;
     constexpr int TPW = DT / NW;
@@ -496,8 +497,14 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
         const uint16_t* toff = reinterpret_cast<const uint16_t*>(tb + tb[3]);
 
         // ---- B: pre-sum every variant of every group ---------------------------------------------------------
-        for (int tk = warp; tk < ntask; tk += NW)
-            presum_task<T>(tb, tb[kBlobHdrWords + 4 * ngrp + tk], var_addr, raw_addr, lane, floor2);
+        for (int tk = warp; tk < ntask; tk += NW) {
+            const uint32_t task = tb[kBlobHdrWords + 4 * ngrp + tk];
+            const uint4 gh = *reinterpret_cast<const uint4*>(tb + kBlobHdrWords + 4 * (task & 0xffu));   // 128-bit broadcast load
+            const uint32_t nent = gh.z & 0xffu;       // warp uniform: the smallest straight-line instance that holds the group
+            if (NEMAX == 8 || nent <= 8u) presum_task<T, 8>(tb, task, var_addr, raw_addr, lane, floor2, gh);
+            else if (NEMAX == 12 || nent <= 12u) presum_task<T, 12>(tb, task, var_addr, raw_addr, lane, floor2, gh);
+            else presum_task<T, 16>(tb, task, var_addr, raw_addr, lane, floor2, gh);
+        }
         __syncthreads();  // variants complete; raw rows and the other blob buffer are free
         if (s + 1 < td.nstage) issue_stage(s + 1);
 
@@ -545,12 +552,12 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     flush_lanes();
 }
 
-template <typename T, int DT>
+template <typename T, int DT, int NEMAX>
 static int launch_tiled_inst(const TiledArgs& a, cudaStream_t st) {
     // the opt-in to 113 KB of dynamic shared memory is a per-device attribute of the function: one flag per device
     constexpr int kMaxDev = 64;
     static std::atomic<bool> attr_set[kMaxDev];
-    auto kern = dedisp_tiled_kernel<T, DT>;
+    auto kern = dedisp_tiled_kernel<T, DT, NEMAX>;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return -1;
     if (dev < 0 || dev >= kMaxDev || !attr_set[dev].load(std::memory_order_acquire)) {
@@ -564,14 +571,23 @@ static int launch_tiled_inst(const TiledArgs& a, cudaStream_t st) {
     return 0;
 }
 
-int launch_dedisp_tiled(bool is_u16, int DT, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
+template <int DT, int NEMAX>
+static int launch_tiled_type(bool is_u16, const TiledArgs& a, cudaStream_t st) {
+    return is_u16 ? launch_tiled_inst<uint16_t, DT, NEMAX>(a, st) : launch_tiled_inst<uint8_t, DT, NEMAX>(a, st);
+}
+
+int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
                         int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
                         const uint32_t* blob, const uint32_t* maxval, const int32_t* skew, int32_t skew_max, int32_t vcap_words,
                         const int32_t* nout, const int64_t* offset, int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, cudaStream_t st) {
     TiledArgs a{in, row_stride, beam_stride, out, out_beam_stride, tiles, sidx, rows, blob, maxval, skew, skew_max, nout, offset,
                 vcap_words, ntile_dm, ntile_t, nbeam};
-    if (DT == 64) return is_u16 ? launch_tiled_inst<uint16_t, 64>(a, st) : launch_tiled_inst<uint8_t, 64>(a, st);
-    if (DT == 32) return is_u16 ? launch_tiled_inst<uint16_t, 32>(a, st) : launch_tiled_inst<uint8_t, 32>(a, st);
+    if (DT == 64 && max_ent == 8) return launch_tiled_type<64, 8>(is_u16, a, st);
+    if (DT == 64 && max_ent == 12) return launch_tiled_type<64, 12>(is_u16, a, st);
+    if (DT == 64 && max_ent == 16) return launch_tiled_type<64, 16>(is_u16, a, st);
+    if (DT == 32 && max_ent == 8) return launch_tiled_type<32, 8>(is_u16, a, st);
+    if (DT == 32 && max_ent == 12) return launch_tiled_type<32, 12>(is_u16, a, st);
+    if (DT == 32 && max_ent == 16) return launch_tiled_type<32, 16>(is_u16, a, st);
     return -1;
 }
 

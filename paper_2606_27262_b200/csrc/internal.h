@@ -23,14 +23,15 @@ constexpr int kMaxWidths = 32;
 constexpr int kH = 256;              // words per trial per tile
 constexpr int kTT = 2 * kH;          // output samples per tile
 constexpr int kThreads = 256;        // 8 warps
-constexpr int kMaxG = 8;             // channels per pre-summed group
+constexpr int kMaxEnt = 16;          // entries (a channel at one of its shifts) per pre-summed group, at most; the pre-sum code
+                                     // exists for groups of up to 8, 12 and 16 entries (ent_class)
 constexpr int kMaxVar = 16;          // variants per group
 constexpr int kMaxDT = 64;           // trials per DM tile
 constexpr int kMaxStageGroups = 8;   // groups per stage
 constexpr int kChunkU = 128;         // variant words one warp builds per pre-sum task (4 per lane)
 constexpr int kBlobBytes = 3072;     // per-stage table blob (two buffers in shared memory)
 constexpr int kSmemBytes = 113 * 1024;                                   // two blocks per SM (228 KB incl. 1 KB each reserved)
-constexpr int kMaxStageRows = kMaxStageGroups * kMaxG;                   // raw rows of one stage
+constexpr int kMaxStageRows = 96;                                        // raw rows (channels) of one stage
 constexpr int kSmemCtrlBytes = 64 + kMaxDT * 16 + 2 * (kMaxStageRows * 16 + 16);  // mbarrier, per-trial {row pointer, nout},
                                                                          // next stage's {RowDesc[], StageIndex} x 2
 constexpr int kSmemDataBytes = kSmemBytes - kSmemCtrlBytes - 2 * kBlobBytes;  // variant region + raw-row region
@@ -40,21 +41,23 @@ constexpr int kSmemDataBytes = kSmemBytes - kSmemCtrlBytes - 2 * kBlobBytes;  //
 //   [4 ..)        ngrp x { vbase | channels << 16, vlen, nent | ntog << 8 | ncorr << 16 | nvar << 24, cdesc_off | vdesc_off << 16 }
 //                 (offsets inside the blob)
 //   task table    ntask x { group | chunk << 8 }: warp task = kChunkU variant words of every variant of one group
-//   cdesc         per group, kMaxG entries of 2 words (the first nent are real, the rest repeat the first one without
-//                 bit 26), in PREFIX ORDER (most-often-taken delta first; the first ntog have
+//   cdesc         per group, ent_class(nent) entries of 2 words (the first nent are real, the rest repeat the first one
+//                 without bit 26), in PREFIX ORDER (most-often-taken delta first; the first ntog have
 //                 a delta that some trial takes); an entry is a channel at one of its shifts: bits 0-17 byte offset
 //                 inside the raw region of the aligned 32-bit word (uint16 input: 8-byte unit) that holds the entry's sample
 //                 at u = 0, bits 24-25 position of that sample inside it, bit 26 = the entry is the channel's smallest shift and adds
 //                 it to the base sum.  The entry's delta (sample one later minus sample) moves its channel one later.
 //                 Second word: what the kernel's realignment needs (uint8: bits 0-4 funnel-shift amount, bits 8-23 PRMT
 //                 selector of the fifth sample; uint16: bits 0-1 = that position).
-//   vdesc         per group: kChainWords chain words, word k <= ntog = offset in the variant region of the variant "base sum
+//   vdesc         per group: chain_words(ent_class(nent)) chain words, word k <= ntog = offset in the variant region of the variant "base sum
 //                 + deltas of the first k entries" (0xffffffff: no trial uses it); then ncorr x { offset, mask } for the
 //                 variants off the chain: all ntog deltas minus those in mask.  Headers, cdesc and vdesc are 16-byte
 //                 aligned: the kernel reads them with 128-bit broadcast loads.
 //   trial_off     ngrp x DT uint16 = word offset of the trial's read start in the variant region
 constexpr int kBlobHdrWords = 4;
-constexpr int kChainWords = 12;      // chain words of a group's vdesc, padded (kMaxG + 1 used at most); corrections follow
+// The pre-sum code is straight-line over a fixed number of entries; a group runs the smallest instance that holds it.
+constexpr int ent_class(int nent) { return nent <= 8 ? 8 : nent <= 12 ? 12 : 16; }
+constexpr int chain_words(int cls) { return cls + 4; }   // cls + 1 chain words used at most, padded to 128-bit loads; corrections follow
 constexpr uint32_t kEntryAddBase = 1u << 26;
 
 struct RowDesc {            // one raw channel row of a stage; 16 bytes
@@ -100,8 +103,12 @@ struct RangePlan {
     std::vector<int32_t> skew;       // [ntiles_dm][DT]: trial i of a tile computes the outputs t0 - skew[i] + [0, kTT)
     int32_t skew_max = 0;
     int32_t vcap_words = 0;          // words of the variant region; the raw region follows it
+    int32_t max_ent = 8;             // entry cap the tables were built for: selects the kernel instance
     int32_t ntile_t = 0;             // time tiles
     int64_t ngroups = 0, nvariants = 0, ncorrected = 0;   // totals, for reports (ncorrected: variants off the prefix chain)
+    // work of the pre-sum over all DM tiles, for the cost model that picks the entry cap (build_tiling) and for reports:
+    // warp tasks, entries processed (straight-line: the class size of each task's group), variants stored, rounds of 8 tasks
+    int64_t ntasks = 0, task_entries = 0, task_variants = 0, presum_rounds = 0;
 };
 
 struct DeviceState;  // defined in api.cu
@@ -118,7 +125,8 @@ struct Plan {
     int64_t dmt_elems = 0;           // per beam
     // options
     int32_t opt_kernel = 0;          // 0 tiled, 1 naive
-    int32_t opt_group = 8;
+    int32_t opt_group = 0;           // channels per group, at most (0: 8 or 16, with the entry cap)
+    int32_t opt_max_ent = 0;         // entries per group, at most: 8, 12 or 16 (0: chosen per range by the cost model)
     int32_t opt_dm_tile = 64;
     int32_t opt_profile = 0;
     int32_t opt_skew = 1;            // per-trial output skew inside a DM tile (0: all trials of a tile share t0)

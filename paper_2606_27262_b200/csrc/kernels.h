@@ -20,7 +20,7 @@ void launch_dedisp_naive(const T* y, int64_t row_stride, int64_t beam_stride, co
                          const int32_t* d_nout, const int64_t* d_offset, int32_t nchan, int32_t ndm, int32_t nbeam,
                          int32_t max_nout, int32_t* out, int64_t out_beam_stride, cudaStream_t st);
 
-int launch_dedisp_tiled(bool is_u16, int DT, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
+int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
                         int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
                         const uint32_t* blob, const uint32_t* maxval, const int32_t* skew, int32_t skew_max, int32_t vcap_words,
                         const int32_t* nout, const int64_t* offset,

@@ -115,7 +115,7 @@ inline int popcount32(uint32_t x) { return __builtin_popcount(x); }
 // "tau_j > l".  Bits sorted by how often they are set form the prefix chain.
 // skew[i] (tile local): trial i's output window starts skew[i] samples early, i.e. its effective delays are
 // delay - skew[i] (they may be negative); relative delays between channels do not change.
-static bool make_group(const Plan& p, const RangePlan& rp, int32_t d0, int32_t ntrial, int32_t c0, int G, int es,
+static bool make_group(const Plan& p, const RangePlan& rp, int32_t d0, int32_t ntrial, int32_t c0, int G, int max_ent, int es,
                        const int32_t* skew, PendingGroup& g) {
     g.chan0 = c0;
     int32_t dmin = INT32_MAX, dmax = INT32_MIN;
@@ -146,7 +146,7 @@ static bool make_group(const Plan& p, const RangePlan& rp, int32_t d0, int32_t n
             if (lo < 0 || hi > 30000) return false;
             g.smin[j] = (int16_t)lo; g.smax[j] = (int16_t)hi;
             nent += std::max(1, hi - lo);
-            if (nent > kMaxG) ok = false;
+            if (nent > max_ent) ok = false;
         }
         if (!ok) continue;   // gsize == 1 always passes: channel c0 relative to itself
         g.ent.clear();
@@ -212,11 +212,14 @@ static bool make_group(const Plan& p, const RangePlan& rp, int32_t d0, int32_t n
     return true;
 }
 
-int build_tiling(Plan& p) {
-    const int G = p.opt_group, DT = p.opt_dm_tile;
-    for (RangePlan& rp : p.ranges) {
+// Tables of one DM range for groups of at most G channels and max_ent entries.
+static int build_range(const Plan& p, RangePlan& rp, const int G, const int max_ent) {
+    const int DT = p.opt_dm_tile;
+    rp.max_ent = max_ent;
+    {
         rp.tiles.clear(); rp.sidx.clear(); rp.rows.clear(); rp.blob.clear();
         rp.ngroups = rp.nvariants = rp.ncorrected = 0;
+        rp.ntasks = rp.task_entries = rp.task_variants = rp.presum_rounds = 0;
         // Output skew per trial: trial i of a DM tile computes the outputs t0 - skew[i] + [0, kTT)
         // with skew[i] = delay[i][cref] - delay[0][cref], so that at channel cref all trials of the tile read the same
         // window and elsewhere the windows spread by |delay slope(c) - delay slope(cref)| only.  cref minimises the sum
@@ -259,7 +262,7 @@ int build_tiling(Plan& p) {
             int64_t vb = 0, rb = 0;
             for (int32_t c = 0; c < p.nchan;) {
                 PendingGroup g;
-                if (!make_group(p, rp, d0, nt, c, G, es, &rp.skew[(size_t)(d0 / DT) * DT], g)) return SPT_ERR_UNSUPPORTED;
+                if (!make_group(p, rp, d0, nt, c, G, max_ent, es, &rp.skew[(size_t)(d0 / DT) * DT], g)) return SPT_ERR_UNSUPPORTED;
                 vb += (int64_t)g.vwords * 4; rb += g.raw_bytes;
                 c += g.nch;
             }
@@ -281,7 +284,7 @@ int build_tiling(Plan& p) {
             auto blob_words_of = [&](const std::vector<PendingGroup>& gs, const PendingGroup* extra) {
                 int64_t w = kBlobHdrWords + 4;
                 auto one = [&](const PendingGroup& g) {
-                    w += 4 + (g.vlen + kChunkU - 1) / kChunkU + 2 * kMaxG + kChainWords + 2 * g.ncorrected + 3 + DT / 2;
+                    w += 4 + (g.vlen + kChunkU - 1) / kChunkU + 2 * ent_class(g.nent) + chain_words(ent_class(g.nent)) + 2 * g.ncorrected + 3 + DT / 2;
                 };
                 for (const PendingGroup& g : gs) one(g);
                 if (extra) one(*extra);
@@ -320,7 +323,7 @@ int build_tiling(Plan& p) {
                         // second word, ready for the kernel: uint8: funnel-shift amount and the PRMT selector of sample 4
                         cdesc.push_back(es == 1 ? (a0 * 8u) | ((a0 * 0x1111u + 0x4400u) << 8) : a0);
                     }
-                    for (int q = g.nent; q < kMaxG; ++q) {   // padding: straight-line code in the kernel; deltas never taken
+                    for (int q = g.nent; q < ent_class(g.nent); ++q) {   // padding: straight-line code in the kernel; deltas never taken
                         const uint32_t c0 = cdesc[cdesc.size() - 2 * (size_t)g.nent], c1 = cdesc[cdesc.size() - 2 * (size_t)g.nent + 1];
                         cdesc.push_back(c0 & ~kEntryAddBase);
                         cdesc.push_back(c1);
@@ -336,6 +339,8 @@ int build_tiling(Plan& p) {
                     vbase += g.vwords;
                     rbase += g.raw_bytes;
                     rp.ngroups++; rp.nvariants += g.nvar; rp.ncorrected += g.ncorrected;
+                    const int64_t nt = (g.vlen + kChunkU - 1) / kChunkU;
+                    rp.ntasks += nt; rp.task_entries += nt * ent_class(g.nent); rp.task_variants += nt * g.nvar;
                 }
                 const uint32_t vdesc0 = cdesc0 + (uint32_t)cdesc.size();
                 vbase = 0;
@@ -349,7 +354,7 @@ int build_tiling(Plan& p) {
                             if (g.vars[r].k == k2 && !(g.vars[r].plus | g.vars[r].minus)) dst = (uint32_t)(vbase + r * g.vlen);
                         vdesc.push_back(dst);
                     }
-                    for (int k2 = g.ntog + 1; k2 < kChainWords; ++k2) vdesc.push_back(0xffffffffu);   // three 128-bit loads
+                    for (int k2 = g.ntog + 1; k2 < chain_words(ent_class(g.nent)); ++k2) vdesc.push_back(0xffffffffu);   // whole 128-bit loads
                     // off the chain: destination and the mask of the deltas NOT taken (subtracted from the full sum)
                     for (int r = 0; r < g.nvar; ++r)
                         if (g.vars[r].plus | g.vars[r].minus) {
@@ -362,6 +367,7 @@ int build_tiling(Plan& p) {
                 int nch_stage = 0;
                 for (const PendingGroup& g : open) nch_stage += g.nch;
                 hdr[0] = (uint32_t)ngrp; hdr[1] = (flush ? 1u : 0u) | ((uint32_t)nch_stage << 8); hdr[2] = ntask;
+                rp.presum_rounds += (ntask + kThreads / 32 - 1) / (kThreads / 32);
                 while ((vdesc0 + vdesc.size()) % 4) vdesc.push_back(0);   // trial_off rows are read with 128-bit loads
                 hdr[3] = vdesc0 + (uint32_t)vdesc.size();
                 rp.blob.insert(rp.blob.end(), hdr.begin(), hdr.end());
@@ -380,7 +386,7 @@ int build_tiling(Plan& p) {
             std::vector<PendingGroup> all;
             for (int32_t c = 0; c < p.nchan;) {
                 PendingGroup g;
-                if (!make_group(p, rp, d0, td.ntrial, c, std::min(G, lane_channels), es, &rp.skew[(size_t)(d0 / DT) * DT], g))
+                if (!make_group(p, rp, d0, td.ntrial, c, std::min(G, lane_channels), max_ent, es, &rp.skew[(size_t)(d0 / DT) * DT], g))
                     return SPT_ERR_UNSUPPORTED;
                 c += g.nch;
                 if (g.vwords > rp.vcap_words || g.raw_bytes > rcap_bytes || blob_words_of({}, &g) * 4 > kBlobBytes)
@@ -401,9 +407,9 @@ int build_tiling(Plan& p) {
                 for (size_t n = 1; i0 + n <= all.size() && n <= (size_t)kMaxStageGroups; ++n) {
                     const PendingGroup& g = all[i0 + n - 1];
                     v += g.vwords; r += g.raw_bytes; nch += g.nch;
-                    words += 4 + (g.vlen + kChunkU - 1) / kChunkU + 2 * kMaxG + kChainWords + 2 * g.ncorrected + 3 + DT / 2;
+                    words += 4 + (g.vlen + kChunkU - 1) / kChunkU + 2 * ent_class(g.nent) + chain_words(ent_class(g.nent)) + 2 * g.ncorrected + 3 + DT / 2;
                     tasks += (g.vlen + kChunkU - 1) / kChunkU;
-                    if (n > 1 && (v > rp.vcap_words || r > rcap_bytes || words * 4 > kBlobBytes || nch > lane_channels)) break;
+                    if (n > 1 && (v > rp.vcap_words || r > rcap_bytes || words * 4 > kBlobBytes || nch > lane_channels || nch > kMaxStageRows)) break;
                     const double cost = ((tasks + kWarps - 1) / kWarps + kStageOverheadRounds) / nch;
                     if (cost <= best_cost) { best_cost = cost; best_n = n; }
                 }
@@ -417,6 +423,35 @@ int build_tiling(Plan& p) {
         // a stage's transaction also fetches the NEXT stage's index and a fixed-size slice of its rows: pad the arrays
         rp.sidx.push_back(StageIndex{0, 0, 0, 0});
         rp.rows.resize(rp.rows.size() + kMaxStageRows, RowDesc{0, 0, 0, 0});
+    }
+    return SPT_OK;
+}
+
+// Modelled time of a range's launch per time tile, arbitrary units ("entry cap"): the gather and the
+// stage loop cost per group, the pre-sum per entry processed and variant stored; the 12- and 16-entry pre-sum instances run
+// 1.5x and 2.1x slower per unit than the 8-entry one (register pressure: fewer loads in flight).  Constants fitted to the
+// range-0 launches of configs 3 and 6 measured with caps 8, 12 and 16.
+static double modelled_cost(const RangePlan& rp) {
+    const double pen = rp.max_ent <= 8 ? 1.0 : rp.max_ent <= 12 ? 1.5 : 2.1;
+    return 2.456e-3 * (double)rp.ngroups + 2.37e-5 * pen * (double)(rp.task_entries + rp.task_variants);
+}
+
+int build_tiling(Plan& p) {
+    for (RangePlan& rp : p.ranges) {
+        int rc;
+        if (p.opt_max_ent != 0) {                 // fixed by the caller (A/B runs, tests)
+            if ((rc = build_range(p, rp, p.opt_group ? p.opt_group : (p.opt_max_ent > 8 ? 16 : 8), p.opt_max_ent)) != SPT_OK) return rc;
+            continue;
+        }
+        // default: groups of up to 8 entries, or of up to 12 where the model says the smaller gather outweighs the costlier
+        // pre-sum (bands whose sweeps are short: few variants per group) -- by a margin for the decimated ranges, whose
+        // pre-sum the constants fit less well
+        if ((rc = build_range(p, rp, p.opt_group ? p.opt_group : 8, 8)) != SPT_OK) return rc;
+        if (p.opt_group != 0 && p.opt_group <= 8) continue;
+        const double c8 = modelled_cost(rp);
+        RangePlan alt = rp;
+        if (build_range(p, alt, p.opt_group ? p.opt_group : 16, 12) != SPT_OK) continue;
+        if (modelled_cost(alt) < c8 * (rp.decim == 1 ? 0.97 : 0.90)) rp = std::move(alt);
     }
     p.tiling_built = true;
     return SPT_OK;
