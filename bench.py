@@ -608,15 +608,15 @@ def run_stream(args, local_rank):
     nblk = 4
     long_w = synth.workload(3, nsamp=nnew * nblk)
     fb = synth.generate(long_w)
-    blocks = [torch.from_numpy(fb[:, i * nnew:(i + 1) * nnew].T.copy()).cuda()[None] for i in range(nblk)]
+    blocks = [torch.from_numpy(fb[:, i * nnew:(i + 1) * nnew].T.copy()).cuda()[:, None, :] for i in range(nblk)]   # [t][beam][chan]
     d_dmt = torch.empty((1, plan.dmt_elems_per_beam), dtype=torch.int32, device="cuda")
     stream = torch.cuda.current_stream()
     _, _, dec, nout, _ = plan.trial_table()
     adds_new = int(sum(nnew // int(k) for k in dec)) * w.nchan          # algorithmic adds of the NEW outputs of a push
     adds_full = int(nout.astype("int64").sum()) * w.nchan                 # what recomputing the whole buffer costs
 
-    def push(i):
-        plan.segment_push(blocks[i % nblk], False, d_dmt, stream)
+    def push(i, incremental=True):
+        plan.segment_push(blocks[i % nblk], False, d_dmt, stream, spliced=True, whole_rows=not incremental)
         plan.segment_search(d_dmt, nnew, w.threshold, stream)
         return plan.candidates_count()
 
@@ -631,16 +631,28 @@ def run_stream(args, local_rank):
     e1.record(stream)
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / steps
+    e0.record(stream)
+    for i in range(4):                          # for the record: every push recomputing the whole buffer (whole_rows = 1)
+        push(i, incremental=False)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_whole = e0.elapsed_time(e1) / 4
     # batch rate on the same GPU for comparison: config 3 as bench.py times it
     mb = Measurement(args, w, 0, 1)
     tb = mb.timed(10, 3, local_rank)
     ms_b = tb["ms_total"] / 10
     out = {"stream": {"nnew": nnew, "history": nsamp - nnew, "min_history_search": hsearch, "nsamp_buffer": nsamp, "pushes": steps,
-                      "ms_per_push": ms, "rtf": nnew * w.tsamp / (ms * 1e-3), "adds_new_per_push": adds_new,
+                      "ms_per_push": ms, "ms_per_push_whole_rows": ms_whole, "rtf": nnew * w.tsamp / (ms * 1e-3), "adds_new_per_push": adds_new,
                       "adds_if_whole_buffer_recomputed": adds_full, "value_new_outputs": adds_new / (ms * 1e-3),
                       "candidates_last_push": ncand, "api": "spt_segment_push + spt_segment_search + spt_candidates_count"},
            "batch": {"workload": w.name, "ms_per_step": ms_b, "rtf": mb.data_s / (ms_b * 1e-3), "value": mb.adds_step / (ms_b * 1e-3)},
            "stream_rtf_over_batch_rtf": (nnew * w.tsamp / (ms * 1e-3)) / (mb.data_s / (ms_b * 1e-3)),
+           "stream_rate_over_batch_rate": (adds_new / (ms * 1e-3)) / (mb.adds_step / (ms_b * 1e-3)),
+           "note": "a stream yields nnew/decim outputs per trial per nnew samples; the batch call yields nout < nsamp/decim (the "
+                   "sweep is lost at the end of its buffer), i.e. %.1f %% fewer additions per second of data: the RTF ratio "
+                   "cannot exceed %.3f at equal addition rates" % (
+                       100.0 * (1.0 - (mb.adds_step / mb.data_s) / (adds_new / (nnew * w.tsamp))),
+                       (mb.adds_step / mb.data_s) / (adds_new / (nnew * w.tsamp))),
            "unit": UNIT}
     print(json.dumps(out), flush=True)
 

@@ -231,17 +231,25 @@ int spt_stream_pop(spt_plan* plan, int64_t* ncand, int32_t* overflowed);
  * highest frequency first; every segment is read with an overlap so that each DM trial has its full
  * sweep; reading F).
  *
- * spt_corner_turn: d_out[b][c'][t] = d_in[b][t][c], c' = flip ? nchan-1-c : c.   d_in DEVICE uint8 [nbeam][nsamp][nchan]
- *   (time-major), d_out DEVICE uint8 [nbeam][nchan][nsamp] (what spt_dedisperse takes).  Needs no plan.  Enqueues.
+ * spt_corner_turn: d_out[b][c'][t] = d_in(b, t, c), c' = flip ? nchan-1-c : c.   d_in DEVICE uint8, time-major:
+ *   spliced = 0: [nbeam][nsamp][nchan] (one block per beam); spliced = 1: [nsamp][nbeam][nchan] (the beams of a host
+ *   time-spliced sample by sample, as the telescope's rings hold them).  d_out DEVICE uint8
+ *   [nbeam][nchan][nsamp] (what spt_dedisperse takes).  Needs no plan.  Enqueues.
  *
  * spt_segment_push: overlap-save.  The plan's nsamp is the length of a library-owned working buffer per channel row =
  *   history + new samples.  A push drops the oldest nnew samples of every row, appends the corner-turned new block
- *   (d_new DEVICE uint8 [nbeam][nnew][nchan], time-major; flip as above) and computes the DM transform of the buffer
- *   into d_dmt exactly as spt_dedisperse would (same layout).  The buffer starts as zeros.  With
+ *   (d_new DEVICE uint8, time-major, [nbeam][nnew][nchan] or, spliced = 1, [nnew][nbeam][nchan]; flip as above) and
+ *   dedisperses the buffer into d_dmt in the layout of spt_dedisperse.  The buffer starts as zeros.  With
  *   nsamp - nnew >= min_history every trial d gains nnew/decim new outputs per push: the LAST nnew/decim of its nout[d]
- *   samples; the ones before them repeat outputs of earlier pushes.  nnew must be a multiple of `granule` (16, or the
- *   largest decimation factor if larger) so that the shift keeps the decimation phase and the row alignment.
- *   SPT_ERR_SHAPE when the history is shorter than min_history.  Enqueues on cuda_stream.
+ *   samples; the ones before them repeat outputs of earlier pushes.
+ *     whole_rows = 1: every row is computed in full, exactly as spt_dedisperse would;
+ *     whole_rows = 0: only what is new is computed -- the last nnew/decim + wmax - 1 outputs of every row (wmax = the
+ *       widest boxcar; those wmax - 1 repeat the end of the previous push's row: they are the lead-in of the window
+ *       spt_segment_search reads) -- and every other element of d_dmt is left as it was.  Per push that is
+ *       nchan * sum_d (nnew/decim_d + wmax - 1) additions instead of nchan * sum_d nout[d].
+ *   nnew must be a multiple of `granule` (16, or the largest decimation factor if larger) so that the shift keeps the
+ *   decimation phase and the row alignment.  SPT_ERR_SHAPE when the history is shorter than min_history.  Enqueues on
+ *   cuda_stream (the history copy runs on a side stream beside the corner turn and is joined before the dedispersion).
  * spt_segment_info: min_history = the longest sweep of the plan in raw samples, rounded up to the granule;
  *   min_history_search = the same plus (widest boxcar - 1) samples of the coarsest rate (what spt_segment_search needs).
  *
@@ -253,13 +261,13 @@ int spt_stream_pop(spt_plan* plan, int64_t* ncand, int32_t* overflowed);
  *   the index inside the row (add the row's stream offset for an absolute time).  d_dmt: what spt_segment_push wrote.
  *   Needs nsamp - nnew >= min_history_search (else SPT_ERR_SHAPE).  Read-out calls as after spt_single_pulse_search.
  * ----------------------------------------------------------------------------------------------------- */
-int spt_corner_turn(const uint8_t* d_in /*DEVICE*/, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip,
+int spt_corner_turn(const uint8_t* d_in /*DEVICE*/, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip, int32_t spliced,
                     uint8_t* d_out /*DEVICE*/, void* cuda_stream);
 int spt_segment_info(const spt_plan* plan, int64_t* min_history, int64_t* min_history_search, int64_t* granule);
 int spt_segment_search(spt_plan* plan, const int32_t* d_dmt /*DEVICE*/, int32_t nbeam, int64_t nnew, float threshold,
                        void* cuda_stream);
-int spt_segment_push(spt_plan* plan, const uint8_t* d_new /*DEVICE*/, int32_t nbeam, int64_t nnew, int32_t flip,
-                     int32_t* d_dmt /*DEVICE*/, void* cuda_stream);
+int spt_segment_push(spt_plan* plan, const uint8_t* d_new /*DEVICE*/, int32_t nbeam, int64_t nnew, int32_t flip, int32_t spliced,
+                     int32_t whole_rows, int32_t* d_dmt /*DEVICE*/, void* cuda_stream);
 
 /* -------------------------------------------------------------------------------------------------------
  * spt_sift -- candidate optimisation after the search (reading G), on a HOST list (typically

@@ -214,6 +214,13 @@ def corner_turn(x_time_major: np.ndarray, flip: bool = False) -> np.ndarray:
     return np.ascontiguousarray(y[::-1]) if flip else y
 
 
+def corner_turn_spliced(block: np.ndarray, flip: bool = False) -> List[np.ndarray]:
+    """A time-spliced block [nsamp][nbeam][nchan] (the beams of one host interleaved sample by sample) ->
+    per beam the channel-major [nchan][nsamp] array: beam b's samples are block[:, b, :]."""
+    block = np.asarray(block, dtype=np.uint8)
+    return [corner_turn(block[:, b, :], flip) for b in range(block.shape[1])]
+
+
 def overlap_save_buffers(blocks_time_major: Sequence[np.ndarray], nsamp: int, flip: bool = False) -> List[np.ndarray]:
     """The working buffer ([nchan][nsamp]) after each push of a stream that starts on a history of zeros: the last
     nsamp samples of zeros ++ block 0 ++ block 1 ++ ... (every trial of a dedispersion of it has its full sweep when

@@ -66,10 +66,10 @@ SYMBOLS = {
     "spt_peak_filter": (ctypes.c_int, [_vp, _P(_i32), _i32, _vp]),
     "spt_peaks_count": (ctypes.c_int, [_vp, _P(_i64)]),
     "spt_peaks_read": (ctypes.c_int, [_vp, _vp, _i64, _P(_i64)]),
-    "spt_corner_turn": (ctypes.c_int, [_vp, _i32, _i64, _i32, _i32, _vp, _vp]),
+    "spt_corner_turn": (ctypes.c_int, [_vp, _i32, _i64, _i32, _i32, _i32, _vp, _vp]),
     "spt_segment_info": (ctypes.c_int, [_vp, _P(_i64), _P(_i64), _P(_i64)]),
     "spt_segment_search": (ctypes.c_int, [_vp, _vp, _i32, _i64, _f32, _vp]),
-    "spt_segment_push": (ctypes.c_int, [_vp, _vp, _i32, _i64, _i32, _vp, _vp]),
+    "spt_segment_push": (ctypes.c_int, [_vp, _vp, _i32, _i64, _i32, _i32, _i32, _vp, _vp]),
     "spt_cutout": (ctypes.c_int, [_vp, _i32, _i64, _f64, _f64, _f64, _f64, _f64, _i32, _i64, _i32, _i32, _i32, _vp, _vp, _vp]),
     "spt_delta_dm": (_f64, [_f64, _f64, _f64, _f64]),
     "spt_sift": (ctypes.c_int, [_vp, _vp, _i64, _i32, _P(spt_sift_params), _vp, _i64, _P(_i64), _P(_i64)]),
@@ -303,16 +303,20 @@ class Plan:
         _check(lib().spt_segment_search(self._h, _dev_ptr(d_dmt), d_dmt.shape[0], int(nnew), float(threshold),
                                         _stream_ptr(stream)), "spt_segment_search")
 
-    def segment_push(self, d_new, flip: bool = False, d_dmt=None, stream=None):
-        """Overlap-save push of a time-major CUDA uint8 block [nbeam][nnew][nchan]; returns the DM transform tensor."""
+    def segment_push(self, d_new, flip: bool = False, d_dmt=None, stream=None, spliced: bool = False, whole_rows: bool = True):
+        """Overlap-save push of a time-major CUDA uint8 block, [nbeam][nnew][nchan] or (spliced) [nnew][nbeam][nchan];
+        whole_rows=False computes only the new tail of every row.  Returns the DM transform tensor."""
         import torch
-        nbeam, nnew, nchan = d_new.shape
+        if spliced:
+            nnew, nbeam, nchan = d_new.shape
+        else:
+            nbeam, nnew, nchan = d_new.shape
         if nchan != self.nchan or d_new.dtype != torch.uint8:
-            raise ValueError("block must be uint8 [nbeam][nnew][nchan]")
+            raise ValueError("block must be uint8 [nbeam][nnew][nchan] or [nnew][nbeam][nchan]")
         if d_dmt is None:
             d_dmt = torch.empty((nbeam, self.dmt_elems_per_beam), dtype=torch.int32, device=d_new.device)
-        _check(lib().spt_segment_push(self._h, _dev_ptr(d_new), nbeam, nnew, int(bool(flip)), _dev_ptr(d_dmt),
-                                      _stream_ptr(stream)), "spt_segment_push")
+        _check(lib().spt_segment_push(self._h, _dev_ptr(d_new), nbeam, nnew, int(bool(flip)), int(bool(spliced)),
+                                      int(bool(whole_rows)), _dev_ptr(d_dmt), _stream_ptr(stream)), "spt_segment_push")
         return d_dmt
 
     def sift(self, cands: np.ndarray, nbeam: int, eps: float = 0.5, min_pts: int = 5, time_unit_s: float = 1.0,
@@ -386,13 +390,17 @@ def delta_dm(width_s: float, nu_mhz: float, bw_mhz: float, snr_ratio: float = 0.
     return float(lib().spt_delta_dm(width_s, snr_ratio, nu_mhz, bw_mhz))
 
 
-def corner_turn(d_in, flip: bool = False, stream=None):
-    """Time-major CUDA uint8 [nbeam][nsamp][nchan] -> channel-major [nbeam][nchan][nsamp] (optionally band-flipped)."""
+def corner_turn(d_in, flip: bool = False, stream=None, spliced: bool = False):
+    """Time-major CUDA uint8 [nbeam][nsamp][nchan] (spliced: [nsamp][nbeam][nchan]) -> channel-major [nbeam][nchan][nsamp]
+    (optionally band-flipped)."""
     import torch
-    nbeam, nsamp, nchan = d_in.shape
+    if spliced:
+        nsamp, nbeam, nchan = d_in.shape
+    else:
+        nbeam, nsamp, nchan = d_in.shape
     out = torch.empty((nbeam, nchan, nsamp), dtype=torch.uint8, device=d_in.device)
-    _check(lib().spt_corner_turn(_dev_ptr(d_in), nbeam, nsamp, nchan, int(bool(flip)), _dev_ptr(out), _stream_ptr(stream)),
-           "spt_corner_turn")
+    _check(lib().spt_corner_turn(_dev_ptr(d_in), nbeam, nsamp, nchan, int(bool(flip)), int(bool(spliced)), _dev_ptr(out),
+                                 _stream_ptr(stream)), "spt_corner_turn")
     return out
 
 

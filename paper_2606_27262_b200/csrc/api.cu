@@ -47,6 +47,8 @@ struct DeviceState {
     // nsamp samples of every channel row
     uint8_t* work[2] = {nullptr, nullptr};
     int work_cur = 0;
+    cudaStream_t hist_stream = nullptr;  // the history copy of a push runs beside the corner turn of the new block
+    cudaEvent_t hist_fork = nullptr, hist_join = nullptr;
     int32_t* win_len = nullptr;     // [ntrials] search window of a segment and the start positions it reports,
     int32_t* win_starts = nullptr;  // for the segment length win_nnew
     int64_t win_nnew = -1;
@@ -151,6 +153,9 @@ static void free_device(Plan* p) {
         if (sl.done) cudaEventDestroy(sl.done);
     }
     cudaFree(d->fb_pad); cudaFree(d->h_fb); cudaFree(d->h_dmt);
+    if (d->hist_stream) cudaStreamDestroy(d->hist_stream);
+    if (d->hist_fork) cudaEventDestroy(d->hist_fork);
+    if (d->hist_join) cudaEventDestroy(d->hist_join);
     if (d->own_stream) cudaStreamDestroy(d->own_stream);
     if (d->copy_stream) cudaStreamDestroy(d->copy_stream);
     for (int i = 0; i < 2; ++i) { if (d->side[i]) cudaStreamDestroy(d->side[i]); if (d->join[i]) cudaEventDestroy(d->join[i]); }
@@ -230,8 +235,10 @@ static int ensure_device(Plan* p) {
 
 // defer_join: leave the side streams un-joined (d->side_pending says which carry work); the caller -- do_search with
 // per_range = true, directly afterwards -- enqueues every range's search behind its dedispersion and joins then.
+// tail_raw > 0 (a pushed stream segment of that many new raw samples): only the last tail_raw/decim + wmax - 1 outputs of
+// every row are computed -- the window spt_segment_search reads -- and the rest of d_dmt is left alone.
 static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d_dmt, cudaStream_t st,
-                         bool defer_join = false) {
+                         bool defer_join = false, int64_t tail_raw = 0) {
     DeviceState* d = p->dev;
     const uint8_t* in = d_fb;
     int64_t in_stride = p->nsamp;
@@ -314,9 +321,23 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
             else launch_dedisp_naive<uint8_t>((const uint8_t*)src, rs, (int64_t)p->nchan * rs, rd.delay, nout, off,
                                               p->nchan, rp.ndm, nbeam, rp.max_nout, d_dmt, p->dmt_elems, st);
         } else {
+            int32_t tail = 0, tail_tiles = 0;
+            if (tail_raw > 0) {
+                // time tiles per DM tile, counted back from its last one, that hold the tail of some trial of the tile
+                tail = (int32_t)std::min<int64_t>(tail_raw / rp.decim + p->widths.back() - 1, rp.max_nout);
+                for (const TileDesc& td : rp.tiles) {
+                    int32_t first = INT32_MAX;
+                    for (int t = 0; t < td.ntrial; ++t) {
+                        const int32_t n = rp.nout[td.trial0 + t];
+                        if (n > 0) first = std::min(first, (std::max(0, n - tail) + rp.skew[(size_t)td.skew0 + t]) / kTT);
+                    }
+                    if (td.tt_last >= 0 && first != INT32_MAX) tail_tiles = std::max(tail_tiles, td.tt_last - first + 1);
+                }
+                if (tail_tiles <= 0) continue;
+            }
             const int rc = launch_dedisp_tiled(u16, p->opt_dm_tile, rp.max_ent, src, rs, (int64_t)p->nchan * rs, d_dmt, p->dmt_elems,
                                                rd.tiles, rd.sidx, rd.rows, rd.blob, d->maxval + 2 * i, rd.skew, rp.skew_max, rp.vcap_words, nout, off,
-                                               (int32_t)rp.tiles.size(), rp.ntile_t, nbeam, st);
+                                               (int32_t)rp.tiles.size(), rp.ntile_t, nbeam, tail, tail_tiles, st);
             if (rc != 0) { g_last_error = "dedisp_tiled: launch configuration rejected"; return SPT_ERR_CUDA; }
         }
         p->launches++;
@@ -955,10 +976,11 @@ int spt_peaks_read(spt_plan* plan, spt_candidate* host_out, int64_t cap, int64_t
     return SPT_OK;
 }
 
-int spt_corner_turn(const uint8_t* d_in, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip, uint8_t* d_out,
-                    void* cuda_stream) {
-    if (!d_in || !d_out || nbeam < 1 || nsamp < 1 || nchan < 1 || (flip != 0 && flip != 1)) return SPT_ERR_INVALID;
-    launch_corner_turn(d_in, nbeam, nsamp, nchan, flip, d_out, nsamp, (int64_t)nchan * nsamp, 0, (cudaStream_t)cuda_stream);
+int spt_corner_turn(const uint8_t* d_in, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip, int32_t spliced,
+                    uint8_t* d_out, void* cuda_stream) {
+    if (!d_in || !d_out || nbeam < 1 || nsamp < 1 || nchan < 1 || (flip != 0 && flip != 1) || (spliced != 0 && spliced != 1))
+        return SPT_ERR_INVALID;
+    launch_corner_turn(d_in, nbeam, nsamp, nchan, flip, spliced, d_out, nsamp, (int64_t)nchan * nsamp, 0, (cudaStream_t)cuda_stream);
     SPT_CUDA(cudaGetLastError());
     return SPT_OK;
 }
@@ -1014,9 +1036,11 @@ int spt_segment_search(spt_plan* plan, const int32_t* d_dmt, int32_t nbeam, int6
     return do_search(&p, d_dmt, nbeam, threshold, (cudaStream_t)cuda_stream, 0, true);
 }
 
-int spt_segment_push(spt_plan* plan, const uint8_t* d_new, int32_t nbeam, int64_t nnew, int32_t flip, int32_t* d_dmt,
-                     void* cuda_stream) {
-    if (!plan || !d_new || !d_dmt || nbeam < 1 || nbeam > plan->p.max_beams || (flip != 0 && flip != 1)) return SPT_ERR_INVALID;
+int spt_segment_push(spt_plan* plan, const uint8_t* d_new, int32_t nbeam, int64_t nnew, int32_t flip, int32_t spliced,
+                     int32_t whole_rows, int32_t* d_dmt, void* cuda_stream) {
+    if (!plan || !d_new || !d_dmt || nbeam < 1 || nbeam > plan->p.max_beams || (flip != 0 && flip != 1) ||
+        (spliced != 0 && spliced != 1) || (whole_rows != 0 && whole_rows != 1))
+        return SPT_ERR_INVALID;
     if ((reinterpret_cast<uintptr_t>(d_dmt) & 127) != 0) return SPT_ERR_INVALID;
     Plan& p = plan->p;
     int64_t hmin = 0, gran = 16;
@@ -1044,12 +1068,25 @@ int spt_segment_push(spt_plan* plan, const uint8_t* d_new, int32_t nbeam, int64_
     const uint8_t* prev = d->work[d->work_cur];
     uint8_t* cur = d->work[d->work_cur ^ 1];
     const int64_t keep = p.nsamp - nnew;
-    launch_keep_history(prev, cur, p.nsamp, nnew, keep, (int64_t)nbeam * p.nchan, st);
-    launch_corner_turn(d_new, nbeam, nnew, p.nchan, flip, cur, p.nsamp, (int64_t)p.nchan * p.nsamp, keep, st);
+    // the history moves to the front of the other buffer on a side stream while the new block is corner-turned into its
+    // tail on the caller's: the two write disjoint parts of the buffer
+    if (keep > 0) {
+        if (!d->hist_stream) {
+            SPT_CUDA(cudaStreamCreateWithFlags(&d->hist_stream, cudaStreamNonBlocking));
+            SPT_CUDA(cudaEventCreateWithFlags(&d->hist_fork, cudaEventDisableTiming));
+            SPT_CUDA(cudaEventCreateWithFlags(&d->hist_join, cudaEventDisableTiming));
+        }
+        SPT_CUDA(cudaEventRecord(d->hist_fork, st));
+        SPT_CUDA(cudaStreamWaitEvent(d->hist_stream, d->hist_fork, 0));
+        launch_keep_history(prev, cur, p.nsamp, nnew, keep, (int64_t)nbeam * p.nchan, d->hist_stream);
+        SPT_CUDA(cudaEventRecord(d->hist_join, d->hist_stream));
+    }
+    launch_corner_turn(d_new, nbeam, nnew, p.nchan, flip, spliced, cur, p.nsamp, (int64_t)p.nchan * p.nsamp, keep, st);
+    if (keep > 0) SPT_CUDA(cudaStreamWaitEvent(st, d->hist_join, 0));
     p.launches += keep > 0 ? 2 : 1;
     SPT_CUDA(cudaGetLastError());
     d->work_cur ^= 1;
-    return do_dedisperse(&p, cur, nbeam, d_dmt, st);
+    return do_dedisperse(&p, cur, nbeam, d_dmt, st, false, whole_rows ? 0 : nnew);
 }
 
 int spt_sift(spt_plan* plan, const spt_candidate* h_in, int64_t n, int32_t nbeam, const spt_sift_params* prm,

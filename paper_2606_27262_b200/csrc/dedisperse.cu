@@ -195,6 +195,8 @@ struct TiledArgs {
     const int32_t* nout;       // range local
     const int64_t* offset;     // range local
     int32_t vcap_words, ntile_dm, ntile_t, nbeam;
+    int32_t tail;              // > 0: only the last `tail` outputs of every row are computed (a pushed stream segment) ...
+    int32_t tail_tiles;        // ... by this many time tiles per DM tile, counted back from the tile's last one
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -373,9 +375,11 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     int bid = blockIdx.x;
     const int dmt = bid % a.ntile_dm; bid /= a.ntile_dm;
-    const int beam = bid / a.ntile_t;
+    const int ntt = a.tail > 0 ? a.tail_tiles : a.ntile_t;
+    const int beam = bid / ntt;
     const TileDesc td = a.tiles[dmt];
-    const int tt = (bid % a.ntile_t + a.ntile_t - td.tshift % a.ntile_t) % a.ntile_t;
+    const int tt = a.tail > 0 ? td.tt_last - bid % ntt : (bid % ntt + ntt - td.tshift % ntt) % ntt;
+    if (tt < 0) return;
     const int64_t t0 = (int64_t)tt * kTT;   // trial i of the tile computes the outputs t0 - skew[i] + [0, kTT)
 
     const T* in = reinterpret_cast<const T*>(a.in) + (int64_t)beam * a.beam_stride;
@@ -429,7 +433,9 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
         const int d = td.trial0 + (tid < td.ntrial ? tid : td.ntrial - 1);
         const int64_t first = t0 - a.skew[td.skew0 + tid];                 // output sample of accumulator index 0
         s_rowp[tid] = a.out + (int64_t)beam * a.out_beam_stride + a.offset[d] + first;
-        const int lo = (int)min((int64_t)kTT, max((int64_t)0, -first));
+        // first valid output of the trial in this tile: the start of the row, or of the tail that is wanted
+        const int64_t want = a.tail > 0 ? max((int64_t)0, (int64_t)a.nout[d] - a.tail) : 0;
+        const int lo = (int)min((int64_t)kTT, max((int64_t)0, want - first));
         const int hi = tid < td.ntrial ? (int)min((int64_t)kTT, max((int64_t)lo, (int64_t)a.nout[d] - first)) : lo;
         s_valid[tid] = make_int2(lo, hi);
         have = hi > lo;
@@ -564,7 +570,7 @@ static int launch_tiled_inst(const TiledArgs& a, cudaStream_t st) {
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes) != cudaSuccess) return -1;
         if (dev >= 0 && dev < kMaxDev) attr_set[dev].store(true, std::memory_order_release);
     }
-    const int64_t nblocks = (int64_t)a.ntile_dm * a.ntile_t * a.nbeam;
+    const int64_t nblocks = (int64_t)a.ntile_dm * (a.tail > 0 ? a.tail_tiles : a.ntile_t) * a.nbeam;
     if (nblocks <= 0) return 0;
     if (nblocks > 0x7fffffffLL) return -1;
     kern<<<(unsigned)nblocks, kThreads, kSmemBytes, st>>>(a);
@@ -579,9 +585,10 @@ static int launch_tiled_type(bool is_u16, const TiledArgs& a, cudaStream_t st) {
 int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
                         int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
                         const uint32_t* blob, const uint32_t* maxval, const int32_t* skew, int32_t skew_max, int32_t vcap_words,
-                        const int32_t* nout, const int64_t* offset, int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, cudaStream_t st) {
+                        const int32_t* nout, const int64_t* offset, int32_t ntile_dm, int32_t ntile_t, int32_t nbeam,
+                        int32_t tail, int32_t tail_tiles, cudaStream_t st) {
     TiledArgs a{in, row_stride, beam_stride, out, out_beam_stride, tiles, sidx, rows, blob, maxval, skew, skew_max, nout, offset,
-                vcap_words, ntile_dm, ntile_t, nbeam};
+                vcap_words, ntile_dm, ntile_t, nbeam, tail, tail_tiles};
     if (DT == 64 && max_ent == 8) return launch_tiled_type<64, 8>(is_u16, a, st);
     if (DT == 64 && max_ent == 12) return launch_tiled_type<64, 12>(is_u16, a, st);
     if (DT == 64 && max_ent == 16) return launch_tiled_type<64, 16>(is_u16, a, st);

@@ -82,7 +82,8 @@ struct TileDesc {           // one DM tile of a range
     int32_t skew0;          // first entry of the tile's DT per-trial output skews (RangePlan::skew)
     int32_t tshift;         // the block with time index i works on time tile (i - tshift) mod ntile_t: DM tiles that run
                             // together then read about the same stretch of the input (their delays differ)
-    int32_t pad_[2];
+    int32_t tt_last;        // last time tile in which some trial of the tile has a valid output (-1: none)
+    int32_t pad_;
 };
 
 struct RangePlan {

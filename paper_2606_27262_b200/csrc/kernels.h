@@ -24,7 +24,7 @@ int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, const void* in, int64_
                         int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
                         const uint32_t* blob, const uint32_t* maxval, const int32_t* skew, int32_t skew_max, int32_t vcap_words,
                         const int32_t* nout, const int64_t* offset,
-                        int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, cudaStream_t st);
+                        int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, int32_t tail, int32_t tail_tiles, cudaStream_t st);
 
 struct SpsArgs {
     const int32_t* dmt;
@@ -61,8 +61,8 @@ void launch_peaks_stencil(const PeakArgs& a, int32_t window, const uint8_t* aliv
 void launch_peaks_compact(const PeakArgs& a, const uint8_t* alive, spt_candidate* out, unsigned long long* out_count,
                           long long out_capacity, cudaStream_t st);
 
-void launch_corner_turn(const uint8_t* in, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip, uint8_t* out,
-                        int64_t out_row_stride, int64_t out_beam_stride, int64_t out_t0, cudaStream_t st);
+void launch_corner_turn(const uint8_t* in, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip, int32_t spliced,
+                        uint8_t* out, int64_t out_row_stride, int64_t out_beam_stride, int64_t out_t0, cudaStream_t st);
 void launch_keep_history(const uint8_t* src, uint8_t* dst, int64_t row_bytes, int64_t shift_bytes, int64_t keep_bytes,
                          int64_t nrows, cudaStream_t st);
 

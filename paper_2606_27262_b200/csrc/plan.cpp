@@ -279,6 +279,10 @@ static int build_range(const Plan& p, RangePlan& rp, const int G, const int max_
             td.trial0 = d0;
             td.ntrial = std::min(DT, rp.ndm - d0);
             td.tshift = rp.delay[(size_t)(d0 + td.ntrial / 2) * p.nchan + p.nchan / 2] / kTT;   // median delay over the channels
+            td.tt_last = -1;
+            for (int i = 0; i < td.ntrial; ++i)
+                if (rp.nout[d0 + i] > 0)
+                    td.tt_last = std::max(td.tt_last, (rp.nout[d0 + i] - 1 + rp.skew[(size_t)td.skew0 + i]) / kTT);
             td.stage0 = (int32_t)rp.sidx.size();
             std::vector<PendingGroup> open;
             auto blob_words_of = [&](const std::vector<PendingGroup>& gs, const PendingGroup* extra) {

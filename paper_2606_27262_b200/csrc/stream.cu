@@ -12,14 +12,17 @@ namespace spt {
 
 // out[b][c'][t0 + t] = in[b][t][c],  c' = flip ? nchan-1-c : c.  Tile: 64 samples x 128 channels through shared memory;
 // loads are 128-byte rows of channels, stores are 64-byte runs of samples.
+// The input is addressed as in[b*in_beam_stride + t*in_t_stride + c]: a block per beam ([beam][t][chan]: strides nsamp*nchan
+// and nchan) or time-spliced over the beams ([t][beam][chan]: strides nchan and nbeam*nchan).
 __global__ void __launch_bounds__(256) corner_turn_kernel(const uint8_t* __restrict__ in, int64_t nsamp, int32_t nchan,
+                                                          int64_t in_beam_stride, int64_t in_t_stride,
                                                           int32_t flip, uint8_t* __restrict__ out, int64_t out_row_stride,
                                                           int64_t out_beam_stride, int64_t out_t0) {
     __shared__ uint8_t tile[128][64 + 4];                 // [channel][sample], padded rows
     const int b = blockIdx.z;
     const int64_t t0 = (int64_t)blockIdx.x * 64;
     const int c0 = blockIdx.y * 128;
-    const uint8_t* src = in + (int64_t)b * nsamp * nchan;
+    const uint8_t* src = in + (int64_t)b * in_beam_stride;
     const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;          // 32 x 8
     // load: one warp reads 128 consecutive channels of one sample (4 per lane)
     for (int i = ty; i < 64; i += 8) {
@@ -27,7 +30,7 @@ __global__ void __launch_bounds__(256) corner_turn_kernel(const uint8_t* __restr
         const int c = c0 + 4 * tx;
         uint32_t v = 0;
         if (t < nsamp) {
-            const uint8_t* p = src + t * nchan + c;
+            const uint8_t* p = src + t * in_t_stride + c;
             if (c + 4 <= nchan && ((reinterpret_cast<uintptr_t>(p) & 3) == 0)) v = *reinterpret_cast<const uint32_t*>(p);
             else
                 for (int k = 0; k < 4; ++k)
@@ -55,11 +58,14 @@ __global__ void __launch_bounds__(256) corner_turn_kernel(const uint8_t* __restr
     }
 }
 
-void launch_corner_turn(const uint8_t* in, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip, uint8_t* out,
-                        int64_t out_row_stride, int64_t out_beam_stride, int64_t out_t0, cudaStream_t st) {
+void launch_corner_turn(const uint8_t* in, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip, int32_t spliced,
+                        uint8_t* out, int64_t out_row_stride, int64_t out_beam_stride, int64_t out_t0, cudaStream_t st) {
     if (nbeam <= 0 || nsamp <= 0 || nchan <= 0) return;
     dim3 grid((unsigned)((nsamp + 63) / 64), (unsigned)((nchan + 127) / 128), (unsigned)nbeam);
-    corner_turn_kernel<<<grid, 256, 0, st>>>(in, nsamp, nchan, flip, out, out_row_stride, out_beam_stride, out_t0);
+    const int64_t beam_stride = spliced ? (int64_t)nchan : nsamp * (int64_t)nchan;
+    const int64_t t_stride = spliced ? (int64_t)nbeam * nchan : (int64_t)nchan;
+    corner_turn_kernel<<<grid, 256, 0, st>>>(in, nsamp, nchan, beam_stride, t_stride, flip, out, out_row_stride, out_beam_stride,
+                                             out_t0);
 }
 
 // dst[row][0 .. nkeep) = src[row][shift .. shift + nkeep): the history of every channel row moves to the front of the

@@ -19,6 +19,52 @@ def test_corner_turn(cuda, api, orc, shape, flip):
         assert np.array_equal(got[b], orc.corner_turn(x[b], flip))
 
 
+@pytest.mark.parametrize("shape,flip", [((1000, 3, 71), True), ((64, 2, 4096), False), ((7, 5, 5), False)])
+def test_corner_turn_time_spliced(cuda, api, orc, shape, flip):
+    """The rings' layout: [t][beam][chan], the beams of a host interleaved sample by sample."""
+    rs = np.random.default_rng(sum(shape) + 1)
+    x = rs.integers(0, 256, size=shape, dtype=np.uint8)
+    got = api.corner_turn(cuda.from_numpy(x).cuda(), flip, spliced=True).cpu().numpy()
+    for b, exp in enumerate(orc.corner_turn_spliced(x, flip)):
+        assert np.array_equal(got[b], exp)
+
+
+def test_incremental_push_computes_only_the_new_tail(cuda, api, orc):
+    """whole_rows = 0 with time-spliced input: after every push the last nnew/k + wmax - 1 outputs of every row equal the
+    oracle's dedispersion of the stream buffer, and nothing else in the DM transform buffer is touched."""
+    nchan, nnew, nbeam = 256, 2048, 2
+    widths = [1, 2, 4, 16]
+    w = Shape(500.0, -200.0 / nchan, nchan, 0, [(0.0, 0.2, 70, 1), (10.0, 0.5, 40, 2), (30.0, 1.0, 33, 4)], widths, 6.0, nbeam=nbeam)
+    probe = api.Plan(w.fch1, w.foff, nchan, w.tsamp, 1 << 16, w.ranges, w.widths)
+    _, hsearch, _ = probe.segment_info()
+    w.nsamp = hsearch + nnew + 1024                                 # rows longer than the tail: there is something to leave alone
+    rs = np.random.default_rng(10)
+    blocks = [rs.integers(0, 256, size=(nnew, nbeam, nchan), dtype=np.uint8) for _ in range(3)]   # [t][beam][chan]
+    plan = make_plan(api, w, nbeam=nbeam)
+    refs = [orc.overlap_save_buffers([blk[:, b, :] for blk in blocks], w.nsamp, flip=True) for b in range(nbeam)]
+    _, _, dec, nout, off = plan.trial_table()
+    SENT = -123456789
+    for i, blk in enumerate(blocks):
+        d_dmt = cuda.full((nbeam, plan.dmt_elems_per_beam), SENT, dtype=cuda.int32, device="cuda")
+        plan.segment_push(cuda.from_numpy(blk).cuda(), flip=True, d_dmt=d_dmt, spliced=True, whole_rows=False)
+        dmt = d_dmt.cpu().numpy()
+        untouched = 0
+        for b in range(nbeam):
+            ref = oracle_path(orc, w, refs[b][i], search=False)
+            d = 0
+            for rr in ref:
+                for j in range(len(rr.nout)):
+                    n, k = int(nout[d]), int(dec[d])
+                    tail = min(n, nnew // k + max(widths) - 1)
+                    got = dmt[b][off[d]: off[d] + n]
+                    exp = rr.dmt[rr.rowoff[j]: rr.rowoff[j + 1]]
+                    assert np.array_equal(got[n - tail:], exp[n - tail:]), (i, b, d)
+                    assert np.all(got[: n - tail] == SENT), (i, b, d)          # not a single output before the tail
+                    untouched += n - tail
+                    d += 1
+        assert untouched > 100000
+
+
 def test_overlap_save_segments(cuda, api, orc):
     nchan, nnew = 256, 2048
     w = Shape(500.0, -200.0 / nchan, nchan, 0, [(0.0, 0.2, 70, 1), (10.0, 0.5, 40, 2), (30.0, 1.0, 33, 4)], [1, 2, 4], 6.0, nbeam=2)
@@ -54,7 +100,8 @@ def test_overlap_save_segments(cuda, api, orc):
     assert e.value.code == api.SPT_ERR_INVALID
 
 
-def test_segment_search_matches_the_oracle_window(cuda, api, orc):
+@pytest.mark.parametrize("whole_rows", [True, False])
+def test_segment_search_matches_the_oracle_window(cuda, api, orc, whole_rows):
     """spt_segment_search after every push: per trial, statistics and candidates of the window (last nnew/k + wmax - 1
     samples) restricted to its first nnew/k start positions, against the oracle's composition of C1-C5 on that window."""
     nchan, nnew = 128, 4096
@@ -71,10 +118,11 @@ def test_segment_search_matches_the_oracle_window(cuda, api, orc):
     rs = np.random.default_rng(21)
     _, _, dec, nout, off = plan.trial_table()
     total = 0
+    d_dmt = cuda.zeros((1, plan.dmt_elems_per_beam), dtype=cuda.int32, device="cuda")
     for i in range(3):
         blk = rs.normal(128, 12, size=(1, nnew, nchan)).round().clip(0, 255).astype(np.uint8)
         blk[0, 1000 + 300 * i: 1003 + 300 * i, :] += 20            # a zero-DM spike per segment
-        d_dmt = plan.segment_push(cuda.from_numpy(blk).cuda())
+        d_dmt = plan.segment_push(cuda.from_numpy(blk).cuda(), d_dmt=d_dmt, whole_rows=whole_rows)
         plan.segment_search(d_dmt, nnew, w.threshold)
         n, ovf = plan.candidates_count()
         assert not ovf
@@ -85,7 +133,7 @@ def test_segment_search_matches_the_oracle_window(cuda, api, orc):
         for c in cands:
             got.setdefault(int(c["trial"]), []).append((int(c["t"]), int(c["width"]), float(c["snr"])))
         for d in range(plan.ntrials):
-            row = dmt[off[d]: off[d] + nout[d]]
+            row = dmt[off[d]: off[d] + nout[d]]     # (whole_rows = False: only its tail, the window, is defined)
             sx, sxx, t, bw, snr = orc.search_segment(row, widths, w.threshold, nnew // int(dec[d]))
             assert (int(s_all[0, d]), int(q_all[0, d])) == (sx, sxx), d
             g = sorted(got.get(d, []))

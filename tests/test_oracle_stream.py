@@ -9,6 +9,14 @@ def test_corner_turn_worked_example(orc):
     assert orc.corner_turn(x, flip=True).tolist() == [[3, 6], [2, 5], [1, 4]]   # last channel (highest frequency) first
 
 
+def test_corner_turn_spliced_worked_example(orc):
+    # 2 samples x 2 beams x 3 channels, time-spliced: sample 0 of beam 0, sample 0 of beam 1, sample 1 of beam 0, ...
+    x = np.array([[[1, 2, 3], [11, 12, 13]], [[4, 5, 6], [14, 15, 16]]], dtype=np.uint8)
+    b0, b1 = orc.corner_turn_spliced(x)
+    assert b0.tolist() == [[1, 4], [2, 5], [3, 6]] and b1.tolist() == [[11, 14], [12, 15], [13, 16]]
+    assert orc.corner_turn_spliced(x, flip=True)[1].tolist() == [[13, 16], [12, 15], [11, 14]]
+
+
 def test_overlap_save_buffers_worked_example(orc):
     b0 = np.array([[1, 10], [2, 20]], dtype=np.uint8)                    # 2 new samples x 2 channels per push
     b1 = np.array([[3, 30], [4, 40]], dtype=np.uint8)
