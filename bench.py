@@ -657,6 +657,52 @@ def run_stream(args, local_rank):
     print(json.dumps(out), flush=True)
 
 
+def run_cutouts(args, local_rank):
+    """NEXT-4 timed: the classifier's two 256 x 256 features for a batch of 64 candidates on the
+    config-3 beam (4096 channels), DM ranges from Eq. 4 as printed -- ms per candidate, against one call per candidate."""
+    import numpy as np
+    import torch
+
+    from paper_2606_27262_b200 import api, build, synth
+    build.build()
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    w = synth.workload(3)
+    d_fb = torch.from_numpy(synth.generate(w)).cuda()[None]
+    rs = np.random.default_rng(0)
+    ncand, ndm, nt, nf = 64, 256, 256, 256
+    cands = []
+    for _ in range(ncand):
+        width_s = float(np.exp(rs.uniform(np.log(1e-3), np.log(20e-3))))
+        dm0 = float(rs.uniform(20.0, 1900.0))
+        ddm = min(dm0, api.delta_dm(width_s, 400.0, 200.0))               # Eq. 4 (PAPER.md:244), ratio 0.1
+        cands.append((dm0, ddm, int(rs.integers(0, w.nsamp - 70000)), 1, 0))
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, reps):
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(reps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) / reps
+
+    ms_batch = timed(lambda: api.cutout_batch(d_fb, w.fch1, w.foff, w.tsamp, cands, ndm, nt, nf, stream), 5)
+    ms_single = timed(lambda: [api.cutout(d_fb[0], w.fch1, w.foff, w.tsamp, c[0], c[1], ndm, c[2], 1, nt, nf, stream) for c in cands[:8]], 3) / 8
+    adds = ncand * (ndm * nt * w.nchan + nt * w.nchan)
+    # bytes a candidate must read at least: every channel's window once per 32-trial group is the kernel's traffic; the
+    # compulsory figure is one window per channel
+    out = {"cutouts": {"ncand": ncand, "shape": [ndm, nt, nf], "nchan": w.nchan, "tbin": 1,
+                       "ms_per_candidate_batch": ms_batch / ncand, "ms_per_candidate_single_calls": ms_single,
+                       "adds_per_s": adds / (ms_batch * 1e-3), "api": "spt_cutout_batch (one launch of 64)",
+                       "mean_ddm": float(np.mean([c[1] for c in cands]))}}
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -671,6 +717,7 @@ def main():
     ap.add_argument("--no-worst-case", action="store_true")
     ap.add_argument("--all-configs", action="store_true")
     ap.add_argument("--stream", action="store_true")
+    ap.add_argument("--cutouts", action="store_true")
     ap.add_argument("--two-calls", action="store_true", help="step = spt_dedisperse + spt_single_pulse_search instead of spt_search")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -682,6 +729,8 @@ def main():
         run_all_configs(args, local_rank)
     elif args.stream:
         run_stream(args, local_rank)
+    elif args.cutouts:
+        run_cutouts(args, local_rank)
     else:
         run_ours(args, rank, world, local_rank)
 

@@ -312,6 +312,22 @@ int spt_sift(spt_plan* plan, const spt_candidate* h_in /*HOST*/, int64_t n, int3
 int spt_cutout(const uint8_t* d_fb /*DEVICE*/, int32_t nchan, int64_t nsamp, double fch1_mhz, double foff_mhz, double tsamp_s,
                double dm0, double ddm, int32_t ndm, int64_t ts, int32_t tbin, int32_t nt, int32_t nf,
                int32_t* d_dds /*DEVICE*/, int32_t* d_dmt /*DEVICE*/, void* cuda_stream);
+/* spt_cutout_batch -- the same two features for MANY candidates in one launch (10 to 100 candidates per beam
+ * per block reach this stage; "custom, optimised GPU kernels").  d_fb: DEVICE uint8 [nbeam][nchan][nsamp];
+ * h_cands: HOST array of ncand records {dm0, ddm, ts, tbin, beam}; ndm, nt, nf are common to the batch (the classifier's
+ * input shape).  Outputs, DEVICE int32: d_dds [ncand][nf][nt], d_dmt [ncand][ndm][nt], candidate k at index k.  Same
+ * definitions, argument checks and error codes as spt_cutout (which is a batch of one).  The records are copied into the
+ * launch: h_cands may be reused as soon as the call returns.  Enqueues on cuda_stream; allocates nothing. */
+typedef struct {
+    double dm0;     /* the candidate's DM, pc cm^-3 */
+    double ddm;     /* half-width of the DM range of the narrow DM transform (Eq. 4: spt_delta_dm) */
+    int64_t ts;     /* first raw sample of the window at the top of the band (may be negative) */
+    int32_t tbin;   /* raw samples per time bin, >= 1 */
+    int32_t beam;   /* which beam of d_fb */
+} spt_cutout_params;
+int spt_cutout_batch(const uint8_t* d_fb /*DEVICE*/, int32_t nbeam, int32_t nchan, int64_t nsamp, double fch1_mhz, double foff_mhz,
+                     double tsamp_s, const spt_cutout_params* h_cands /*HOST*/, int32_t ncand, int32_t ndm, int32_t nt, int32_t nf,
+                     int32_t* d_dds /*DEVICE*/, int32_t* d_dmt /*DEVICE*/, void* cuda_stream);
 double spt_delta_dm(double width_s, double snr_ratio, double nu_mhz, double bw_mhz);
 
 /* With option "profile" = 1: device time (ms) of each kernel launched by the LAST spt_dedisperse and the LAST

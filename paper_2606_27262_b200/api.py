@@ -29,6 +29,11 @@ class spt_candidate(ctypes.Structure):
                 ("width", ctypes.c_int32), ("snr", ctypes.c_float)]
 
 
+class spt_cutout_params(ctypes.Structure):
+    _fields_ = [("dm0", ctypes.c_double), ("ddm", ctypes.c_double), ("ts", ctypes.c_int64), ("tbin", ctypes.c_int32),
+                ("beam", ctypes.c_int32)]
+
+
 class spt_sift_params(ctypes.Structure):
     _fields_ = [("eps", ctypes.c_double), ("time_unit_s", ctypes.c_double), ("dm_unit", ctypes.c_double),
                 ("min_pts", ctypes.c_int32), ("snr_min", ctypes.c_float), ("dm_min", ctypes.c_double),
@@ -71,6 +76,8 @@ SYMBOLS = {
     "spt_segment_search": (ctypes.c_int, [_vp, _vp, _i32, _i64, _f32, _vp]),
     "spt_segment_push": (ctypes.c_int, [_vp, _vp, _i32, _i64, _i32, _i32, _i32, _vp, _vp]),
     "spt_cutout": (ctypes.c_int, [_vp, _i32, _i64, _f64, _f64, _f64, _f64, _f64, _i32, _i64, _i32, _i32, _i32, _vp, _vp, _vp]),
+    "spt_cutout_batch": (ctypes.c_int, [_vp, _i32, _i32, _i64, _f64, _f64, _f64, _P(spt_cutout_params), _i32, _i32, _i32, _i32, _vp,
+                                        _vp, _vp]),
     "spt_delta_dm": (_f64, [_f64, _f64, _f64, _f64]),
     "spt_sift": (ctypes.c_int, [_vp, _vp, _i64, _i32, _P(spt_sift_params), _vp, _i64, _P(_i64), _P(_i64)]),
     "spt_stream_push": (ctypes.c_int, [_vp, _vp, _i32, _f32]),
@@ -383,6 +390,22 @@ def cutout(d_fb, fch1: float, foff: float, tsamp: float, dm0: float, ddm: float,
     dmt = torch.empty((ndm, nt), dtype=torch.int32, device=d_fb.device)
     _check(lib().spt_cutout(_dev_ptr(d_fb), nchan, nsamp, fch1, foff, tsamp, dm0, ddm, ndm, ts, tbin, nt, nf, _dev_ptr(dds),
                             _dev_ptr(dmt), _stream_ptr(stream)), "spt_cutout")
+    return dds, dmt
+
+
+def cutout_batch(d_fb, fch1: float, foff: float, tsamp: float, cands, ndm: int, nt: int, nf: int, stream=None):
+    """The cut-outs of many candidates in one launch.  d_fb: CUDA uint8 [nbeam][nchan][nsamp]; cands: sequence of
+    (dm0, ddm, ts, tbin, beam).  Returns (dds [ncand][nf][nt], dmt [ncand][ndm][nt]) int32 CUDA tensors."""
+    import torch
+    if d_fb.dim() == 2:
+        d_fb = d_fb.unsqueeze(0)
+    nbeam, nchan, nsamp = d_fb.shape
+    n = len(cands)
+    arr = (spt_cutout_params * n)(*[spt_cutout_params(float(a), float(b), int(c), int(d), int(e)) for a, b, c, d, e in cands])
+    dds = torch.empty((n, nf, nt), dtype=torch.int32, device=d_fb.device)
+    dmt = torch.empty((n, ndm, nt), dtype=torch.int32, device=d_fb.device)
+    _check(lib().spt_cutout_batch(_dev_ptr(d_fb), nbeam, nchan, nsamp, fch1, foff, tsamp, arr, n, ndm, nt, nf, _dev_ptr(dds),
+                                  _dev_ptr(dmt), _stream_ptr(stream)), "spt_cutout_batch")
     return dds, dmt
 
 

@@ -1180,22 +1180,57 @@ int spt_sift(spt_plan* plan, const spt_candidate* h_in, int64_t n, int32_t nbeam
     return SPT_OK;
 }
 
-int spt_cutout(const uint8_t* d_fb, int32_t nchan, int64_t nsamp, double fch1_mhz, double foff_mhz, double tsamp_s, double dm0,
-               double ddm, int32_t ndm, int64_t ts, int32_t tbin, int32_t nt, int32_t nf, int32_t* d_dds, int32_t* d_dmt,
-               void* cuda_stream) {
-    if (!d_fb || !d_dds || !d_dmt || nchan < 1 || nsamp < 1 || ndm < 1 || tbin < 1 || nt < 1 || nf < 1 || nchan % nf != 0 ||
-        !(tsamp_s > 0.0) || !(fch1_mhz > 0.0) || !(dm0 >= 0.0) || !(ddm >= 0.0))
+int spt_cutout_batch(const uint8_t* d_fb, int32_t nbeam, int32_t nchan, int64_t nsamp, double fch1_mhz, double foff_mhz,
+                     double tsamp_s, const spt_cutout_params* h_cands, int32_t ncand, int32_t ndm, int32_t nt, int32_t nf,
+                     int32_t* d_dds, int32_t* d_dmt, void* cuda_stream) {
+    if (!d_fb || !d_dds || !d_dmt || !h_cands || ncand < 1 || nbeam < 1 || nchan < 1 || nsamp < 1 || ndm < 1 || nt < 1 || nf < 1 ||
+        nchan % nf != 0 || !(tsamp_s > 0.0) || !(fch1_mhz > 0.0))
         return SPT_ERR_INVALID;
     if (!(foff_mhz < 0.0)) return SPT_ERR_UNSUPPORTED;
     if (!(fch1_mhz + (double)(nchan - 1) * foff_mhz > 0.0)) return SPT_ERR_INVALID;
-    if ((double)nchan * 255.0 * tbin >= 2147483648.0 || ndm + nf > 65535) return SPT_ERR_UNSUPPORTED;
-    if (launch_cutout(d_fb, nchan, nsamp, fch1_mhz, foff_mhz, tsamp_s, dm0, ddm, ndm, ts, tbin, nt, nf, d_dds, d_dmt,
-                      (cudaStream_t)cuda_stream) != 0) {
-        g_last_error = "spt_cutout: launch failed";
-        cudaGetLastError();
-        return SPT_ERR_CUDA;
+    if (ndm + nf > 65535) return SPT_ERR_UNSUPPORTED;
+    for (int32_t k = 0; k < ncand; ++k) {
+        const spt_cutout_params& c = h_cands[k];
+        if (c.tbin < 1 || c.beam < 0 || c.beam >= nbeam || !(c.dm0 >= 0.0) || !(c.ddm >= 0.0)) return SPT_ERR_INVALID;
+        if ((double)nchan * 255.0 * c.tbin >= 2147483648.0) return SPT_ERR_UNSUPPORTED;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    SPT_CUDA(cudaMemsetAsync(d_dds, 0, (size_t)ncand * nf * nt * 4, st));       // the kernel adds into its outputs
+    SPT_CUDA(cudaMemsetAsync(d_dmt, 0, (size_t)ncand * ndm * nt * 4, st));
+    CutoutArgs a{};
+    a.x = d_fb; a.nsamp = nsamp; a.beam_stride = (long long)nchan * nsamp;
+    a.fch1 = fch1_mhz; a.foff = foff_mhz; a.tsamp = tsamp_s;
+    a.nchan = nchan; a.ndm = ndm; a.nt = nt; a.nf = nf;
+    a.dds = d_dds; a.dmt = d_dmt;
+    // candidates whose bins are one sample wide and the others run different kernel instances; each kind goes in launches of
+    // at most kCutoutMaxCand candidates, whose parameters travel in the kernel's parameter block
+    for (int kind = 0; kind < 2; ++kind) {
+        int32_t k = 0;
+        while (k < ncand) {
+            a.ncand = 0;
+            for (; k < ncand && a.ncand < kCutoutMaxCand; ++k) {
+                if ((h_cands[k].tbin > 1) != (kind == 1)) continue;
+                CutoutCand& c = a.cand[a.ncand++];
+                c.dm0 = h_cands[k].dm0; c.ddm = h_cands[k].ddm; c.ts = h_cands[k].ts; c.tbin = h_cands[k].tbin;
+                c.beam = h_cands[k].beam; c.out = k; c.pad_ = 0;
+            }
+            if (a.ncand == 0) continue;
+            if (launch_cutout_batch(a, st) != 0) {
+                g_last_error = "spt_cutout_batch: launch failed";
+                cudaGetLastError();
+                return SPT_ERR_CUDA;
+            }
+        }
     }
     return SPT_OK;
+}
+
+int spt_cutout(const uint8_t* d_fb, int32_t nchan, int64_t nsamp, double fch1_mhz, double foff_mhz, double tsamp_s, double dm0,
+               double ddm, int32_t ndm, int64_t ts, int32_t tbin, int32_t nt, int32_t nf, int32_t* d_dds, int32_t* d_dmt,
+               void* cuda_stream) {
+    spt_cutout_params c{};
+    c.dm0 = dm0; c.ddm = ddm; c.ts = ts; c.tbin = tbin; c.beam = 0;
+    return spt_cutout_batch(d_fb, 1, nchan, nsamp, fch1_mhz, foff_mhz, tsamp_s, &c, 1, ndm, nt, nf, d_dds, d_dmt, cuda_stream);
 }
 
 double spt_delta_dm(double width_s, double snr_ratio, double nu_mhz, double bw_mhz) {

@@ -88,9 +88,24 @@ struct SiftArgs {                   // all arrays DEVICE, n entries sorted by (b
 };
 void launch_sift(const SiftArgs& a, cudaStream_t st);
 
-int launch_cutout(const uint8_t* x, int32_t nchan, int64_t nsamp, double fch1, double foff, double tsamp, double dm0,
-                  double ddm, int32_t ndm, int64_t ts, int32_t tbin, int32_t nt, int32_t nf, int32_t* dds, int32_t* dmt,
-                  cudaStream_t st);
+constexpr int kCutoutMaxCand = 96;   // candidates per launch: they travel in the kernel's parameter block (< 4 KB)
+struct CutoutCand {
+    double dm0, ddm;
+    long long ts;
+    int32_t tbin, beam;
+    int32_t out, pad_;               // index of the candidate's outputs in dds / dmt
+};
+struct CutoutArgs {
+    const uint8_t* x;                // [nbeam][nchan][nsamp]
+    long long nsamp, beam_stride;
+    double fch1, foff, tsamp;
+    int32_t nchan, ndm, nt, nf, ncand;
+    int32_t wcap, wstride, nsub;     // set by the launcher: window capacity (elements), row stride (words), channels staged at a time
+    int32_t* dds;                    // [..][nf][nt]
+    int32_t* dmt;                    // [..][ndm][nt]
+    CutoutCand cand[kCutoutMaxCand];
+};
+int launch_cutout_batch(CutoutArgs& a, cudaStream_t st);
 
 int run_probe(int kind, int reps, double* warp_instr_per_s, double* elapsed_ms);
 
