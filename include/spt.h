@@ -99,7 +99,8 @@ int spt_plan_delays(const spt_plan* plan, int32_t trial, int32_t* host_out);
 /* Kernel-selection knobs, for A/B measurements and tests; must be set before the first spt_dedisperse.
  *   "dedisp_kernel": 0 = tiled shared-memory kernel (default, the product), 1 = one-thread-per-output kernel
  *                    reading global memory (bring-up / cross-check kernel, same results)
- *   "group":         largest pre-summed channel group of the tiled kernel: 1, 2, 4 or 8 (default)
+ *   "group":         largest pre-summed channel group of the tiled kernel in channels: 1, 2, 4, 8, 12 or 16 (default: 8, or 16
+ *                    where the cost model picks groups of 12 entries)
  *   "dm_tile":       trials per block tile (32 or 64; default 64)
  *   "skew":          1 (default) = every trial of a DM tile computes an output window shifted by its own delay at a
  *                    reference channel, which narrows the windows the tile reads; 0 = one window start per tile
@@ -108,6 +109,11 @@ int spt_plan_delays(const spt_plan* plan, int32_t trial, int32_t* host_out);
  *                    profile = 1 the DM ranges run one after the other on the caller's stream (so that each launch can
  *                    be timed alone) instead of side by side on the library's side streams; results are identical, the
  *                    step is about 3 % slower.  Leave it 0 for production and for end-to-end timing.
+ *   "max_entries":   largest pre-summed group of the tiled kernel in entries (a channel at one of its shifts): 8, 12 or 16;
+ *                    default: chosen per DM range by the cost model
+ *   "peaks_lookup":  how spt_peak_filter finds a neighbour's S/N: 0 (default) = by the density of the list, 1 = hash table
+ *                    (memory follows the list), 2 = dense plane laid out like the DM transform (at most 4 GiB: a slice of
+ *                    beams at a time), 3 = dense plane of one beam at a time; same results; may be switched at any time
  * Unknown names / values -> SPT_ERR_INVALID. */
 int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value);
 

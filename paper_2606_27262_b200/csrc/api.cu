@@ -52,8 +52,13 @@ struct DeviceState {
     int32_t* win_len = nullptr;     // [ntrials] search window of a segment and the start positions it reports,
     int32_t* win_starts = nullptr;  // for the segment length win_nnew
     int64_t win_nnew = -1;
-    // peak filter (lazily allocated): lookup plane laid out like the DM transform, live flags, peak list
+    // peak filter (lazily allocated): S/N lookup -- a hash table for sparse lists, a dense plane over a slice of beams for
+    // dense ones --, live flags, peak list
     uint32_t* plane = nullptr;
+    int32_t plane_beams = 0;        // beams the plane covers
+    unsigned long long* hkeys = nullptr;
+    uint32_t* hvals = nullptr;
+    uint64_t hcap = 0;
     uint8_t* alive[2] = {nullptr, nullptr};
     int64_t alive_cap = 0;
     spt_candidate* peaks = nullptr;
@@ -144,7 +149,7 @@ static void free_device(Plan* p) {
     }
     cudaFree(d->maxval); cudaFree(d->nout); cudaFree(d->offset); cudaFree(d->range_lo); cudaFree(d->range_hi);
     cudaFree(d->work[0]); cudaFree(d->work[1]); cudaFree(d->win_len); cudaFree(d->win_starts);
-    cudaFree(d->plane); cudaFree(d->alive[0]); cudaFree(d->alive[1]); cudaFree(d->peaks); cudaFree(d->peaks_count);
+    cudaFree(d->plane); cudaFree(d->hkeys); cudaFree(d->hvals); cudaFree(d->alive[0]); cudaFree(d->alive[1]); cudaFree(d->peaks); cudaFree(d->peaks_count);
     for (auto& b : d->bufs) { cudaFree(b.sum); cudaFree(b.sumsq); cudaFree(b.cand); cudaFree(b.count); }
     for (auto& sl : d->slot) {
         cudaFree(sl.fb);
@@ -536,6 +541,11 @@ int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value) {
         p.opt_profile = (int32_t)value;
         return SPT_OK;
     }
+    if (!std::strcmp(name, "peaks_lookup")) {
+        if (value < 0 || value > 3) return SPT_ERR_INVALID;
+        p.opt_peaks_lookup = (int32_t)value;
+        return SPT_OK;
+    }
     if (p.dev) return SPT_ERR_STATE;
     if (!std::strcmp(name, "dedisp_kernel")) {
         if (value != 0 && value != 1) return SPT_ERR_INVALID;
@@ -922,12 +932,7 @@ int spt_peak_filter(spt_plan* plan, const int32_t* windows, int32_t nwindows, vo
     if (rc != SPT_OK) return rc;
     if (ovf) return SPT_ERR_SHAPE;                               // an incomplete list cannot be filtered
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (!d->plane) {
-        const size_t bytes = (size_t)p.max_beams * p.dmt_elems * sizeof(uint32_t);
-        SPT_CUDA(cudaMalloc((void**)&d->plane, bytes ? bytes : 4));
-        SPT_CUDA(cudaMemset(d->plane, 0, bytes));
-        SPT_CUDA(cudaMalloc((void**)&d->peaks_count, 8));
-    }
+    if (!d->peaks_count) SPT_CUDA(cudaMalloc((void**)&d->peaks_count, 8));
     if (total > d->alive_cap) {
         cudaFree(d->alive[0]); cudaFree(d->alive[1]); cudaFree(d->peaks);
         d->alive[0] = d->alive[1] = nullptr; d->peaks = nullptr; d->alive_cap = d->peaks_cap = 0;
@@ -937,16 +942,63 @@ int spt_peak_filter(spt_plan* plan, const int32_t* windows, int32_t nwindows, vo
         d->alive_cap = d->peaks_cap = total;
     }
     SPT_CUDA(cudaMemsetAsync(d->peaks_count, 0, 8, st));
-    PeakArgs a{d->bufs[d->cur].cand, total, d->plane, p.dmt_elems, d->nout, d->offset, d->range_lo, d->range_hi};
-    launch_peaks_scatter(a, true, st);
+    PeakArgs a{};
+    a.cand = d->bufs[d->cur].cand; a.n = total; a.beam_stride = p.dmt_elems;
+    a.nout = d->nout; a.offset = d->offset; a.range_lo = d->range_lo; a.range_hi = d->range_hi;
+    const int32_t nbeam = d->nbeam_search;
+    // Sparse list (the paper's regime): a hash table of two slots per candidate.  Dense list (a sizeable fraction of all cells):
+    // a plane like the DM transform, 4 GiB at most, covering as many beams as fit and passed over the list once per slice.
+    uint64_t hcap = 1024;
+    while (hcap < 2 * (uint64_t)total) hcap <<= 1;
+    const double plane_all = (double)nbeam * (double)p.dmt_elems * 4.0;
+    const bool use_hash = p.opt_peaks_lookup == 1 || (p.opt_peaks_lookup == 0 && (double)hcap * 12.0 <= plane_all / 4.0);
     const uint8_t* in = nullptr;
-    for (int32_t i = 0; i < nwindows; ++i) {
-        launch_peaks_stencil(a, windows[i], in, d->alive[i & 1], st);
-        in = d->alive[i & 1];
+    int64_t nlaunch = 0;
+    if (total > 0 && use_hash) {
+        if (hcap > d->hcap) {
+            cudaFree(d->hkeys); cudaFree(d->hvals);
+            d->hkeys = nullptr; d->hvals = nullptr; d->hcap = 0;
+            SPT_CUDA(cudaMalloc((void**)&d->hkeys, (size_t)hcap * 8));
+            SPT_CUDA(cudaMalloc((void**)&d->hvals, (size_t)hcap * 4));
+            d->hcap = hcap;
+        }
+        SPT_CUDA(cudaMemsetAsync(d->hkeys, 0xff, (size_t)hcap * 8, st));
+        a.hkeys = d->hkeys; a.vals = d->hvals; a.hmask = hcap - 1;
+        launch_peaks_insert(a, st);
+        for (int32_t i = 0; i < nwindows; ++i) {
+            launch_peaks_stencil(a, windows[i], in, d->alive[i & 1], st);
+            if (i + 1 < nwindows) launch_peaks_erase(a, in, d->alive[i & 1], false, st);
+            in = d->alive[i & 1];
+        }
+        nlaunch = 2 * nwindows;
+    } else if (total > 0) {
+        const int64_t per_beam = p.dmt_elems * 4;
+        const int32_t fit = p.opt_peaks_lookup == 3 ? 1 :
+            (int32_t)std::max<int64_t>(1, std::min<int64_t>(nbeam, (4ll << 30) / std::max<int64_t>(per_beam, 1)));
+        if (fit > d->plane_beams || (p.opt_peaks_lookup == 3 && d->plane_beams != 1)) {
+            cudaFree(d->plane);
+            d->plane = nullptr; d->plane_beams = 0;
+            SPT_CUDA(cudaMalloc((void**)&d->plane, (size_t)fit * per_beam));
+            SPT_CUDA(cudaMemsetAsync(d->plane, 0xff, (size_t)fit * per_beam, st));   // all empty; every call leaves it so
+            d->plane_beams = fit;
+        }
+        a.vals = d->plane;
+        for (int32_t b0 = 0; b0 < nbeam; b0 += d->plane_beams) {
+            a.beam0 = b0; a.nbeam_slice = std::min(d->plane_beams, nbeam - b0);
+            launch_peaks_insert(a, st);
+            const uint8_t* sin = nullptr;
+            for (int32_t i = 0; i < nwindows; ++i) {
+                launch_peaks_stencil(a, windows[i], sin, d->alive[i & 1], st);
+                if (i + 1 < nwindows) launch_peaks_erase(a, sin, d->alive[i & 1], false, st);
+                sin = d->alive[i & 1];
+            }
+            launch_peaks_erase(a, nullptr, nullptr, true, st);
+            nlaunch += 2 * nwindows + 1;
+        }
+        in = d->alive[(nwindows - 1) & 1];
     }
-    launch_peaks_compact(a, in, d->peaks, d->peaks_count, d->peaks_cap, st);
-    launch_peaks_scatter(a, false, st);                          // the plane is all zero again
-    p.launches += (total > 0) ? 3 + nwindows : 0;
+    if (total > 0) { launch_peaks_compact(a, in, d->peaks, d->peaks_count, d->peaks_cap, st); ++nlaunch; }
+    p.launches += nlaunch;
     SPT_CUDA(cudaGetLastError());
     d->last_stream = st;
     d->wait_event = nullptr;

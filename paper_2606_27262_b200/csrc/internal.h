@@ -130,6 +130,7 @@ struct Plan {
     int32_t opt_max_ent = 0;         // entries per group, at most: 8, 12 or 16 (0: chosen per range by the cost model)
     int32_t opt_dm_tile = 64;
     int32_t opt_profile = 0;
+    int32_t opt_peaks_lookup = 0;    // peak filter's S/N lookup: 0 by list density, 1 hash table, 2 dense plane, 3 dense plane of one beam
     int32_t opt_skew = 1;            // per-trial output skew inside a DM tile (0: all trials of a tile share t0)
     bool tiling_built = false;
     int64_t launches = 0;

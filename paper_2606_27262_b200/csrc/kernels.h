@@ -49,15 +49,19 @@ void launch_sps(const SpsArgs& a, int32_t nbeam, cudaStream_t st);
 struct PeakArgs {
     const spt_candidate* cand;      // the list of the last search
     int64_t n;                      // records in it
-    uint32_t* plane;                // [nbeam][beam_stride] lookup table, all zero between calls
-    int64_t beam_stride;
+    uint32_t* vals;                 // float bits of the live candidates' S/N (0xffffffff: none): dense plane cells or hash slots
+    unsigned long long* hkeys;      // hash table keys (cell number over all beams), NULL: dense plane
+    uint64_t hmask;                 // hash capacity - 1
+    int64_t beam_stride;            // cells per beam (= DM-transform elements per beam)
+    int32_t beam0, nbeam_slice;     // dense plane: the beams it covers in this pass
     const int32_t* nout;            // [ntrials]
     const int64_t* offset;          // [ntrials]
     const int32_t* range_lo;        // [ntrials] first / last trial of the trial's DM range
     const int32_t* range_hi;
 };
-void launch_peaks_scatter(const PeakArgs& a, bool set, cudaStream_t st);
+void launch_peaks_insert(const PeakArgs& a, cudaStream_t st);
 void launch_peaks_stencil(const PeakArgs& a, int32_t window, const uint8_t* alive_in, uint8_t* alive_out, cudaStream_t st);
+void launch_peaks_erase(const PeakArgs& a, const uint8_t* alive_before, const uint8_t* alive_after, bool all, cudaStream_t st);
 void launch_peaks_compact(const PeakArgs& a, const uint8_t* alive, spt_candidate* out, unsigned long long* out_count,
                           long long out_capacity, cudaStream_t st);
 

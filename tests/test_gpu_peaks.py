@@ -20,12 +20,15 @@ def oracle_filter_of_list(orc, plan, cands, windows):
     return cands[keep]
 
 
+@pytest.mark.parametrize("lookup", [0, 1, 2])
 @pytest.mark.parametrize("windows", [(3,), (11,), (3, 11), (5, 3, 7)])
-def test_filter_is_exact_on_the_same_list(cuda, api, orc, synth, windows):
+def test_filter_is_exact_on_the_same_list(cuda, api, orc, synth, windows, lookup):
+    """lookup: how the filter finds a neighbour's S/N -- chosen by the list's density, hash table, dense plane."""
     w = mini3(synth, 12)
     fb = synth.generate(w)
     plan, dmt, cands = run_gpu(cuda, api, w, fb[None], cand_capacity=1 << 20)
     assert cands.size > 1000
+    plan.set_option("peaks_lookup", lookup)
     peaks = plan.peak_filter(windows)
     expect = oracle_filter_of_list(orc, plan, cands, windows)
     assert 0 < peaks.size < cands.size
@@ -44,7 +47,10 @@ def test_quantised_ties_and_multibeam(cuda, api, orc):
     s = np.sort(cands["snr"])
     assert np.count_nonzero(np.diff(s) == 0) > cands.size // 2        # the premise: exact ties are common
     for windows in ((3,), (3, 11)):
-        assert as_set(plan.peak_filter(windows)) == as_set(oracle_filter_of_list(orc, plan, cands, windows))
+        expect = as_set(oracle_filter_of_list(orc, plan, cands, windows))
+        for lookup in (0, 1, 2, 3, 0):          # hash table, one plane for both beams, a one-beam plane passed over twice
+            plan.set_option("peaks_lookup", lookup)
+            assert as_set(plan.peak_filter(windows)) == expect, lookup
 
 
 def test_end_to_end_against_the_oracle_path(cuda, api, orc, synth):
