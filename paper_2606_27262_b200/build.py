@@ -40,7 +40,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
             if not force and not _stale():
                 return LIB
             tmp = LIB + ".tmp.%d" % os.getpid()
-            cmd = [NVCC, *FLAGS, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
+            extra = os.environ.get("SPT_NVCC_EXTRA", "").split()      # e.g. -DSPS_ITERS=9 for an A/B build
+            cmd = [NVCC, *FLAGS, *extra, "-o", tmp, *[os.path.join(CSRC, s) for s in SOURCES]]
             r = subprocess.run(cmd, capture_output=True, text=True)
             if verbose or r.returncode != 0:
                 sys.stderr.write(r.stdout + r.stderr)

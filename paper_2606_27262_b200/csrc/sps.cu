@@ -13,15 +13,20 @@
 // HBM bound by design (one compulsory read of the DM transform; the second pass of a row re-reads it from L2).
 #include <cuda_runtime.h>
 
+#include <atomic>
+
 #include "kernels.h"
 
 namespace spt {
 
 constexpr int kSpsThreads = 512;
 constexpr int kSpsWarps = kSpsThreads / 32;
-constexpr int kIters = 5;                           // 128-element warp rows per warp per segment
+#ifndef SPS_ITERS
+#define SPS_ITERS 7
+#endif
+constexpr int kIters = SPS_ITERS;                   // 128-element warp rows per warp per segment
 constexpr int kWarpSpan = kIters * 128;             // 640 consecutive elements per warp
-constexpr int kSegLoad = kSpsWarps * kWarpSpan;     // 10240 elements staged per segment (outputs + halo of the widest boxcar)
+constexpr int kSegLoad = kSpsWarps * kWarpSpan;     // 14336 elements staged per segment (outputs + halo of the widest boxcar)
 constexpr int kCOff = 3;                            // s_c[kCOff + 1 + e] = inclusive prefix through element e (16-byte aligned rows)
 constexpr int kEpt = 8;                             // outputs per thread per sub-block of the fast path
 // exact path geometry (kept from the first kernel): 8 samples per thread per segment
@@ -99,7 +104,8 @@ __device__ __forceinline__ void append(const SpsArgs& a, bool hit, int b, int d,
 // WIN = false: the whole row (the window logic folds away); WIN = true: a segment's window
 template <bool WIN>
 __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
-    __shared__ __align__(16) SpsShared sh;
+    extern __shared__ __align__(16) unsigned char sps_smem[];
+    SpsShared& sh = *reinterpret_cast<SpsShared*>(sps_smem);
     const int d = a.trial0 + blockIdx.x, b = blockIdx.y;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n = a.nout[d];                                  // end of the row
@@ -376,8 +382,19 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
 void launch_sps(const SpsArgs& a, int32_t nbeam, cudaStream_t st) {
     if (a.nlaunch <= 0 || nbeam <= 0) return;
     dim3 grid((unsigned)a.nlaunch, (unsigned)nbeam);
-    if (a.win_len) sps_kernel<true><<<grid, kSpsThreads, 0, st>>>(a);
-    else sps_kernel<false><<<grid, kSpsThreads, 0, st>>>(a);
+    // the staged segment makes SpsShared larger than the 48 KB a kernel gets without asking: opt in once per device
+    constexpr int kMaxDev = 64;
+    static std::atomic<bool> attr_set[kMaxDev];
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return;
+    if (dev < 0 || dev >= kMaxDev || !attr_set[dev].load(std::memory_order_acquire)) {
+        if (cudaFuncSetAttribute(sps_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SpsShared)) != cudaSuccess ||
+            cudaFuncSetAttribute(sps_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SpsShared)) != cudaSuccess)
+            return;                                   // the launch below then fails and the caller reports it
+        if (dev >= 0 && dev < kMaxDev) attr_set[dev].store(true, std::memory_order_release);
+    }
+    if (a.win_len) sps_kernel<true><<<grid, kSpsThreads, sizeof(SpsShared), st>>>(a);
+    else sps_kernel<false><<<grid, kSpsThreads, sizeof(SpsShared), st>>>(a);
 }
 
 }  // namespace spt
