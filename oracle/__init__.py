@@ -20,6 +20,12 @@ _SRC = os.path.join(_HERE, "oracle.cpp")
 _SO = os.path.join(_HERE, "liboracle.so")
 
 CXXFLAGS = ["-O2", "-fopenmp", "-ffp-contract=off", "-std=c++17", "-shared", "-fPIC"]
+# ORACLE_SANITIZE=1: the same source built with AddressSanitizer + UndefinedBehaviorSanitizer into its own library, for
+#   ORACLE_SANITIZE=1 LD_PRELOAD=$(gcc -print-file-name=libasan.so) ASAN_OPTIONS=detect_leaks=0 python -m pytest tests -m "not gpu"
+# (the result of the last such run is recorded in DESIGN.md section 3)
+if os.environ.get("ORACLE_SANITIZE") == "1":
+    CXXFLAGS = CXXFLAGS[:1] + ["-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"] + CXXFLAGS[1:]
+    _SO = os.path.join(_HERE, "liboracle_san.so")
 
 
 def build(force: bool = False) -> str:
