@@ -356,11 +356,21 @@ class Measurement:
         for _ in range(nsync):                   # and unpipelined (one synchronous spt_search_host per step), for the record
             p.search_host(self.h_fb, w.threshold)
         sync_ms = 1e3 * (time.perf_counter() - t0) / nsync
+        # what the host link gives on this box: the same pinned buffer copied alone (the floor of any end-to-end step)
+        c0, c1 = self.torch.cuda.Event(enable_timing=True), self.torch.cuda.Event(enable_timing=True)
+        self.d_fb.copy_(self.h_fb, non_blocking=True)
+        c0.record(self.stream)
+        for _ in range(3):
+            self.d_fb.copy_(self.h_fb, non_blocking=True)
+        c1.record(self.stream)
+        self.torch.cuda.synchronize()
+        h2d_ms = c0.elapsed_time(c1) / 3
         return {"value": self.adds_step * self.world * steps / e2e_s, "unit": UNIT,
                 "h2d_bytes_per_step": int(self.h_fb.numel()), "d2h_bytes_per_step": 8, "ms_per_step": 1e3 * e2e_s / steps,
                 "rtf": self.data_s * self.world * steps / e2e_s,
                 "api": "spt_stream_push/spt_stream_pop (two batches in flight)",
-                "ms_per_step_synchronous_call": sync_ms}, ncand
+                "ms_per_step_synchronous_call": sync_ms, "h2d_copy_alone_ms": h2d_ms,
+                "h2d_copy_alone_gbs": self.h_fb.numel() / h2d_ms / 1e6}, ncand
 
     def per_kernel(self, peaks_adds, hbm_gbs):
         """Every kernel of the step against the roofline SURVEY.md 8(d) assigns it: dedispersion vs the measured INT32 add

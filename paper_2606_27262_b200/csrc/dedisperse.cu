@@ -468,7 +468,17 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     const uint32_t floor2 = floor1 * 0x00010001u;
     const int lane_cap = (int)(65535u / max(1u, vmax - floor1));
     int since = 0;
+    // A warp none of whose trials has an output in this tile (the last DM tile of a range holds fewer than DT trials; rows end
+    // at different samples; a stream push wants only the tail) still does its share of the pre-sums but neither gathers nor
+    // widens.  s_valid was published by the barrier above.
+    bool warp_live = false;
+#pragma unroll
+    for (int q = 0; q < TPW; ++q) {
+        const int2 ok = s_valid[warp * TPW + q];
+        warp_live = warp_live || ok.y > ok.x;
+    }
     auto flush_lanes = [&]() {
+        if (!warp_live) return;
         const uint64_t pol_out = policy_evict_last();
         const uint32_t back = (uint32_t)since * floor1;   // the floor of the channels summed since the last pass
 #pragma unroll
@@ -516,7 +526,7 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
 
         if (since + nch_stage > lane_cap) { flush_lanes(); since = 0; }
         // ---- C: gather-accumulate ------------------------------------------------------------------------------
-        {
+        if (warp_live) {
             const uint32_t lane_addr = var_addr + (uint32_t)lane * 4u;
             const uint16_t* to = toff + warp * TPW;
             auto offsets = [&](const uint16_t* t, uint32_t (&off)[TPW]) {
