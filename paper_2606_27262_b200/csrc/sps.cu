@@ -66,7 +66,7 @@ struct SpsShared {
     int negT[kMaxWidths];                           // fast path: -floor(tau_w), clamped to +-2^30
     long long S;
     unsigned long long Q;
-    int live, fast, m, nw_eff;
+    int live, fast, lean, m, nw_eff;
 };
 
 // Full evaluation of one sample (readings C3-C5): widths in increasing order, strict '>', numerator exact.
@@ -189,6 +189,7 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
                 a.sum[(int64_t)b * a.ntrials + d] = S;
                 a.sumsq[(int64_t)b * a.ntrials + d] = Q;
                 sh.S = S; sh.Q = Q; sh.live = live; sh.fast = fast; sh.m = (int)m;
+                sh.lean = (dev * (long long)kSegLoad < (1ll << 30)) ? 1 : 0;     // no prefix sum of a staged segment can reach 2^30
                 int ne = 0;
                 while (ne < a.nw && a.widths[ne] <= nn) ++ne;                            // widths > N never apply
                 sh.nw_eff = ne;
@@ -220,6 +221,7 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
         // ---- pass 2, fast path ---------------------------------------------------------------------------------------
         const int m = sh.m;
         const int nw_eff = sh.nw_eff;
+        const bool lean = sh.lean != 0;
         // outputs per segment (launch_sps: wmax <= kXSeg - 32): whole sub-blocks of kSpsThreads * kEpt start positions when
         // the halo leaves room for them, so that no slot of the unrolled test below idles
         const int room = kSegLoad - halo;
@@ -228,44 +230,42 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
         // so its tail is what L1 and L2 still hold.
         for (int tb = (nbest - 1) / adv * adv; tb >= 0; tb -= adv) {
             __syncthreads();                                    // the previous segment's readers are done
-            // stage x - m: warp `warp` owns elements [warp*640, +640) of the segment; zero beyond N
-            int4 v[kIters];
-            int tot = 0;
-#pragma unroll
-            for (int it = 0; it < kIters; ++it) {
-                const int e = lo_al + tb + warp * kWarpSpan + it * 128 + lane * 4;
-                if (e >= lo && e + 4 <= n) {
-                    v[it] = ld4_hint(reinterpret_cast<const int4*>(x + e), l2_policy(0));
-                    v[it].x -= m; v[it].y -= m; v[it].z -= m; v[it].w -= m;
-                } else {                                          // the ends of the window: zero outside [lo, n)
-                    v[it].x = (e >= lo && e < n) ? x[e] - m : 0;
-                    v[it].y = (e + 1 >= lo && e + 1 < n) ? x[e + 1] - m : 0;
-                    v[it].z = (e + 2 >= lo && e + 2 < n) ? x[e + 2] - m : 0;
-                    v[it].w = (e + 3 >= lo && e + 3 < n) ? x[e + 3] - m : 0;
-                }
-                tot += v[it].x + v[it].y + v[it].z + v[it].w;
-            }
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
-            if (lane == 0) sh.wtot[warp] = (uint32_t)tot;
-            __syncthreads();
+            // stage prefix sums of x - m: warp `warp` owns kWarpSpan consecutive elements of the segment and each of its
+            // lanes 4*kIters consecutive ones of those (zero beyond N), so that ONE warp scan serves the whole span: a lane's
+            // running sums, then a shuffle scan of the lanes' totals, then the warps' totals through shared memory
+            uint32_t p[kIters][4];
             uint32_t run = 0;
-            for (int w = 0; w < warp; ++w) run += sh.wtot[w];   // exclusive offset of this warp
 #pragma unroll
             for (int it = 0; it < kIters; ++it) {
-                const uint32_t p0 = (uint32_t)v[it].x, p1 = p0 + (uint32_t)v[it].y, p2 = p1 + (uint32_t)v[it].z,
-                               p3 = p2 + (uint32_t)v[it].w;
-                uint32_t incl = p3;
-#pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
-                    if (lane >= o) incl += y;
+                const int e = lo_al + tb + warp * kWarpSpan + lane * (4 * kIters) + it * 4;
+                int4 v;
+                if (e >= lo && e + 4 <= n) {
+                    v = ld4_hint(reinterpret_cast<const int4*>(x + e), l2_policy(0));
+                    v.x -= m; v.y -= m; v.z -= m; v.w -= m;
+                } else {                                          // the ends of the window: zero outside [lo, n)
+                    v.x = (e >= lo && e < n) ? x[e] - m : 0;
+                    v.y = (e + 1 >= lo && e + 1 < n) ? x[e + 1] - m : 0;
+                    v.z = (e + 2 >= lo && e + 2 < n) ? x[e + 2] - m : 0;
+                    v.w = (e + 3 >= lo && e + 3 < n) ? x[e + 3] - m : 0;
                 }
-                const uint32_t base = run + incl - p3;
-                *reinterpret_cast<uint4*>(&sh.c[kCOff + 1 + warp * kWarpSpan + it * 128 + lane * 4]) =
-                    make_uint4(base + p0, base + p1, base + p2, base + p3);
-                run += __shfl_sync(0xffffffffu, incl, 31);
+                p[it][0] = run + (uint32_t)v.x; p[it][1] = p[it][0] + (uint32_t)v.y;
+                p[it][2] = p[it][1] + (uint32_t)v.z; p[it][3] = p[it][2] + (uint32_t)v.w;
+                run = p[it][3];
             }
+            uint32_t incl = run;                                  // inclusive scan of the lanes' totals
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += y;
+            }
+            if (lane == 31) sh.wtot[warp] = incl;
+            __syncthreads();
+            uint32_t base = incl - run;                           // exclusive offset of this lane inside the warp's span ...
+            for (int w = 0; w < warp; ++w) base += sh.wtot[w];    // ... plus the spans of the warps before
+#pragma unroll
+            for (int it = 0; it < kIters; ++it)
+                *reinterpret_cast<uint4*>(&sh.c[kCOff + 1 + warp * kWarpSpan + lane * (4 * kIters) + it * 4]) =
+                    make_uint4(base + p[it][0], base + p[it][1], base + p[it][2], base + p[it][3]);
             if (tid == 0) sh.c[kCOff] = 0u;
             __syncthreads();
 
@@ -283,41 +283,77 @@ __global__ void __launch_bounds__(kSpsThreads, 2) sps_kernel(const SpsArgs a) {
                 // Slots past the end of the segment are not clamped: i + w stays inside sh.c (i < i0 + 4096 <= the staged
                 // length minus the halo, or < 4096 with w <= 4064), they read stale words and are dropped by `pre` below.
                 // So slot e sits at a fixed distance from slot 0 and its loads take an immediate offset.
-                int nc0[kEpt], mxv[kEpt];
                 const uint32_t a0 = (uint32_t)__cvta_generic_to_shared(&sh.c[kCOff]) + 4u * (uint32_t)(i0 + tid);
-#pragma unroll
-                for (int e = 0; e < kEpt; ++e) {
-                    nc0[e] = -(int)sh.c[kCOff + i0 + e * kSpsThreads + tid];
-                    mxv[e] = (int)0x80000000;
-                }
-                int k = 0;
-                for (; k + 2 <= nw_eff; k += 2) {                          // two widths per pass: one 3-input max for both
-                    const uint32_t aw0 = a0 + 4u * (uint32_t)a.widths[k], aw1 = a0 + 4u * (uint32_t)a.widths[k + 1];
-                    const int nT0 = sh.negT[k], nT1 = sh.negT[k + 1];
+                unsigned premask = 0u;                                     // bit e: slot e passed the integer pre-test
+                if (lean) {
+                    // No prefix sum of the segment can wrap (|c| < 2^30, decided per row from its range), so the largest
+                    // c[i + w] - floor(tau_w) is taken first -- one load and one fused add-max per (slot, width) -- and
+                    // compared with c[i] once.
+                    int c0[kEpt], mxv[kEpt];
 #pragma unroll
                     for (int e = 0; e < kEpt; ++e) {
-                        uint32_t v0, v1;
-                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v0) : "r"(aw0 + (uint32_t)(e * kSpsThreads * 4)));   // [R + imm]
-                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v1) : "r"(aw1 + (uint32_t)(e * kSpsThreads * 4)));
-                        mxv[e] = max(mxv[e], max((int)v0 + nc0[e] + nT0, (int)v1 + nc0[e] + nT1));
+                        c0[e] = (int)sh.c[kCOff + i0 + e * kSpsThreads + tid];
+                        mxv[e] = (int)0x80000000;
                     }
-                }
-                if (k < nw_eff) {
-                    const uint32_t aw = a0 + 4u * (uint32_t)a.widths[k];
-                    const int nT = sh.negT[k];
+#pragma unroll 2
+                    for (int k = 0; k < nw_eff; ++k) {
+                        const uint32_t aw = a0 + 4u * (uint32_t)a.widths[k];
+                        const int nT = sh.negT[k];
+#pragma unroll
+                        for (int e = 0; e < kEpt; ++e) {
+                            uint32_t v;
+                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(aw + (uint32_t)(e * kSpsThreads * 4)));   // [R + imm]
+                            mxv[e] = __viaddmax_s32((int)v, nT, mxv[e]);
+                        }
+                    }
+#pragma unroll
+                    for (int e = 0; e < kEpt; ++e) premask |= (mxv[e] >= c0[e] ? 1u : 0u) << e;
+                } else {
+                    int nc0[kEpt], mxv[kEpt];
 #pragma unroll
                     for (int e = 0; e < kEpt; ++e) {
-                        uint32_t v;
-                        asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(aw + (uint32_t)(e * kSpsThreads * 4)));
-                        mxv[e] = max(mxv[e], (int)v + nc0[e] + nT);
+                        nc0[e] = -(int)sh.c[kCOff + i0 + e * kSpsThreads + tid];
+                        mxv[e] = (int)0x80000000;
                     }
+                    int k = 0;
+                    for (; k + 2 <= nw_eff; k += 2) {                          // two widths per pass: one 3-input max for both
+                        const uint32_t aw0 = a0 + 4u * (uint32_t)a.widths[k], aw1 = a0 + 4u * (uint32_t)a.widths[k + 1];
+                        const int nT0 = sh.negT[k], nT1 = sh.negT[k + 1];
+#pragma unroll
+                        for (int e = 0; e < kEpt; ++e) {
+                            uint32_t v0, v1;
+                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v0) : "r"(aw0 + (uint32_t)(e * kSpsThreads * 4)));
+                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v1) : "r"(aw1 + (uint32_t)(e * kSpsThreads * 4)));
+                            mxv[e] = max(mxv[e], max((int)v0 + nc0[e] + nT0, (int)v1 + nc0[e] + nT1));
+                        }
+                    }
+                    if (k < nw_eff) {
+                        const uint32_t aw = a0 + 4u * (uint32_t)a.widths[k];
+                        const int nT = sh.negT[k];
+#pragma unroll
+                        for (int e = 0; e < kEpt; ++e) {
+                            uint32_t v;
+                            asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(aw + (uint32_t)(e * kSpsThreads * 4)));
+                            mxv[e] = max(mxv[e], (int)v + nc0[e] + nT);
+                        }
+                    }
+#pragma unroll
+                    for (int e = 0; e < kEpt; ++e) premask |= (mxv[e] >= 0 ? 1u : 0u) << e;
                 }
+                // slots outside the segment or the window read stale words: drop them; then one vote for the whole sub-block
+                // (a pass is rare on noise: 6e-5 of the samples of config 3)
 #pragma unroll
                 for (int e = 0; e < kEpt; ++e) {
                     const int i = i0 + e * kSpsThreads + tid;
-                    const int t = lo_al + tb + i;
-                    const bool pre = i < nthis && t >= lo && mxv[e] >= 0;
+                    if (!(i < nthis && lo_al + tb + i >= lo)) premask &= ~(1u << e);
+                }
+                if (!__any_sync(0xffffffffu, premask != 0u)) continue;
+#pragma unroll 1
+                for (int e = 0; e < kEpt; ++e) {
+                    const bool pre = (premask >> e) & 1u;
                     if (!__any_sync(0xffffffffu, pre)) continue;
+                    const int i = i0 + e * kSpsThreads + tid;
+                    const int t = lo_al + tb + i;
                     bool hit = false;
                     double best = 0.0;
                     int bw = w0;
