@@ -272,8 +272,26 @@ class Measurement:
         self.stream = torch.cuda.current_stream()
         self.data_s = nbeam * w.nsamp * w.tsamp
 
+    def capture(self):
+        """--graph: spt_search only enqueues, so the step's launches can be captured once into a CUDA graph and replayed (what
+        a launch-bound small plan wants); the count readback stays outside."""
+        torch = self.torch
+        self.plan.set_option("profile", 0)
+        self.plan.search(self.d_fb, self.w.threshold, self.d_dmt, self.stream)
+        torch.cuda.synchronize()
+        self.gstream = torch.cuda.Stream()
+        self.graph = torch.cuda.CUDAGraph()
+        l0 = self.plan.launches()
+        with torch.cuda.graph(self.graph, stream=self.gstream):
+            self.plan.search(self.d_fb, self.w.threshold, self.d_dmt, self.gstream)
+        self.graph_launches = self.plan.launches() - l0        # kernel nodes of the graph: every replay launches them again
+        torch.cuda.synchronize()
+
     def step(self):
         p, w = self.plan, self.w
+        if getattr(self, "graph", None) is not None:
+            self.graph.replay()
+            return p.candidates_count()
         if self.args.two_calls:             # spt_dedisperse, then spt_single_pulse_search
             p.dedisperse(self.d_fb, self.d_dmt, self.stream)
             p.single_pulse_search(self.d_dmt, w.threshold, self.stream)
@@ -303,6 +321,8 @@ class Measurement:
         for _ in range(warm):
             self.step()
         self.ktimes = self.kernel_times()
+        if self.args.graph:
+            self.capture()
         ncand, ovf = self.step()            # profiling off: the timed region runs as a user would run it
         launches0 = self.plan.launches()
         sampler = ClockSampler(local_rank)
@@ -316,7 +336,10 @@ class Measurement:
         self.barrier()
         clocks = sampler.stop()
         ms_total = self.shard.max_over_ranks(e0.elapsed_time(e1), device="cuda")
-        return {"ms_total": ms_total, "launches": self.plan.launches() - launches0, "clocks": clocks,
+        nl = self.plan.launches() - launches0
+        if getattr(self, "graph", None) is not None:
+            nl = steps * self.graph_launches
+        return {"ms_total": ms_total, "launches": nl, "clocks": clocks,
                 "ncand": ncand, "overflowed": ovf}
 
     def peak_filter(self):
@@ -550,7 +573,8 @@ def run_ours(args, rank, world, local_rank):
             "dtype": "int32", "data": "synthetic", "config": workload_config(w, world),
             "launch": {"group": args.group or 8, "dm_tile": args.dm_tile or 64,
                        "step_api": "spt_dedisperse + spt_single_pulse_search + spt_candidates_count" if args.two_calls
-                                   else "spt_search + spt_candidates_count",
+                                   else ("CUDA graph of spt_search, replayed + spt_candidates_count" if args.graph
+                                         else "spt_search + spt_candidates_count"),
                        "dmt_mib_per_beam": plan.dmt_elems_per_beam * 4 / 2**20},
             "rtf": rtf, "realtime_beams": rtf, "candidates": ncand, "overflowed": t["overflowed"],
             "e2e": e2e, "peak_filter": peak_info, "gpu_launches": t["launches"], "clocks": t["clocks"], "kernel_ms": kernels,
@@ -728,6 +752,7 @@ def main():
     ap.add_argument("--all-configs", action="store_true")
     ap.add_argument("--stream", action="store_true")
     ap.add_argument("--cutouts", action="store_true")
+    ap.add_argument("--graph", action="store_true", help="replay a CUDA graph of spt_search instead of calling it every step")
     ap.add_argument("--two-calls", action="store_true", help="step = spt_dedisperse + spt_single_pulse_search instead of spt_search")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

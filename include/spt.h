@@ -98,7 +98,8 @@ int spt_plan_delays(const spt_plan* plan, int32_t trial, int32_t* host_out);
 
 /* Kernel-selection knobs, for A/B measurements and tests; must be set before the first spt_dedisperse.
  *   "dedisp_kernel": 0 = tiled shared-memory kernel (default, the product), 1 = one-thread-per-output kernel
- *                    reading global memory (bring-up / cross-check kernel, same results)
+ *                    reading global memory (bring-up / cross-check kernel, same results; it always computes whole rows,
+ *                    also for spt_segment_push with whole_rows = 0)
  *   "group":         largest pre-summed channel group of the tiled kernel in channels: 1, 2, 4, 8, 12 or 16 (default: 8, or 16
  *                    where the cost model picks groups of 12 entries)
  *   "dm_tile":       trials per block tile (32 or 64; default 64)

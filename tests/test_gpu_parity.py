@@ -245,6 +245,34 @@ def test_search_host_matches_device_path(cuda, api, orc, synth):
     assert plan.launches() >= 2
 
 
+# ---- spt_search inside a CUDA graph: the call only enqueues (memsets, kernels, event fork/join of its side streams), so a
+# caller can capture it once and replay it -- what a launch-bound small plan wants ------------------------------------
+def test_search_can_be_captured_in_a_cuda_graph(cuda, api, orc, synth):
+    w = mini3(synth, 12)
+    fbs = [synth.generate(w, beam=b) for b in range(2)]           # two different inputs through the same graph
+    plan = make_plan(api, w, cand_capacity=1 << 20)
+    d_fb = cuda.from_numpy(fbs[0][None]).cuda()
+    d_dmt = cuda.zeros((1, plan.dmt_elems_per_beam), dtype=cuda.int32, device="cuda")
+    plan.search(d_fb, w.threshold, d_dmt)                          # first call outside the capture: it allocates and uploads
+    cuda.cuda.synchronize()
+    side = cuda.cuda.Stream()
+    graph = cuda.cuda.CUDAGraph()
+    with cuda.cuda.graph(graph, stream=side):
+        plan.search(d_fb, w.threshold, d_dmt, side)
+    for fb in fbs[::-1] + fbs:
+        d_fb.copy_(cuda.from_numpy(fb[None]))
+        d_dmt.fill_(-3)
+        graph.replay()
+        total, ovf = plan.candidates_count()
+        cands = plan.candidates_read()
+        assert not ovf and cands.size == total
+        ref = oracle_path(orc, w, fb)
+        check_dmt_against_oracle(plan, d_dmt.cpu().numpy(), ref)
+        check_stats_against_oracle(plan, ref)
+        st = check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+        assert st["oracle"] > 100, st
+
+
 # ---- spt_search: both steps in one call, every range searched behind its own dedispersion --------------------------
 @pytest.mark.parametrize("profile", [0, 1])
 def test_fused_search_call_matches_oracle_and_two_call_path(cuda, api, orc, synth, profile):
