@@ -264,6 +264,9 @@ class Measurement:
             opts["dm_tile"] = args.dm_tile
         if args.max_entries:
             opts["max_entries"] = args.max_entries
+        for kv in args.opt or []:                      # any other plan option, e.g. --opt compact=0
+            k, v = kv.split("=")
+            opts[k] = int(v)
         self.plan = api.Plan(w.fch1, w.foff, w.nchan, w.tsamp, w.nsamp, w.ranges, w.widths, max_beams=nbeam,
                              cand_capacity=CAND_CAPACITY[w.index], options=opts)
         self.adds_step = algorithmic_adds(self.plan, w.nchan) * nbeam
@@ -747,6 +750,7 @@ def main():
     ap.add_argument("--group", type=int, default=0)
     ap.add_argument("--dm-tile", type=int, default=0)
     ap.add_argument("--max-entries", type=int, default=0)
+    ap.add_argument("--opt", action="append", help="plan option name=value (spt_plan_set_option), may be repeated")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-worst-case", action="store_true")
     ap.add_argument("--all-configs", action="store_true")

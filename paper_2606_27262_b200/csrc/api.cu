@@ -34,6 +34,15 @@ struct RangeDev {
     uint32_t* blob = nullptr;
     int32_t* skew = nullptr;
     uint16_t* series = nullptr;     // decimated input [max_beams][nchan][stride_k] (decim > 1)
+    // decim > 1: the 8-bit copy of the series (sample - smallest sample, made per call when the series spans < 256), its
+    // kernel tables, and {largest value, 0, valid flag, smallest sample} written by the kernel that makes it
+    uint8_t* series8 = nullptr;
+    uint32_t* cinfo = nullptr;
+    TileDesc* c_tiles = nullptr;
+    StageIndex* c_sidx = nullptr;
+    RowDesc* c_rows = nullptr;
+    uint32_t* c_blob = nullptr;
+    int32_t* c_skew = nullptr;
 };
 
 struct DeviceState {
@@ -146,6 +155,8 @@ static void free_device(Plan* p) {
     for (RangeDev& r : d->r) {
         cudaFree(r.delay); cudaFree(r.tiles); cudaFree(r.sidx); cudaFree(r.rows); cudaFree(r.blob); cudaFree(r.skew);
         cudaFree(r.series);
+        cudaFree(r.series8); cudaFree(r.cinfo); cudaFree(r.c_tiles); cudaFree(r.c_sidx); cudaFree(r.c_rows); cudaFree(r.c_blob);
+        cudaFree(r.c_skew);
     }
     cudaFree(d->maxval); cudaFree(d->nout); cudaFree(d->offset); cudaFree(d->range_lo); cudaFree(d->range_hi);
     cudaFree(d->work[0]); cudaFree(d->work[1]); cudaFree(d->win_len); cudaFree(d->win_starts);
@@ -219,6 +230,17 @@ static int ensure_device(Plan* p) {
             cudaError_t ce = cudaMalloc((void**)&rd.series, bytes);
             if (ce == cudaSuccess) ce = cudaMemset(rd.series, 0, bytes);
             if (ce != cudaSuccess) rc = cuda_fail(ce, "series alloc");
+            if (rc == SPT_OK && p->opt_kernel == 0 && i < p->compact.size() && !p->compact[i].tiles.empty()) {
+                const RangePlan& cp = p->compact[i];
+                ce = cudaMalloc((void**)&rd.series8, bytes / 2);
+                if (ce == cudaSuccess) ce = cudaMalloc((void**)&rd.cinfo, 4 * sizeof(uint32_t));
+                if (ce != cudaSuccess) rc = cuda_fail(ce, "compact series alloc");
+                if (rc == SPT_OK) rc = upload(&rd.c_tiles, cp.tiles);
+                if (rc == SPT_OK) rc = upload(&rd.c_sidx, cp.sidx);
+                if (rc == SPT_OK) rc = upload(&rd.c_rows, cp.rows);
+                if (rc == SPT_OK) rc = upload(&rd.c_blob, cp.blob);
+                if (rc == SPT_OK) rc = upload(&rd.c_skew, cp.skew);
+            }
         }
     }
     if (rc == SPT_OK) rc = upload(&d->nout, nout_all);
@@ -304,6 +326,11 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
                         (int64_t)p->nchan * rp.stride_k, p->nchan, nbeam, rp.nsamp_k, rp.decim, s);
         launch_max_u16(d->r[i].series, (int64_t)nbeam * p->nchan * rp.stride_k, d->maxval + 2 * i, s);
         p->launches += 2;
+        if (d->r[i].series8) {               // the 8-bit copy, if the series spans less than 256 (decided on the device)
+            launch_compact_u16(d->r[i].series, d->r[i].series8, (int64_t)nbeam * p->nchan * rp.stride_k, d->maxval + 2 * i,
+                               d->r[i].cinfo, s);
+            p->launches++;
+        }
         return SPT_OK;
     };
     // launch order: the side streams' pre-passes, then the first range (pre-pass and grid), then the other grids
@@ -340,9 +367,29 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
                 }
                 if (tail_tiles <= 0) continue;
             }
-            const int rc = launch_dedisp_tiled(u16, p->opt_dm_tile, rp.max_ent, src, rs, (int64_t)p->nchan * rs, d_dmt, p->dmt_elems,
-                                               rd.tiles, rd.sidx, rd.rows, rd.blob, d->maxval + 2 * i, rd.skew, rp.skew_max, rp.vcap_words, nout, off,
-                                               (int32_t)rp.tiles.size(), rp.ntile_t, nbeam, tail, tail_tiles, st);
+            auto args_of = [&](const RangePlan& t, const void* series, const TileDesc* tiles, const StageIndex* sidx,
+                               const RowDesc* rows, const uint32_t* blob, const int32_t* skew, const uint32_t* bounds) {
+                TiledArgs a{};
+                a.in = series; a.row_stride = rs; a.beam_stride = (int64_t)p->nchan * rs;
+                a.out = d_dmt; a.out_beam_stride = p->dmt_elems;
+                a.tiles = tiles; a.sidx = sidx; a.rows = rows; a.blob = blob; a.maxval = bounds; a.skew = skew;
+                a.skew_max = t.skew_max; a.nout = nout; a.offset = off; a.vcap_words = t.vcap_words;
+                a.ntile_dm = (int32_t)t.tiles.size(); a.ntile_t = t.ntile_t; a.nbeam = nbeam;
+                a.tail = tail; a.tail_tiles = tail_tiles; a.enable = nullptr; a.enable_want = 0u;
+                return a;
+            };
+            const TiledArgs a16 = args_of(rp, src, rd.tiles, rd.sidx, rd.rows, rd.blob, rd.skew, d->maxval + 2 * i);
+            int rc;
+            if (rd.series8) {
+                // a decimated range runs on the 8-bit copy of its series, with the copy's tables, when the copy was made (the
+                // device decided that just before), on the uint16 series otherwise: one launch, the blocks look at the flag
+                const RangePlan& cp = p->compact[i];
+                TiledArgs a8 = args_of(cp, rd.series8, rd.c_tiles, rd.c_sidx, rd.c_rows, rd.c_blob, rd.c_skew, rd.cinfo);
+                a8.enable = rd.cinfo + 2; a8.enable_want = 1u;
+                rc = launch_dedisp_dual(p->opt_dm_tile, rp.max_ent, a8, a16, st);
+            } else {
+                rc = launch_dedisp_tiled(u16, p->opt_dm_tile, rp.max_ent, a16, st);
+            }
             if (rc != 0) { g_last_error = "dedisp_tiled: launch configuration rejected"; return SPT_ERR_CUDA; }
         }
         p->launches++;
@@ -547,6 +594,11 @@ int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value) {
         return SPT_OK;
     }
     if (p.dev) return SPT_ERR_STATE;
+    if (!std::strcmp(name, "compact")) {
+        if (value != 0 && value != 1) return SPT_ERR_INVALID;
+        p.opt_compact = (int32_t)value; p.tiling_built = false;
+        return SPT_OK;
+    }
     if (!std::strcmp(name, "dedisp_kernel")) {
         if (value != 0 && value != 1) return SPT_ERR_INVALID;
         p.opt_kernel = (int32_t)value;
@@ -624,16 +676,10 @@ int spt_plan_tiling_cost(spt_plan* plan, int32_t range, int64_t* ntasks, int64_t
     return SPT_OK;
 }
 
-int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
-    if (!plan || !host_out) return SPT_ERR_INVALID;
-    Plan& p = plan->p;
-    int32_t loc = 0;
-    const RangePlan* rp = range_of_trial(p, trial, &loc);
-    if (!rp) return SPT_ERR_SHAPE;
-    const int rc = ensure_tiling(p);
-    if (rc != SPT_OK) return rc;
+// The delay row of trial `loc` of a range as one set of kernel tables applies it (es: bytes per element of the series the
+// tables address).
+static int tiling_delays_of(const Plan& p, const RangePlan* rp, int es, int32_t loc, int32_t* host_out) {
     const int DT = p.opt_dm_tile;
-    const int es = rp->decim == 1 ? 1 : 2;
     const TileDesc& td = rp->tiles[loc / DT];
     const int dl = loc - td.trial0;
     for (int32_t c = 0; c < p.nchan; ++c) host_out[c] = INT32_MIN;
@@ -686,6 +732,25 @@ int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
     const int32_t sk = rp->skew[(size_t)td.skew0 + dl];
     for (int32_t c = 0; c < p.nchan; ++c)
         if (host_out[c] != INT32_MIN) host_out[c] += sk;
+    return SPT_OK;
+}
+
+int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out) {
+    if (!plan || !host_out) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    int32_t loc = 0;
+    const RangePlan* rp = range_of_trial(p, trial, &loc);
+    if (!rp) return SPT_ERR_SHAPE;
+    int rc = ensure_tiling(p);
+    if (rc != SPT_OK) return rc;
+    if ((rc = tiling_delays_of(p, rp, rp->decim == 1 ? 1 : 2, loc, host_out)) != SPT_OK) return rc;
+    // a decimated range has a second set of tables, for the 8-bit copy of its series: it must say the same
+    const size_t ri = (size_t)(rp - p.ranges.data());
+    if (ri < p.compact.size() && !p.compact[ri].tiles.empty()) {
+        std::vector<int32_t> again((size_t)p.nchan);
+        if ((rc = tiling_delays_of(p, &p.compact[ri], 1, loc, again.data())) != SPT_OK) return rc;
+        if (std::memcmp(again.data(), host_out, sizeof(int32_t) * (size_t)p.nchan) != 0) return SPT_ERR_STATE;
+    }
     return SPT_OK;
 }
 

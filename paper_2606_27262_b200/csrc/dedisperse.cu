@@ -115,6 +115,36 @@ void launch_max_u8(const uint8_t* x, int64_t nbytes, uint32_t* maxval, cudaStrea
     max_u8_kernel<<<sm_count() * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(x), n16, maxval);
 }
 
+// 8-bit copy of a decimated series: c = y - (smallest sample of the series), made only when the series spans less than 256
+// (quantised noise does: its decimated sums sit within a few sigma of k times the mean).  info[0..3] = {largest value of
+// the copy, 0 (its floor), flag: 1 = the copy is valid, bias = the smallest sample (added back per channel when the lanes
+// are widened)}.  The dedispersion of the range is enqueued twice, on the copy and on the uint16 series; each launch looks
+// at the flag and one of them returns at once.
+__global__ void compact_u16_kernel(const uint4* __restrict__ y, uint2* __restrict__ c, int64_t n8, const uint32_t* __restrict__ maxval,
+                                   uint32_t* __restrict__ info) {
+    const uint32_t vmax = __ldg(maxval), vmin = __ldg(maxval + 1);
+    const bool ok = vmin <= vmax && vmax - vmin <= 255u;
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        info[0] = ok ? vmax - vmin : 0u; info[1] = 0u; info[2] = ok ? 1u : 0u; info[3] = ok ? vmin : 0u;
+    }
+    if (!ok) return;
+    const uint32_t m2 = vmin * 0x00010001u;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n8; i += (int64_t)gridDim.x * blockDim.x) {
+        uint4 v = __ldg(y + i);                                   // eight samples
+        v.x -= m2; v.y -= m2; v.z -= m2; v.w -= m2;               // no borrow between the halves: every sample >= vmin
+        uint2 o;
+        o.x = __byte_perm(v.x, v.y, 0x6420);
+        o.y = __byte_perm(v.z, v.w, 0x6420);
+        c[i] = o;
+    }
+}
+
+void launch_compact_u16(const uint16_t* y, uint8_t* c, int64_t nelem, const uint32_t* maxval, uint32_t* info, cudaStream_t st) {
+    const int64_t n8 = nelem / 8;             // rows are 16-element multiples
+    if (n8 <= 0) return;
+    compact_u16_kernel<<<sm_count() * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(y), reinterpret_cast<uint2*>(c), n8, maxval, info);
+}
+
 void launch_decimate(const uint8_t* x, int64_t in_row_stride, int64_t in_beam_stride, uint16_t* y,
                      int64_t out_row_stride, int64_t out_beam_stride, int32_t nchan, int32_t nbeam, int64_t nsamp_k,
                      int32_t k, cudaStream_t st) {
@@ -179,25 +209,6 @@ template void launch_dedisp_naive<uint16_t>(const uint16_t*, int64_t, int64_t, c
 //               floor(65535 / (largest - smallest sample)) channels, at worst every 257/decim) the 16-bit lanes are widened
 //               into the int32 DM transform, the floor added back (first time a store, then RED).
 // ---------------------------------------------------------------------------------------------------------------
-struct TiledArgs {
-    const void* in;            // series of beam 0
-    int64_t row_stride;        // elements (multiple of 16)
-    int64_t beam_stride;       // elements
-    int32_t* out;
-    int64_t out_beam_stride;
-    const TileDesc* tiles;
-    const StageIndex* sidx;
-    const RowDesc* rows;
-    const uint32_t* blob;
-    const uint32_t* maxval;    // {largest, smallest} input sample of this launch (device): bound the 16-bit lanes
-    const int32_t* skew;       // [ntile_dm][DT] output skew of every trial of a DM tile
-    int32_t skew_max;
-    const int32_t* nout;       // range local
-    const int64_t* offset;     // range local
-    int32_t vcap_words, ntile_dm, ntile_t, nbeam;
-    int32_t tail;              // > 0: only the last `tail` outputs of every row are computed (a pushed stream segment) ...
-    int32_t tail_tiles;        // ... by this many time tiles per DM tile, counted back from the tile's last one
-};
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
@@ -356,7 +367,7 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
 // NEMAX: the largest entry class the plan's tables hold (8, 12 or 16): the kernel carries only the pre-sum instances it
 // needs, so that a plan of small groups does not pay for the registers of the large ones.
 template <typename T, int DT, int NEMAX>
-__global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledArgs a) {
+__device__ __forceinline__ void dedisp_tile_body(const TiledArgs& a) {
     constexpr int NW = kThreads / 32;
     constexpr int TPW = DT / NW;
     constexpr int NJ = kH / 32;
@@ -373,6 +384,11 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     const uint32_t var_addr = smem_u32(s_var), raw_addr = smem_u32(s_rawb);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    uint32_t bias = 0u;
+    if (a.enable != nullptr) {
+        if (__ldg(a.enable) != a.enable_want) return;            // the other launch of this range does the work
+        if (a.enable_want == 1u) bias = __ldg(a.enable + 1);
+    }
     int bid = blockIdx.x;
     const int dmt = bid % a.ntile_dm; bid /= a.ntile_dm;
     const int ntt = a.tail > 0 ? a.tail_tiles : a.ntile_t;
@@ -480,7 +496,7 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
     auto flush_lanes = [&]() {
         if (!warp_live) return;
         const uint64_t pol_out = policy_evict_last();
-        const uint32_t back = (uint32_t)since * floor1;   // the floor of the channels summed since the last pass
+        const uint32_t back = (uint32_t)since * (floor1 + bias);   // the floor of the channels summed since the last pass
 #pragma unroll
         for (int q = 0; q < TPW; ++q) {
             const int dl = warp * TPW + q;
@@ -569,18 +585,42 @@ __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledAr
 }
 
 template <typename T, int DT, int NEMAX>
-static int launch_tiled_inst(const TiledArgs& a, cudaStream_t st) {
-    // the opt-in to 113 KB of dynamic shared memory is a per-device attribute of the function: one flag per device
+__global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledArgs a) {
+    dedisp_tile_body<T, DT, NEMAX>(a);
+}
+
+// A decimated range in ONE launch: the 8-bit copy of its series with the copy's tables when the copy was made (a8.enable
+// points at {flag, bias}, written on the device just before), the uint16 series with its own tables otherwise.  The two
+// table sets tile the range identically (same DM tiles, same skews, same grid), so a block does the same tile either way.
+template <int DT, int NEMAX>
+__global__ void __launch_bounds__(kThreads, 2) dedisp_dual_kernel(const TiledArgs a8, const TiledArgs a16) {
+    if (__ldg(a8.enable) == 1u) dedisp_tile_body<uint8_t, DT, NEMAX>(a8);
+    else dedisp_tile_body<uint16_t, DT, NEMAX>(a16);
+}
+
+// the opt-in to 113 KB of dynamic shared memory is a per-device attribute of the function: one flag per device and instance
+template <typename K>
+static int opt_in_smem(K kern, std::atomic<bool>* attr_set) {
     constexpr int kMaxDev = 64;
-    static std::atomic<bool> attr_set[kMaxDev];
-    auto kern = dedisp_tiled_kernel<T, DT, NEMAX>;
     int dev = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return -1;
     if (dev < 0 || dev >= kMaxDev || !attr_set[dev].load(std::memory_order_acquire)) {
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemBytes) != cudaSuccess) return -1;
         if (dev >= 0 && dev < kMaxDev) attr_set[dev].store(true, std::memory_order_release);
     }
-    const int64_t nblocks = (int64_t)a.ntile_dm * (a.tail > 0 ? a.tail_tiles : a.ntile_t) * a.nbeam;
+    return 0;
+}
+
+static int64_t blocks_of(const TiledArgs& a) {
+    return (int64_t)a.ntile_dm * (a.tail > 0 ? a.tail_tiles : a.ntile_t) * a.nbeam;
+}
+
+template <typename T, int DT, int NEMAX>
+static int launch_tiled_inst(const TiledArgs& a, cudaStream_t st) {
+    static std::atomic<bool> attr_set[64];
+    auto kern = dedisp_tiled_kernel<T, DT, NEMAX>;
+    if (opt_in_smem(kern, attr_set) != 0) return -1;
+    const int64_t nblocks = blocks_of(a);
     if (nblocks <= 0) return 0;
     if (nblocks > 0x7fffffffLL) return -1;
     kern<<<(unsigned)nblocks, kThreads, kSmemBytes, st>>>(a);
@@ -592,13 +632,30 @@ static int launch_tiled_type(bool is_u16, const TiledArgs& a, cudaStream_t st) {
     return is_u16 ? launch_tiled_inst<uint16_t, DT, NEMAX>(a, st) : launch_tiled_inst<uint8_t, DT, NEMAX>(a, st);
 }
 
-int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
-                        int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
-                        const uint32_t* blob, const uint32_t* maxval, const int32_t* skew, int32_t skew_max, int32_t vcap_words,
-                        const int32_t* nout, const int64_t* offset, int32_t ntile_dm, int32_t ntile_t, int32_t nbeam,
-                        int32_t tail, int32_t tail_tiles, cudaStream_t st) {
-    TiledArgs a{in, row_stride, beam_stride, out, out_beam_stride, tiles, sidx, rows, blob, maxval, skew, skew_max, nout, offset,
-                vcap_words, ntile_dm, ntile_t, nbeam, tail, tail_tiles};
+template <int DT, int NEMAX>
+static int launch_dual_inst(const TiledArgs& a8, const TiledArgs& a16, cudaStream_t st) {
+    static std::atomic<bool> attr_set[64];
+    auto kern = dedisp_dual_kernel<DT, NEMAX>;
+    if (opt_in_smem(kern, attr_set) != 0) return -1;
+    const int64_t nblocks = blocks_of(a16);
+    if (nblocks != blocks_of(a8)) return -1;
+    if (nblocks <= 0) return 0;
+    if (nblocks > 0x7fffffffLL) return -1;
+    kern<<<(unsigned)nblocks, kThreads, kSmemBytes, st>>>(a8, a16);
+    return 0;
+}
+
+int launch_dedisp_dual(int DT, int max_ent, const TiledArgs& a8, const TiledArgs& a16, cudaStream_t st) {
+    if (DT == 64 && max_ent == 8) return launch_dual_inst<64, 8>(a8, a16, st);
+    if (DT == 64 && max_ent == 12) return launch_dual_inst<64, 12>(a8, a16, st);
+    if (DT == 64 && max_ent == 16) return launch_dual_inst<64, 16>(a8, a16, st);
+    if (DT == 32 && max_ent == 8) return launch_dual_inst<32, 8>(a8, a16, st);
+    if (DT == 32 && max_ent == 12) return launch_dual_inst<32, 12>(a8, a16, st);
+    if (DT == 32 && max_ent == 16) return launch_dual_inst<32, 16>(a8, a16, st);
+    return -1;
+}
+
+int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, const TiledArgs& a, cudaStream_t st) {
     if (DT == 64 && max_ent == 8) return launch_tiled_type<64, 8>(is_u16, a, st);
     if (DT == 64 && max_ent == 12) return launch_tiled_type<64, 12>(is_u16, a, st);
     if (DT == 64 && max_ent == 16) return launch_tiled_type<64, 16>(is_u16, a, st);

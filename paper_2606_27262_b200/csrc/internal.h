@@ -31,7 +31,7 @@ constexpr int kMaxStageGroups = 8;   // groups per stage
 constexpr int kChunkU = 128;         // variant words one warp builds per pre-sum task (4 per lane)
 constexpr int kBlobBytes = 3072;     // per-stage table blob (two buffers in shared memory)
 constexpr int kSmemBytes = 113 * 1024;                                   // two blocks per SM (228 KB incl. 1 KB each reserved)
-constexpr int kMaxStageRows = 96;                                        // raw rows (channels) of one stage
+constexpr int kMaxStageRows = 64;                                        // raw rows (channels) of one stage
 constexpr int kSmemCtrlBytes = 64 + kMaxDT * 16 + 2 * (kMaxStageRows * 16 + 16);  // mbarrier, per-trial {row pointer, nout},
                                                                          // next stage's {RowDesc[], StageIndex} x 2
 constexpr int kSmemDataBytes = kSmemBytes - kSmemCtrlBytes - 2 * kBlobBytes;  // variant region + raw-row region
@@ -122,6 +122,8 @@ struct Plan {
     int64_t cand_capacity = 0;
     std::vector<int32_t> widths;
     std::vector<RangePlan> ranges;
+    std::vector<RangePlan> compact;  // per range with decim > 1: the kernel tables for the 8-bit copy of its decimated series
+                                     // (empty tables otherwise); built by build_tiling
     int32_t ntrials = 0;
     int64_t dmt_elems = 0;           // per beam
     // options
@@ -130,6 +132,7 @@ struct Plan {
     int32_t opt_max_ent = 0;         // entries per group, at most: 8, 12 or 16 (0: chosen per range by the cost model)
     int32_t opt_dm_tile = 64;
     int32_t opt_profile = 0;
+    int32_t opt_compact = 1;         // decimated ranges: dedisperse the 8-bit copy of the series when its values span < 256
     int32_t opt_peaks_lookup = 0;    // peak filter's S/N lookup: 0 by list density, 1 hash table, 2 dense plane, 3 dense plane of one beam
     int32_t opt_skew = 1;            // per-trial output skew inside a DM tile (0: all trials of a tile share t0)
     bool tiling_built = false;

@@ -20,11 +20,34 @@ void launch_dedisp_naive(const T* y, int64_t row_stride, int64_t beam_stride, co
                          const int32_t* d_nout, const int64_t* d_offset, int32_t nchan, int32_t ndm, int32_t nbeam,
                          int32_t max_nout, int32_t* out, int64_t out_beam_stride, cudaStream_t st);
 
-int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, const void* in, int64_t row_stride, int64_t beam_stride, int32_t* out,
-                        int64_t out_beam_stride, const TileDesc* tiles, const StageIndex* sidx, const RowDesc* rows,
-                        const uint32_t* blob, const uint32_t* maxval, const int32_t* skew, int32_t skew_max, int32_t vcap_words,
-                        const int32_t* nout, const int64_t* offset,
-                        int32_t ntile_dm, int32_t ntile_t, int32_t nbeam, int32_t tail, int32_t tail_tiles, cudaStream_t st);
+// One launch of the tiled dedispersion kernel (dedisperse.cu) over one series and one set of kernel tables.
+struct TiledArgs {
+    const void* in;            // series of beam 0
+    int64_t row_stride;        // elements (multiple of 16)
+    int64_t beam_stride;       // elements
+    int32_t* out;
+    int64_t out_beam_stride;
+    const TileDesc* tiles;
+    const StageIndex* sidx;
+    const RowDesc* rows;
+    const uint32_t* blob;
+    const uint32_t* maxval;    // {largest, smallest} input sample of this launch (device): bound the 16-bit lanes
+    const int32_t* skew;       // [ntile_dm][DT] output skew of every trial of a DM tile
+    int32_t skew_max;
+    const int32_t* nout;       // range local
+    const int64_t* offset;     // range local
+    int32_t vcap_words, ntile_dm, ntile_t, nbeam;
+    int32_t tail;              // > 0: only the last `tail` outputs of every row are computed (a pushed stream segment) ...
+    int32_t tail_tiles;        // ... by this many time tiles per DM tile, counted back from the tile's last one
+    const uint32_t* enable;    // NULL, or {flag, bias} (device): the launch runs only when flag == enable_want (a decimated
+    uint32_t enable_want;      // range is enqueued on its 8-bit copy and on the uint16 series; the copy may not exist) and
+                               // every channel summed owes `bias` (the floor the 8-bit copy was made with) when want == 1
+};
+int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, const TiledArgs& a, cudaStream_t st);
+// a decimated range in one launch: a8 = the 8-bit copy of the series (a8.enable -> {valid flag, bias}, a8.enable_want = 1), a16
+// = the uint16 series (a16.enable = NULL); the block takes whichever the flag says
+int launch_dedisp_dual(int DT, int max_ent, const TiledArgs& a8, const TiledArgs& a16, cudaStream_t st);
+void launch_compact_u16(const uint16_t* y, uint8_t* c, int64_t nelem, const uint32_t* maxval, uint32_t* info, cudaStream_t st);
 
 struct SpsArgs {
     const int32_t* dmt;

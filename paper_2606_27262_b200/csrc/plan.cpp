@@ -213,7 +213,9 @@ static bool make_group(const Plan& p, const RangePlan& rp, int32_t d0, int32_t n
 }
 
 // Tables of one DM range for groups of at most G channels and max_ent entries.
-static int build_range(const Plan& p, RangePlan& rp, const int G, const int max_ent) {
+// compact: tables for the 8-bit copy of a decimated series (sample - smallest sample of the series, made when that fits a
+// byte): one byte per element and, like the raw input, at most 255 per sample whatever the decimation.
+static int build_range(const Plan& p, RangePlan& rp, const int G, const int max_ent, const bool compact = false) {
     const int DT = p.opt_dm_tile;
     rp.max_ent = max_ent;
     {
@@ -251,9 +253,9 @@ static int build_range(const Plan& p, RangePlan& rp, const int G, const int max_
             }
         }
         rp.ntile_t = (int32_t)((rp.max_nout + rp.skew_max + kTT - 1) / kTT);
-        const int es = rp.decim == 1 ? 1 : 2;
+        const int es = (rp.decim == 1 || compact) ? 1 : 2;
         // 16-bit lanes hold sums of at most floor(65535 / (255*decim)) channel samples
-        const int lane_channels = 65535 / (255 * rp.decim);
+        const int lane_channels = 65535 / (255 * (compact ? 1 : rp.decim));
         if (lane_channels < 1) return SPT_ERR_UNSUPPORTED;
         // split of the data region between variants and raw rows: from the needs of the middle DM tile
         {
@@ -440,24 +442,50 @@ static double modelled_cost(const RangePlan& rp) {
     return 2.456e-3 * (double)rp.ngroups + 2.37e-5 * pen * (double)(rp.task_entries + rp.task_variants);
 }
 
+// The same choice of entry cap for either element size.
+static int build_range_auto(const Plan& p, RangePlan& rp, bool compact);
+
 int build_tiling(Plan& p) {
-    for (RangePlan& rp : p.ranges) {
+    p.compact.clear();
+    p.compact.resize(p.ranges.size());
+    for (size_t i = 0; i < p.ranges.size(); ++i) {
+        int rc;
+        if ((rc = build_range_auto(p, p.ranges[i], false)) != SPT_OK) return rc;
+        if (p.ranges[i].decim > 1 && p.opt_compact) {
+            // second set of tables for the 8-bit copy of the decimated series (the delay table is shared by value: a few MB)
+            // Both sets run in one kernel instance, so they share the entry cap: the copy's choice (it is the set that runs
+            // on well-behaved data), and the same DM tiles and skews, so that a block does the same tile either way.
+            p.compact[i] = p.ranges[i];
+            if ((rc = build_range_auto(p, p.compact[i], true)) != SPT_OK) return rc;
+            if (p.compact[i].max_ent != p.ranges[i].max_ent) {
+                const int G = p.opt_group ? p.opt_group : (p.compact[i].max_ent > 8 ? 16 : 8);
+                if ((rc = build_range(p, p.ranges[i], G, p.compact[i].max_ent, false)) != SPT_OK) return rc;
+            }
+            if (p.compact[i].ntile_t != p.ranges[i].ntile_t || p.compact[i].tiles.size() != p.ranges[i].tiles.size() ||
+                p.compact[i].skew != p.ranges[i].skew)
+                return SPT_ERR_STATE;
+        }
+    }
+    p.tiling_built = true;
+    return SPT_OK;
+}
+
+static int build_range_auto(const Plan& p, RangePlan& rp, const bool compact) {
+    {
         int rc;
         if (p.opt_max_ent != 0) {                 // fixed by the caller (A/B runs, tests)
-            if ((rc = build_range(p, rp, p.opt_group ? p.opt_group : (p.opt_max_ent > 8 ? 16 : 8), p.opt_max_ent)) != SPT_OK) return rc;
-            continue;
+            return build_range(p, rp, p.opt_group ? p.opt_group : (p.opt_max_ent > 8 ? 16 : 8), p.opt_max_ent, compact);
         }
         // default: groups of up to 8 entries, or of up to 12 where the model says the smaller gather outweighs the costlier
         // pre-sum (bands whose sweeps are short: few variants per group) -- by a margin for the decimated ranges, whose
         // pre-sum the constants fit less well
-        if ((rc = build_range(p, rp, p.opt_group ? p.opt_group : 8, 8)) != SPT_OK) return rc;
-        if (p.opt_group != 0 && p.opt_group <= 8) continue;
+        if ((rc = build_range(p, rp, p.opt_group ? p.opt_group : 8, 8, compact)) != SPT_OK) return rc;
+        if (p.opt_group != 0 && p.opt_group <= 8) return SPT_OK;
         const double c8 = modelled_cost(rp);
         RangePlan alt = rp;
-        if (build_range(p, alt, p.opt_group ? p.opt_group : 16, 12) != SPT_OK) continue;
-        if (modelled_cost(alt) < c8 * (rp.decim == 1 ? 0.97 : 0.90)) rp = std::move(alt);
+        if (build_range(p, alt, p.opt_group ? p.opt_group : 16, 12, compact) != SPT_OK) return SPT_OK;
+        if (modelled_cost(alt) < c8 * ((rp.decim == 1 || compact) ? 0.97 : 0.90)) rp = std::move(alt);
     }
-    p.tiling_built = true;
     return SPT_OK;
 }
 

@@ -82,7 +82,8 @@ def test_options_and_state_errors(api):
     p.set_option("dedisp_kernel", 1)
     p.set_option("skew", 0)
     p.set_option("max_entries", 12)
-    for name, v in (("group", 3), ("dm_tile", 48), ("dedisp_kernel", 2), ("skew", 2), ("max_entries", 10), ("nonsense", 1)):
+    p.set_option("compact", 0)
+    for name, v in (("group", 3), ("dm_tile", 48), ("dedisp_kernel", 2), ("skew", 2), ("max_entries", 10), ("compact", 2), ("nonsense", 1)):
         with pytest.raises(api.SptError) as e:
             p.set_option(name, v)
         assert e.value.code == api.SPT_ERR_INVALID

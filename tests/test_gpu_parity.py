@@ -96,7 +96,7 @@ def mini3(synth, seed, nsamp=65536, nchan=1024):
 
 @pytest.mark.parametrize("options", [{"group": 4}, {"group": 8}, {"group": 2, "dm_tile": 32}, {"dedisp_kernel": 1},
                                      {"group": 8, "skew": 0}, {"group": 16, "max_entries": 12},
-                                     {"group": 16, "max_entries": 16}])
+                                     {"group": 16, "max_entries": 16}, {"compact": 0}, {"compact": 0, "max_entries": 12}])
 def test_multirange_decimated_bit_exact(cuda, api, orc, synth, options):
     w = mini3(synth, 11)
     fb = synth.generate(w)
