@@ -412,12 +412,16 @@ class Measurement:
             elif k == 1:
                 kdec = int(dec[rg == r][0])
                 nbytes = (w.nchan * w.nsamp + 2 * w.nchan * (w.nsamp // kdec)) * w.nbeam
+                if not any(o.startswith("compact=0") for o in (self.args.opt or [])):
+                    nbytes += 3 * w.nchan * (w.nsamp // kdec) * w.nbeam      # the 8-bit copy: uint16 series read, bytes written
                 out[f"decimate_range{r}"] = {"bound": "hbm", "bytes": nbytes, "ms": ms, "achieved_gbs": nbytes / ms / 1e6,
-                                             "frac": nbytes / ms / 1e6 / hbm_gbs}
+                                             "frac": nbytes / ms / 1e6 / hbm_gbs,
+                                             "span": "decimation + bounds pass + 8-bit copy of the series"}
             elif k == 3:
                 nbytes = 4 * int(nout.astype("int64").sum()) * w.nbeam
                 out["single_pulse_search"] = {"bound": "hbm", "bytes": nbytes, "ms": ms, "achieved_gbs": nbytes / ms / 1e6,
-                                              "frac": nbytes / ms / 1e6 / hbm_gbs}
+                                              "frac": nbytes / ms / 1e6 / hbm_gbs,
+                                             "span": "decimation + bounds pass + 8-bit copy of the series"}
         return out
 
 

@@ -384,11 +384,7 @@ __device__ __forceinline__ void dedisp_tile_body(const TiledArgs& a) {
     const uint32_t var_addr = smem_u32(s_var), raw_addr = smem_u32(s_rawb);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    uint32_t bias = 0u;
-    if (a.enable != nullptr) {
-        if (__ldg(a.enable) != a.enable_want) return;            // the other launch of this range does the work
-        if (a.enable_want == 1u) bias = __ldg(a.enable + 1);
-    }
+    if (a.enable != nullptr && __ldg(a.enable) != a.enable_want) return;     // the other launch of this range does the work
     int bid = blockIdx.x;
     const int dmt = bid % a.ntile_dm; bid /= a.ntile_dm;
     const int ntt = a.tail > 0 ? a.tail_tiles : a.ntile_t;
@@ -483,6 +479,9 @@ __device__ __forceinline__ void dedisp_tile_body(const TiledArgs& a) {
     const uint32_t floor1 = (t0 < (int64_t)a.skew_max + 32 || vmin > vmax) ? 0u : vmin;
     const uint32_t floor2 = floor1 * 0x00010001u;
     const int lane_cap = (int)(65535u / max(1u, vmax - floor1));
+    // what every channel summed owes when the lanes are widened: the floor taken off its samples here and, for the 8-bit
+    // copy of a decimated series, the floor the copy was made with
+    const uint32_t back1 = floor1 + ((a.enable != nullptr && a.enable_want == 1u) ? __ldg(a.enable + 1) : 0u);
     int since = 0;
     // A warp none of whose trials has an output in this tile (the last DM tile of a range holds fewer than DT trials; rows end
     // at different samples; a stream push wants only the tail) still does its share of the pre-sums but neither gathers nor
@@ -496,7 +495,7 @@ __device__ __forceinline__ void dedisp_tile_body(const TiledArgs& a) {
     auto flush_lanes = [&]() {
         if (!warp_live) return;
         const uint64_t pol_out = policy_evict_last();
-        const uint32_t back = (uint32_t)since * (floor1 + bias);   // the floor of the channels summed since the last pass
+        const uint32_t back = (uint32_t)since * back1;    // the floor of the channels summed since the last pass
 #pragma unroll
         for (int q = 0; q < TPW; ++q) {
             const int dl = warp * TPW + q;
