@@ -390,3 +390,28 @@ def test_candidate_overflow_is_reported(cuda, api, synth):
     ncand, ovf = plan.search_host(fb[None], 2.0)
     assert ovf and ncand > 3
     assert plan.candidates_read().size == 3
+
+
+# ---- the degenerate corners of the plan space ------------------------------------------------------------------
+@pytest.mark.parametrize("case", [
+    dict(nchan=1, nsamp=64, ranges=[(0.0, 1.0, 1, 1)], widths=[1, 2], thr=-1e9),            # one channel, one trial: out = in
+    dict(nchan=3, nsamp=16, ranges=[(0.0, 5.0, 2, 1)], widths=[1, 64], thr=0.5),             # a width longer than the rows
+    dict(nchan=5, nsamp=200, ranges=[(0.0, 1.0, 3, 64)], widths=[1, 2], thr=-1e9),           # decimation 64: rows of 3 samples
+    dict(nchan=64, nsamp=515, ranges=[(0.0, 0.5, 130, 1), (65.0, 1.0, 2, 2)], widths=[1, 3, 9], thr=-1e9),   # every start a candidate
+    dict(nchan=4096, nsamp=600, ranges=[(0.0, 0.05, 65, 1)], widths=[1], thr=3.0),           # rows shorter than two tiles, 65 trials
+])
+def test_degenerate_plans(cuda, api, orc, case):
+    nchan = case["nchan"]
+    w = Shape(500.0, -200.0 / nchan, nchan, case["nsamp"], case["ranges"], case["widths"], case["thr"])
+    rs = np.random.default_rng(nchan + case["nsamp"])
+    fb = rs.integers(0, 256, size=(nchan, w.nsamp), dtype=np.uint8)
+    ref = oracle_path(orc, w, fb)
+    plan, dmt, cands = run_gpu(cuda, api, w, fb[None])
+    check_plan_against_oracle(orc, plan, w)
+    check_dmt_against_oracle(plan, dmt, ref)
+    check_stats_against_oracle(plan, ref)
+    st = check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+    if case["thr"] < -1e8:                      # every start position of every row with a non-zero variance is a candidate, once
+        assert st["gpu"] == st["oracle"] == st["matched"] > 0
+    if nchan == 1:
+        assert np.array_equal(dmt[0][: w.nsamp], fb[0].astype(np.int32))
