@@ -112,6 +112,9 @@ int spt_plan_delays(const spt_plan* plan, int32_t trial, int32_t* host_out);
  *                    step is about 3 % slower.  Leave it 0 for production and for end-to-end timing.
  *   "max_entries":   largest pre-summed group of the tiled kernel in entries (a channel at one of its shifts): 8, 12 or 16;
  *                    default: chosen per DM range by the cost model
+ *   "tile_words":    width of the tiled kernel's time tile in packed words (the tile is twice as many outputs): 224 or 256
+ *                    (224 only with dm_tile = 64); default 0: chosen per DM range by the cost model together with the
+ *                    entry cap
  *   "compact":       1 (default) = a decimated range is dedispersed from an 8-bit copy of its series (sample - smallest
  *                    sample) whenever the series spans fewer than 256 values -- decided on the device per call; 0 = always
  *                    from the uint16 series; same results

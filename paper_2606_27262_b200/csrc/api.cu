@@ -361,7 +361,7 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
                     int32_t first = INT32_MAX;
                     for (int t = 0; t < td.ntrial; ++t) {
                         const int32_t n = rp.nout[td.trial0 + t];
-                        if (n > 0) first = std::min(first, (std::max(0, n - tail) + rp.skew[(size_t)td.skew0 + t]) / kTT);
+                        if (n > 0) first = std::min(first, (std::max(0, n - tail) + rp.skew[(size_t)td.skew0 + t]) / (2 * rp.kh));
                     }
                     if (td.tt_last >= 0 && first != INT32_MAX) tail_tiles = std::max(tail_tiles, td.tt_last - first + 1);
                 }
@@ -386,9 +386,9 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
                 const RangePlan& cp = p->compact[i];
                 TiledArgs a8 = args_of(cp, rd.series8, rd.c_tiles, rd.c_sidx, rd.c_rows, rd.c_blob, rd.c_skew, rd.cinfo);
                 a8.enable = rd.cinfo + 2; a8.enable_want = 1u;
-                rc = launch_dedisp_dual(p->opt_dm_tile, rp.max_ent, a8, a16, st);
+                rc = launch_dedisp_dual(p->opt_dm_tile, rp.max_ent, rp.kh, a8, a16, st);
             } else {
-                rc = launch_dedisp_tiled(u16, p->opt_dm_tile, rp.max_ent, a16, st);
+                rc = launch_dedisp_tiled(u16, p->opt_dm_tile, rp.max_ent, rp.kh, a16, st);
             }
             if (rc != 0) { g_last_error = "dedisp_tiled: launch configuration rejected"; return SPT_ERR_CUDA; }
         }
@@ -605,6 +605,10 @@ int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value) {
     } else if (!std::strcmp(name, "group")) {
         if (value != 1 && value != 2 && value != 4 && value != 8 && value != 12 && value != 16) return SPT_ERR_INVALID;
         p.opt_group = (int32_t)value; p.tiling_built = false;
+    } else if (!std::strcmp(name, "tile_words")) {
+        if (value != 0 && value != 224 && value != 256) return SPT_ERR_INVALID;
+        if (value == 224 && p.opt_dm_tile != 64) return SPT_ERR_INVALID;
+        p.opt_kh = (int32_t)value; p.tiling_built = false;
     } else if (!std::strcmp(name, "max_entries")) {
         if (value != 8 && value != 12 && value != 16) return SPT_ERR_INVALID;
         p.opt_max_ent = (int32_t)value; p.tiling_built = false;
@@ -613,6 +617,7 @@ int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value) {
         p.opt_skew = (int32_t)value; p.tiling_built = false;
     } else if (!std::strcmp(name, "dm_tile")) {
         if (value != 32 && value != 64) return SPT_ERR_INVALID;
+        if (value != 64 && p.opt_kh == 224) return SPT_ERR_INVALID;          // the narrow tile exists for 64-trial tiles only
         p.opt_dm_tile = (int32_t)value; p.tiling_built = false;
     } else {
         return SPT_ERR_INVALID;

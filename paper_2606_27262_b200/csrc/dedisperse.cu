@@ -267,8 +267,9 @@ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
 // addr: shared-memory byte address of the aligned 32-bit word holding the lane's first sample; c1: the entry's second
 // descriptor word (uint8: bits 0-4 = 8 * position of that sample inside the word, bits 8-23 = PRMT selector of sample 4;
 // uint16: bits 0-1 = position inside the 8-byte unit the address points at).
-template <typename T>
+template <typename T, int KH>
 __device__ __forceinline__ void load_entry(uint32_t addr, uint32_t c1, uint32_t (&w)[5]) {
+    constexpr int kH = KH;
     if (sizeof(T) == 1) {
         const uint32_t aL = lds32(addr), bL = lds32(addr + 4), aH = lds32(addr + kH), bH = lds32(addr + kH + 4);
         uint32_t Lw, Hw;   // samples 0..3 (the shift amount is taken modulo 32: the selector bits above do not matter)
@@ -301,7 +302,7 @@ __device__ __forceinline__ void load_entry(uint32_t addr, uint32_t c1, uint32_t 
 // B: one warp task = kChunkU variant words (4 per lane) of every variant of one group.  All control flow is warp
 // uniform and the NE entries are straight-line code (unused entries repeat the first one; their deltas are never
 // taken): a lane past the end of the variants works on the last four words and does not store.
-template <typename T, int NE>
+template <typename T, int NE, int KH>
 __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uint32_t task, uint32_t var_addr,
                                             uint32_t raw_addr, int lane, uint32_t floor2, const uint4 gh) {
     const int vlen = (int)gh.y;
@@ -326,7 +327,7 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
             const int q = 2 * q2 + h;
             const uint32_t cx = h ? c2.z : c2.x, cy = h ? c2.w : c2.y;
             uint32_t w[5];
-            load_entry<T>(rbase + (cx & 0x3ffffu), cy, w);
+            load_entry<T, KH>(rbase + (cx & 0x3ffffu), cy, w);
 #pragma unroll
             for (int i = 0; i < 4; ++i) dl[q][i] = w[i + 1] - w[i];
             if (cx & kEntryAddBase) {
@@ -366,8 +367,10 @@ __device__ __forceinline__ void presum_task(const uint32_t* __restrict__ tb, uin
 
 // NEMAX: the largest entry class the plan's tables hold (8, 12 or 16): the kernel carries only the pre-sum instances it
 // needs, so that a plan of small groups does not pay for the registers of the large ones.
-template <typename T, int DT, int NEMAX>
+// KH: packed words per trial per tile (the tile is 2*KH outputs wide): 256, or 224 where the plan's cost model prefers it.
+template <typename T, int DT, int NEMAX, int KH>
 __device__ __forceinline__ void dedisp_tile_body(const TiledArgs& a) {
+    constexpr int kH = KH, kTT = 2 * KH;
     constexpr int NW = kThreads / 32;
     constexpr int TPW = DT / NW;
     constexpr int NJ = kH / 32;
@@ -532,9 +535,9 @@ __device__ __forceinline__ void dedisp_tile_body(const TiledArgs& a) {
             const uint32_t task = tb[kBlobHdrWords + 4 * ngrp + tk];
             const uint4 gh = *reinterpret_cast<const uint4*>(tb + kBlobHdrWords + 4 * (task & 0xffu));   // 128-bit broadcast load
             const uint32_t nent = gh.z & 0xffu;       // warp uniform: the smallest straight-line instance that holds the group
-            if (NEMAX == 8 || nent <= 8u) presum_task<T, 8>(tb, task, var_addr, raw_addr, lane, floor2, gh);
-            else if (NEMAX == 12 || nent <= 12u) presum_task<T, 12>(tb, task, var_addr, raw_addr, lane, floor2, gh);
-            else presum_task<T, 16>(tb, task, var_addr, raw_addr, lane, floor2, gh);
+            if (NEMAX == 8 || nent <= 8u) presum_task<T, 8, KH>(tb, task, var_addr, raw_addr, lane, floor2, gh);
+            else if (NEMAX == 12 || nent <= 12u) presum_task<T, 12, KH>(tb, task, var_addr, raw_addr, lane, floor2, gh);
+            else presum_task<T, 16, KH>(tb, task, var_addr, raw_addr, lane, floor2, gh);
         }
         __syncthreads();  // variants complete; raw rows and the other blob buffer are free
         if (s + 1 < td.nstage) issue_stage(s + 1);
@@ -583,18 +586,18 @@ __device__ __forceinline__ void dedisp_tile_body(const TiledArgs& a) {
     flush_lanes();
 }
 
-template <typename T, int DT, int NEMAX>
+template <typename T, int DT, int NEMAX, int KH>
 __global__ void __launch_bounds__(kThreads, 2) dedisp_tiled_kernel(const TiledArgs a) {
-    dedisp_tile_body<T, DT, NEMAX>(a);
+    dedisp_tile_body<T, DT, NEMAX, KH>(a);
 }
 
 // A decimated range in ONE launch: the 8-bit copy of its series with the copy's tables when the copy was made (a8.enable
 // points at {flag, bias}, written on the device just before), the uint16 series with its own tables otherwise.  The two
 // table sets tile the range identically (same DM tiles, same skews, same grid), so a block does the same tile either way.
-template <int DT, int NEMAX>
+template <int DT, int NEMAX, int KH>
 __global__ void __launch_bounds__(kThreads, 2) dedisp_dual_kernel(const TiledArgs a8, const TiledArgs a16) {
-    if (__ldg(a8.enable) == 1u) dedisp_tile_body<uint8_t, DT, NEMAX>(a8);
-    else dedisp_tile_body<uint16_t, DT, NEMAX>(a16);
+    if (__ldg(a8.enable) == 1u) dedisp_tile_body<uint8_t, DT, NEMAX, KH>(a8);
+    else dedisp_tile_body<uint16_t, DT, NEMAX, KH>(a16);
 }
 
 // the opt-in to 113 KB of dynamic shared memory is a per-device attribute of the function: one flag per device and instance
@@ -614,10 +617,10 @@ static int64_t blocks_of(const TiledArgs& a) {
     return (int64_t)a.ntile_dm * (a.tail > 0 ? a.tail_tiles : a.ntile_t) * a.nbeam;
 }
 
-template <typename T, int DT, int NEMAX>
+template <typename T, int DT, int NEMAX, int KH>
 static int launch_tiled_inst(const TiledArgs& a, cudaStream_t st) {
     static std::atomic<bool> attr_set[64];
-    auto kern = dedisp_tiled_kernel<T, DT, NEMAX>;
+    auto kern = dedisp_tiled_kernel<T, DT, NEMAX, KH>;
     if (opt_in_smem(kern, attr_set) != 0) return -1;
     const int64_t nblocks = blocks_of(a);
     if (nblocks <= 0) return 0;
@@ -626,15 +629,10 @@ static int launch_tiled_inst(const TiledArgs& a, cudaStream_t st) {
     return 0;
 }
 
-template <int DT, int NEMAX>
-static int launch_tiled_type(bool is_u16, const TiledArgs& a, cudaStream_t st) {
-    return is_u16 ? launch_tiled_inst<uint16_t, DT, NEMAX>(a, st) : launch_tiled_inst<uint8_t, DT, NEMAX>(a, st);
-}
-
-template <int DT, int NEMAX>
+template <int DT, int NEMAX, int KH>
 static int launch_dual_inst(const TiledArgs& a8, const TiledArgs& a16, cudaStream_t st) {
     static std::atomic<bool> attr_set[64];
-    auto kern = dedisp_dual_kernel<DT, NEMAX>;
+    auto kern = dedisp_dual_kernel<DT, NEMAX, KH>;
     if (opt_in_smem(kern, attr_set) != 0) return -1;
     const int64_t nblocks = blocks_of(a16);
     if (nblocks != blocks_of(a8)) return -1;
@@ -644,24 +642,30 @@ static int launch_dual_inst(const TiledArgs& a8, const TiledArgs& a16, cudaStrea
     return 0;
 }
 
-int launch_dedisp_dual(int DT, int max_ent, const TiledArgs& a8, const TiledArgs& a16, cudaStream_t st) {
-    if (DT == 64 && max_ent == 8) return launch_dual_inst<64, 8>(a8, a16, st);
-    if (DT == 64 && max_ent == 12) return launch_dual_inst<64, 12>(a8, a16, st);
-    if (DT == 64 && max_ent == 16) return launch_dual_inst<64, 16>(a8, a16, st);
-    if (DT == 32 && max_ent == 8) return launch_dual_inst<32, 8>(a8, a16, st);
-    if (DT == 32 && max_ent == 12) return launch_dual_inst<32, 12>(a8, a16, st);
-    if (DT == 32 && max_ent == 16) return launch_dual_inst<32, 16>(a8, a16, st);
+// Instances: 64-trial tiles at both tile widths, 32-trial tiles (option dm_tile, tests) at the wide one only.
+#define SPT_DISPATCH(CALL)                                                                   \
+    if (DT == 64 && kh == 256 && max_ent == 8) return CALL(64, 8, 256);                       \
+    if (DT == 64 && kh == 256 && max_ent == 12) return CALL(64, 12, 256);                     \
+    if (DT == 64 && kh == 256 && max_ent == 16) return CALL(64, 16, 256);                     \
+    if (DT == 64 && kh == 224 && max_ent == 8) return CALL(64, 8, 224);                       \
+    if (DT == 64 && kh == 224 && max_ent == 12) return CALL(64, 12, 224);                     \
+    if (DT == 64 && kh == 224 && max_ent == 16) return CALL(64, 16, 224);                     \
+    if (DT == 32 && kh == 256 && max_ent == 8) return CALL(32, 8, 256);                       \
+    if (DT == 32 && kh == 256 && max_ent == 12) return CALL(32, 12, 256);                     \
+    if (DT == 32 && kh == 256 && max_ent == 16) return CALL(32, 16, 256);                     \
     return -1;
+
+int launch_dedisp_dual(int DT, int max_ent, int kh, const TiledArgs& a8, const TiledArgs& a16, cudaStream_t st) {
+#define SPT_CALL_DUAL(D, N, K) launch_dual_inst<D, N, K>(a8, a16, st)
+    SPT_DISPATCH(SPT_CALL_DUAL)
+#undef SPT_CALL_DUAL
 }
 
-int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, const TiledArgs& a, cudaStream_t st) {
-    if (DT == 64 && max_ent == 8) return launch_tiled_type<64, 8>(is_u16, a, st);
-    if (DT == 64 && max_ent == 12) return launch_tiled_type<64, 12>(is_u16, a, st);
-    if (DT == 64 && max_ent == 16) return launch_tiled_type<64, 16>(is_u16, a, st);
-    if (DT == 32 && max_ent == 8) return launch_tiled_type<32, 8>(is_u16, a, st);
-    if (DT == 32 && max_ent == 12) return launch_tiled_type<32, 12>(is_u16, a, st);
-    if (DT == 32 && max_ent == 16) return launch_tiled_type<32, 16>(is_u16, a, st);
-    return -1;
+int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, int kh, const TiledArgs& a, cudaStream_t st) {
+#define SPT_CALL_TILED(D, N, K) (is_u16 ? launch_tiled_inst<uint16_t, D, N, K>(a, st) : launch_tiled_inst<uint8_t, D, N, K>(a, st))
+    SPT_DISPATCH(SPT_CALL_TILED)
+#undef SPT_CALL_TILED
 }
+#undef SPT_DISPATCH
 
 }  // namespace spt

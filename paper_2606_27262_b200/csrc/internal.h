@@ -20,8 +20,8 @@ constexpr int kMaxWidths = 32;
 // ---- tiled dedispersion kernel geometry ------------------------------------------------
 // A block owns DT trials x TT = 2*H output samples; two blocks are resident per SM.  Packed 16-bit accumulator
 // word q of a trial holds the outputs t0+q (low half) and t0+H+q (high half).
-constexpr int kH = 256;              // words per trial per tile
-constexpr int kTT = 2 * kH;          // output samples per tile
+constexpr int kHMax = 256;           // words per trial per tile, at most: a tile is 2*kh output samples wide, kh = 224 or 256 per
+                                     // DM range (RangePlan::kh; the kernel is a template on it)
 constexpr int kThreads = 256;        // 8 warps
 constexpr int kMaxEnt = 16;          // entries (a channel at one of its shifts) per pre-summed group, at most; the pre-sum code
                                      // exists for groups of up to 8, 12 and 16 entries (ent_class)
@@ -105,6 +105,7 @@ struct RangePlan {
     int32_t skew_max = 0;
     int32_t vcap_words = 0;          // words of the variant region; the raw region follows it
     int32_t max_ent = 8;             // entry cap the tables were built for: selects the kernel instance
+    int32_t kh = kHMax;              // packed words per trial per tile the tables were built for (tile = 2*kh outputs)
     int32_t ntile_t = 0;             // time tiles
     int64_t ngroups = 0, nvariants = 0, ncorrected = 0;   // totals, for reports (ncorrected: variants off the prefix chain)
     // work of the pre-sum over all DM tiles, for the cost model that picks the entry cap (build_tiling) and for reports:
@@ -129,6 +130,7 @@ struct Plan {
     // options
     int32_t opt_kernel = 0;          // 0 tiled, 1 naive
     int32_t opt_group = 0;           // channels per group, at most (0: 8 or 16, with the entry cap)
+    int32_t opt_kh = 0;              // tile width in packed words: 224 or 256 (0: chosen per range by the cost model)
     int32_t opt_max_ent = 0;         // entries per group, at most: 8, 12 or 16 (0: chosen per range by the cost model)
     int32_t opt_dm_tile = 64;
     int32_t opt_profile = 0;

@@ -43,10 +43,10 @@ struct TiledArgs {
     uint32_t enable_want;      // range is enqueued on its 8-bit copy and on the uint16 series; the copy may not exist) and
                                // every channel summed owes `bias` (the floor the 8-bit copy was made with) when want == 1
 };
-int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, const TiledArgs& a, cudaStream_t st);
+int launch_dedisp_tiled(bool is_u16, int DT, int max_ent, int kh, const TiledArgs& a, cudaStream_t st);
 // a decimated range in one launch: a8 = the 8-bit copy of the series (a8.enable -> {valid flag, bias}, a8.enable_want = 1), a16
 // = the uint16 series (a16.enable = NULL); the block takes whichever the flag says
-int launch_dedisp_dual(int DT, int max_ent, const TiledArgs& a8, const TiledArgs& a16, cudaStream_t st);
+int launch_dedisp_dual(int DT, int max_ent, int kh, const TiledArgs& a8, const TiledArgs& a16, cudaStream_t st);
 void launch_compact_u16(const uint16_t* y, uint8_t* c, int64_t nelem, const uint32_t* maxval, uint32_t* info, cudaStream_t st);
 
 struct SpsArgs {

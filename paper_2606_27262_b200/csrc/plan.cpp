@@ -90,6 +90,9 @@ const RangePlan* range_of_trial(const Plan& p, int32_t trial, int32_t* local) {
 // -------------------------------------------------------------------------------------------------------------
 namespace {
 
+// cost model of build_range_auto (see modelled_cost)
+constexpr double kCostGroup = 2.348, kCostStage = 0.876, kCostPresum = 0.02205, kPen12Wide = 1.6, kPen12Narrow = 1.5;
+
 struct PendingVariant { int k; uint32_t plus, minus, bits; };
 
 struct PendingEntry { int j, level; bool addbase; int ones; };   // one pre-sum entry: channel offset j at shift s_j + level
@@ -124,6 +127,7 @@ static bool make_group(const Plan& p, const RangePlan& rp, int32_t d0, int32_t n
         dmin = std::min(dmin, v); dmax = std::max(dmax, v);
     }
     g.dmin = dmin;
+    const int kH = rp.kh;
     g.vlen = (int32_t)round_up(kH + (dmax - dmin), 4);
     g.b.resize(ntrial);
     for (int i = 0; i < ntrial; ++i) g.b[i] = rp.delay[(size_t)(d0 + i) * p.nchan + c0] - skew[i] - dmin;
@@ -217,6 +221,7 @@ static bool make_group(const Plan& p, const RangePlan& rp, int32_t d0, int32_t n
 // byte): one byte per element and, like the raw input, at most 255 per sample whatever the decimation.
 static int build_range(const Plan& p, RangePlan& rp, const int G, const int max_ent, const bool compact = false) {
     const int DT = p.opt_dm_tile;
+    const int kTT = 2 * rp.kh;           // rp.kh is set by the caller
     rp.max_ent = max_ent;
     {
         rp.tiles.clear(); rp.sidx.clear(); rp.rows.clear(); rp.blob.clear();
@@ -433,16 +438,20 @@ static int build_range(const Plan& p, RangePlan& rp, const int G, const int max_
     return SPT_OK;
 }
 
-// Modelled time of a range's launch per time tile, arbitrary units ("entry cap"): the gather and the
-// stage loop cost per group, the pre-sum per entry processed and variant stored; the 12- and 16-entry pre-sum instances run
-// 1.5x and 2.1x slower per unit than the 8-entry one (register pressure: fewer loads in flight).  Constants fitted to the
-// range-0 launches of configs 3 and 6 measured with caps 8, 12 and 16.
+// Modelled time of a range's launch, in ms per beam up to a common factor ("Entry cap and tile
+// width"): per time tile the gather costs per group in proportion to the tile width, the stage loop per stage, the pre-sum
+// per entry processed and variant stored; the 12- and 16-entry pre-sum instances run slower per unit of work than the
+// 8-entry one (register pressure: fewer loads in flight).  Constants fitted to eight measured range-0 launches -- configs 3
+// and 6 at tile widths 224 / 256 and caps 8 / 12 -- which the model reproduces within 0.3 ms (1.5 %).
 static double modelled_cost(const RangePlan& rp) {
-    const double pen = rp.max_ent <= 8 ? 1.0 : rp.max_ent <= 12 ? 1.5 : 2.1;
-    return 2.456e-3 * (double)rp.ngroups + 2.37e-5 * pen * (double)(rp.task_entries + rp.task_variants);
+    const bool wide = rp.kh >= 256;
+    const double pen = rp.max_ent <= 8 ? 1.0 : rp.max_ent <= 12 ? (wide ? kPen12Wide : kPen12Narrow) : (wide ? 2.2 : 2.0);
+    const double nstage = (double)rp.sidx.size() - 1.0;
+    const double tile = kCostGroup * (double)rp.ngroups * ((double)rp.kh / 256.0) + kCostStage * nstage +
+                        kCostPresum * pen * (double)(rp.task_entries + rp.task_variants);
+    return 1e-6 * (double)rp.ntile_t * tile;
 }
 
-// The same choice of entry cap for either element size.
 static int build_range_auto(const Plan& p, RangePlan& rp, bool compact);
 
 int build_tiling(Plan& p) {
@@ -453,12 +462,13 @@ int build_tiling(Plan& p) {
         if ((rc = build_range_auto(p, p.ranges[i], false)) != SPT_OK) return rc;
         if (p.ranges[i].decim > 1 && p.opt_compact) {
             // second set of tables for the 8-bit copy of the decimated series (the delay table is shared by value: a few MB)
-            // Both sets run in one kernel instance, so they share the entry cap: the copy's choice (it is the set that runs
-            // on well-behaved data), and the same DM tiles and skews, so that a block does the same tile either way.
+            // Both sets run in one kernel instance, so they share tile width and entry cap: the copy's choice (it is the set
+            // that runs on well-behaved data), and the same DM tiles and skews, so that a block does the same tile either way.
             p.compact[i] = p.ranges[i];
             if ((rc = build_range_auto(p, p.compact[i], true)) != SPT_OK) return rc;
-            if (p.compact[i].max_ent != p.ranges[i].max_ent) {
+            if (p.compact[i].max_ent != p.ranges[i].max_ent || p.compact[i].kh != p.ranges[i].kh) {
                 const int G = p.opt_group ? p.opt_group : (p.compact[i].max_ent > 8 ? 16 : 8);
+                p.ranges[i].kh = p.compact[i].kh;
                 if ((rc = build_range(p, p.ranges[i], G, p.compact[i].max_ent, false)) != SPT_OK) return rc;
             }
             if (p.compact[i].ntile_t != p.ranges[i].ntile_t || p.compact[i].tiles.size() != p.ranges[i].tiles.size() ||
@@ -470,22 +480,39 @@ int build_tiling(Plan& p) {
     return SPT_OK;
 }
 
+// Tile width and entry cap of one range: what the caller fixed (A/B runs, tests), else the cheapest by the model of
+// {256, 224 words} x {8, 12 entries} -- wide tiles and small groups for long sweeps (every channel of a group toggles
+// within a DM tile, the pre-sum dominates), narrower tiles and larger groups where sweeps are short (a variant plus its
+// small halo then fills two pre-sum tasks instead of spilling into a third).
 static int build_range_auto(const Plan& p, RangePlan& rp, const bool compact) {
-    {
-        int rc;
-        if (p.opt_max_ent != 0) {                 // fixed by the caller (A/B runs, tests)
-            return build_range(p, rp, p.opt_group ? p.opt_group : (p.opt_max_ent > 8 ? 16 : 8), p.opt_max_ent, compact);
+    const int khs[2] = {256, 224};
+    const int caps[2] = {8, 12};
+    bool have = false;
+    double best = 0.0;
+    RangePlan keep;
+    for (int kh : khs) {
+        if (p.opt_kh != 0 && kh != p.opt_kh) continue;
+        if (p.opt_kh == 0 && kh != 256 && p.opt_dm_tile != 64) continue;     // the narrow tile exists for 64-trial tiles only
+        for (int cap : caps) {
+            if (p.opt_max_ent != 0 && cap != p.opt_max_ent && !(p.opt_max_ent == 16 && cap == 12)) continue;
+            const int use_cap = (p.opt_max_ent == 16) ? 16 : cap;
+            if (p.opt_max_ent == 0 && p.opt_group != 0 && p.opt_group <= 8 && cap > 8) continue;
+            RangePlan cand = rp;
+            cand.kh = kh;
+            const int G = p.opt_group ? p.opt_group : (use_cap > 8 ? 16 : 8);
+            const int rc = build_range(p, cand, G, use_cap, compact);
+            if (rc != SPT_OK) {
+                if (!have && kh == khs[1] && cap == caps[1]) return rc;
+                continue;
+            }
+            // a margin for the decimated uint16 series, whose pre-sum the constants fit less well: stay with the default there
+            double c = modelled_cost(cand);
+            if (!(kh == 256 && use_cap == 8)) c *= (rp.decim == 1 || compact) ? 1.03 : 1.10;
+            if (!have || c < best) { best = c; keep = std::move(cand); have = true; }
         }
-        // default: groups of up to 8 entries, or of up to 12 where the model says the smaller gather outweighs the costlier
-        // pre-sum (bands whose sweeps are short: few variants per group) -- by a margin for the decimated ranges, whose
-        // pre-sum the constants fit less well
-        if ((rc = build_range(p, rp, p.opt_group ? p.opt_group : 8, 8, compact)) != SPT_OK) return rc;
-        if (p.opt_group != 0 && p.opt_group <= 8) return SPT_OK;
-        const double c8 = modelled_cost(rp);
-        RangePlan alt = rp;
-        if (build_range(p, alt, p.opt_group ? p.opt_group : 16, 12, compact) != SPT_OK) return SPT_OK;
-        if (modelled_cost(alt) < c8 * ((rp.decim == 1 || compact) ? 0.97 : 0.90)) rp = std::move(alt);
     }
+    if (!have) return SPT_ERR_UNSUPPORTED;
+    rp = std::move(keep);
     return SPT_OK;
 }
 

@@ -83,7 +83,8 @@ def test_options_and_state_errors(api):
     p.set_option("skew", 0)
     p.set_option("max_entries", 12)
     p.set_option("compact", 0)
-    for name, v in (("group", 3), ("dm_tile", 48), ("dedisp_kernel", 2), ("skew", 2), ("max_entries", 10), ("compact", 2), ("nonsense", 1)):
+    p.set_option("tile_words", 256)
+    for name, v in (("group", 3), ("dm_tile", 48), ("dedisp_kernel", 2), ("skew", 2), ("max_entries", 10), ("compact", 2), ("tile_words", 192), ("nonsense", 1)):
         with pytest.raises(api.SptError) as e:
             p.set_option(name, v)
         assert e.value.code == api.SPT_ERR_INVALID
@@ -113,18 +114,23 @@ def test_plan_cfg4_zero_length_trials(api, orc, synth):
 
 @pytest.mark.parametrize("group,dm_tile,skew,max_ent", [(1, 64, 1, 8), (2, 64, 1, 8), (4, 64, 1, 8), (8, 64, 1, 8), (4, 32, 1, 8),
                                                         (8, 64, 0, 8), (12, 64, 1, 12), (16, 64, 1, 12), (16, 64, 1, 16),
-                                                        (16, 32, 0, 16)])
+                                                        (16, 32, 0, 16), (8, 64, 1, -8), (16, 64, 1, -12), (0, 64, 1, 0)])
 def test_tiling_tables_reproduce_the_delay_table(api, synth, group, dm_tile, skew, max_ent):
     """Host logic of the tiled kernel: the (skew, window, variant, offset) factorisation gives back every delay."""
     for cfg, stride in ((1, 1), (3, 173)):
         w = synth.workload(cfg)
-        p = make_plan(api, w, options={"group": group, "dm_tile": dm_tile, "skew": skew, "max_entries": max_ent})
+        opts = {"group": group, "dm_tile": dm_tile, "skew": skew, "max_entries": abs(max_ent)}
+        if max_ent < 0:
+            opts["tile_words"] = 224                      # a negative cap in the parameter list: the narrow time tile
+        if group == 0:
+            opts = {}                                     # everything chosen by the cost model
+        p = make_plan(api, w, options=opts)
         for d in list(range(0, p.ntrials, stride)) + [p.ntrials - 1]:
             assert np.array_equal(p.tiling_delays(d), p.delays(d)), (cfg, d)
         for r in range(len(w.ranges)):
             info = p.tiling_info(r)
             assert info["max_stage_words"] <= 227 * 1024 // 4
-            assert info["ngroups"] >= info["ntiles_dm"] * ((w.nchan + group - 1) // group)
+            assert info["ngroups"] >= info["ntiles_dm"] * ((w.nchan + max(group, 16) - 1) // max(group, 16))
             assert info["nvariants"] <= 16 * info["ngroups"]
 
 

@@ -48,6 +48,7 @@ def oracle_path(orc, w, fb, search=True):
     {"dedisp_kernel": 1},
     {"group": 1}, {"group": 2}, {"group": 4}, {"group": 8}, {"group": 4, "dm_tile": 32}, {"group": 8, "dm_tile": 32},
     {"group": 8, "skew": 0}, {"group": 12, "max_entries": 12}, {"group": 16, "max_entries": 12}, {"group": 16, "max_entries": 16},
+    {"tile_words": 224}, {"tile_words": 224, "max_entries": 12}, {"tile_words": 224, "max_entries": 16, "skew": 0},
 ])
 def test_cfg1_dm_transform_bit_exact(cuda, api, orc, synth, options):
     w = synth.workload(1)
@@ -96,7 +97,8 @@ def mini3(synth, seed, nsamp=65536, nchan=1024):
 
 @pytest.mark.parametrize("options", [{"group": 4}, {"group": 8}, {"group": 2, "dm_tile": 32}, {"dedisp_kernel": 1},
                                      {"group": 8, "skew": 0}, {"group": 16, "max_entries": 12},
-                                     {"group": 16, "max_entries": 16}, {"compact": 0}, {"compact": 0, "max_entries": 12}])
+                                     {"group": 16, "max_entries": 16}, {"compact": 0}, {"compact": 0, "max_entries": 12},
+                                     {"tile_words": 224, "max_entries": 12}, {"tile_words": 224, "compact": 0}])
 def test_multirange_decimated_bit_exact(cuda, api, orc, synth, options):
     w = mini3(synth, 11)
     fb = synth.generate(w)
@@ -129,7 +131,7 @@ def test_multirange_search(cuda, api, orc, synth):
 # ---- odd shapes and degenerate inputs -------------------------------------------------------------------------
 @pytest.mark.parametrize("fill", ["uniform", "all255", "zero"])
 @pytest.mark.parametrize("options", [{"group": 4}, {"group": 8}, {"dedisp_kernel": 1}, {"group": 16, "max_entries": 12},
-                                     {"group": 16, "max_entries": 16}])
+                                     {"group": 16, "max_entries": 16}, {"tile_words": 224}, {"tile_words": 224, "max_entries": 12}])
 def test_odd_shapes(cuda, api, orc, fill, options):
     # 71 channels (not a multiple of any group size), 5003 samples (rows not 16-byte multiples), trial counts that
     # are not multiples of the DM tile, decimation 8, a range whose last trials have no valid output at all
