@@ -126,7 +126,9 @@ int spt_plan_set_option(spt_plan* plan, const char* name, int64_t value);
 
 /* Host-side view of the tables the tiled kernel runs on, for tests and reports; builds them
  * if needed, needs no GPU.  Per range: DM tiles, stages, channel groups and pre-summed variants over all tiles, time
- * tiles, and the largest shared-memory footprint (32-bit words) of a stage.  Any out pointer may be NULL. */
+ * tiles, and the largest shared-memory footprint (32-bit words) of a stage.  Any out pointer may be NULL.  The call also
+ * bounds-checks every shared-memory address the kernel will form from the tables (variant stores, gather reads, the pre-sum's
+ * raw loads incl. the words its aligned loads reach past a sample) and returns SPT_ERR_STATE if one leaves its region. */
 int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int64_t* nstages, int64_t* ngroups,
                          int64_t* nvariants, int64_t* ntiles_t, int64_t* max_stage_words);
 /* Work of the kernel's pre-sum phase over all DM tiles of a range (one time tile each): warp tasks, entries processed by

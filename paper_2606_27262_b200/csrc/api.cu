@@ -634,6 +634,72 @@ static int ensure_tiling(Plan& p) {
     }
 }
 
+// Every shared-memory address the kernel will form from one set of tables stays inside the region it belongs to: the variants
+// inside the variant region, the gather's reads inside the variant they read, the pre-sum's raw loads (the last lane's, in
+// the high half, including the words its aligned loads reach past the sample) inside the row that was staged for them.
+// compute-sanitizer is not available on the GPU pool; this is the bounds check it would have made, done
+// on the host for every stage of every tile.  es: bytes per element of the series the tables address.
+static int check_tables(const Plan& p, const RangePlan& rp, int es) {
+    const int DT = p.opt_dm_tile, kh = rp.kh;
+    const int64_t rcap = kSmemDataBytes - (int64_t)rp.vcap_words * 4;
+    if (rp.vcap_words <= 0 || rcap <= 0 || (kh != 224 && kh != 256)) return SPT_ERR_STATE;
+    for (const TileDesc& td : rp.tiles)
+        if (td.nstage < 1 || td.stage0 < 0 || (size_t)(td.stage0 + td.nstage) + 1 > rp.sidx.size() || td.ntrial < 1 || td.ntrial > DT)
+            return SPT_ERR_STATE;
+    for (size_t is = 0; is + 1 < rp.sidx.size(); ++is) {
+        const StageIndex& si = rp.sidx[is];
+        if (si.blob_words * 4u > (uint32_t)kBlobBytes || si.nrows > (uint32_t)kMaxStageRows || si.nrows < 1) return SPT_ERR_STATE;
+        if ((size_t)si.blob_word0 + si.blob_words > rp.blob.size() || (size_t)si.row0 + si.nrows > rp.rows.size()) return SPT_ERR_STATE;
+        const uint32_t* b = &rp.blob[si.blob_word0];
+        const uint32_t ngrp = b[0];
+        if (ngrp < 1 || ngrp > (uint32_t)kMaxStageGroups || b[3] + ngrp * (uint32_t)DT / 2 > si.blob_words) return SPT_ERR_STATE;
+        int64_t raw_end = 0;
+        for (uint32_t k = 0; k < si.nrows; ++k) {
+            const RowDesc& r = rp.rows[si.row0 + k];
+            if (r.nelem <= 0 || (r.nelem & 15) || (r.soff & 15) || (r.astart & 15) || r.chan < 0 || r.chan >= p.nchan) return SPT_ERR_STATE;
+            raw_end = std::max<int64_t>(raw_end, (int64_t)r.soff + (int64_t)r.nelem * es);
+        }
+        if (raw_end > rcap) return SPT_ERR_STATE;
+        const uint16_t* toff = reinterpret_cast<const uint16_t*>(b + b[3]);
+        for (uint32_t g = 0; g < ngrp; ++g) {
+            const uint32_t* gh = b + kBlobHdrWords + 4 * g;
+            const int64_t vbase = gh[0] & 0xffffu, vlen = gh[1];
+            const int nent = (int)(gh[2] & 0xffu), ntog = (int)((gh[2] >> 8) & 0xffu), ncorr = (int)((gh[2] >> 16) & 0xffu);
+            const int nvar = (int)(gh[2] >> 24);
+            if (vlen < kh || (vlen & 3) || nvar < 1 || nvar > kMaxVar || nent < 1 || nent > kMaxEnt || ntog > nent) return SPT_ERR_STATE;
+            if (vbase + (int64_t)nvar * vlen > rp.vcap_words) return SPT_ERR_STATE;
+            const uint32_t* cd = b + (gh[3] & 0xffffu);
+            const uint32_t* vd = b + (gh[3] >> 16);
+            const int cls = ent_class(nent);
+            // the variants the pre-sum stores: whole variants of this group
+            for (int k = 0; k <= ntog; ++k)
+                if (vd[k] != 0xffffffffu && (vd[k] < vbase || (vd[k] - vbase) % vlen != 0 || (vd[k] - vbase) / vlen >= (uint32_t)nvar))
+                    return SPT_ERR_STATE;
+            for (int c = 0; c < ncorr; ++c) {
+                const uint32_t dst = vd[chain_words(cls) + 2 * c];
+                if (dst < vbase || (dst - vbase) % vlen != 0 || (dst - vbase) / vlen >= (uint32_t)nvar) return SPT_ERR_STATE;
+            }
+            // the gather: trial i reads kh words from its offset, inside one variant
+            for (int i = 0; i < DT; ++i) {
+                const int64_t rel = (int64_t)toff[g * DT + i] - vbase;
+                if (rel < 0 || rel / vlen >= nvar || rel % vlen + kh > vlen) return SPT_ERR_STATE;
+            }
+            // the pre-sum's raw loads: the lane with the last four words (u0 = vlen - 4), low and high half
+            for (int q = 0; q < cls; ++q) {
+                const int64_t w0 = cd[2 * q] & 0x3ffffu;               // aligned word (uint8) / 8-byte unit (uint16) of sample u = 0
+                const int64_t last = es == 1 ? w0 + (vlen - 4) + kh + 8 : w0 + 2 * (vlen - 4) + 2 * kh + 16;
+                bool inside = false;
+                for (uint32_t k = 0; k < si.nrows && !inside; ++k) {
+                    const RowDesc& r = rp.rows[si.row0 + k];
+                    inside = w0 >= r.soff && last <= (int64_t)r.soff + (int64_t)r.nelem * es;
+                }
+                if (!inside) return SPT_ERR_STATE;
+            }
+        }
+    }
+    return SPT_OK;
+}
+
 int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int64_t* nstages, int64_t* ngroups,
                          int64_t* nvariants, int64_t* ntiles_t, int64_t* max_stage_words) {
     if (!plan) return SPT_ERR_INVALID;
@@ -642,6 +708,11 @@ int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int6
     const int rc = ensure_tiling(p);
     if (rc != SPT_OK) return rc;
     const RangePlan& rp = p.ranges[range];
+    {   // bounds check of every address the kernel will form from the tables (both sets of a decimated range)
+        int rcc = check_tables(p, rp, rp.decim == 1 ? 1 : 2);
+        if (rcc == SPT_OK && (size_t)range < p.compact.size() && !p.compact[range].tiles.empty()) rcc = check_tables(p, p.compact[range], 1);
+        if (rcc != SPT_OK) return rcc;
+    }
     if (ntiles_dm) *ntiles_dm = (int64_t)rp.tiles.size();
     if (nstages) *nstages = (int64_t)rp.sidx.size() - 1;   // the last entry is padding
     if (ngroups) *ngroups = rp.ngroups;

@@ -140,6 +140,8 @@ def test_tiling_odd_shapes(api):
                  [1, 3, 7], options={"group": 4})
     for d in range(p.ntrials):
         assert np.array_equal(p.tiling_delays(d), p.delays(d)), d
+    for r in range(3):
+        p.tiling_info(r)              # includes the bounds check of every shared-memory address the tables lead to
 
 
 def test_device_calls_fail_loudly_without_gpu(api):
