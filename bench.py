@@ -678,12 +678,28 @@ def run_stream(args, local_rank):
     e1.record(stream)
     torch.cuda.synchronize()
     ms_whole = e0.elapsed_time(e1) / 4
+    # the corner turn of one block alone (HBM bound: reads and writes nnew x nchan bytes)
+    ct = torch.empty((1, w.nchan, nnew), dtype=torch.uint8, device="cuda")
+
+    def turn(i):
+        rc = api.lib().spt_corner_turn(blocks[i % nblk].data_ptr(), 1, nnew, w.nchan, 0, 1, ct.data_ptr(), stream.cuda_stream)
+        assert rc == 0, rc
+
+    turn(0)
+    e0.record(stream)
+    for i in range(10):
+        turn(i)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_ct = e0.elapsed_time(e1) / 10
+    del ct
     # batch rate on the same GPU for comparison: config 3 as bench.py times it
     mb = Measurement(args, w, 0, 1)
     tb = mb.timed(10, 3, local_rank)
     ms_b = tb["ms_total"] / 10
     out = {"stream": {"nnew": nnew, "history": nsamp - nnew, "min_history_search": hsearch, "nsamp_buffer": nsamp, "pushes": steps,
-                      "ms_per_push": ms, "ms_per_push_whole_rows": ms_whole, "rtf": nnew * w.tsamp / (ms * 1e-3), "adds_new_per_push": adds_new,
+                      "ms_per_push": ms, "ms_per_push_whole_rows": ms_whole, "corner_turn_ms": ms_ct,
+                      "corner_turn_gbs": 2.0 * nnew * w.nchan / ms_ct / 1e6, "rtf": nnew * w.tsamp / (ms * 1e-3), "adds_new_per_push": adds_new,
                       "adds_if_whole_buffer_recomputed": adds_full, "value_new_outputs": adds_new / (ms * 1e-3),
                       "candidates_last_push": ncand, "api": "spt_segment_push + spt_segment_search + spt_candidates_count"},
            "batch": {"workload": w.name, "ms_per_step": ms_b, "rtf": mb.data_s / (ms_b * 1e-3), "value": mb.adds_step / (ms_b * 1e-3)},
