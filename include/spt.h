@@ -218,6 +218,36 @@ int spt_peaks_count(spt_plan* plan, int64_t* total);
 int spt_peaks_read(spt_plan* plan, spt_candidate* host_out /*HOST*/, int64_t cap, int64_t* nwritten);
 
 /* -------------------------------------------------------------------------------------------------------
+ * spt_peak_filter_static -- the same filter (same rule, same tie-break) for callers that must not allocate
+ * device memory: a real-time loop, where a cudaMalloc or cudaFree inside the library would stall every stream of the
+ * device while it runs, and a process whose device memory is already owned by another allocator (a framework's pool
+ * that took the whole card, a fixed partition), where a library allocation fails or eats into someone else's budget.
+ * spt_peak_filter grows its hash table and flag arrays with cudaMalloc; this call never calls cudaMalloc, cudaFree or
+ * any routine that allocates.  Its working memory is a fixed 6.5 MiB block inside the library image, which every GPU
+ * that loads libspt.so holds until the process exits -- hence the limit:
+ *     n <= SPT_PEAKS_STATIC_MAX records; a longer list gets SPT_ERR_UNSUPPORTED (text via spt_last_error) and nothing
+ *     is enqueued.
+ * The caller passes input and output:
+ *   d_cand   DEVICE, n records of a search made with THIS plan (beam >= 0, trial and t inside the plan's rows; the
+ *            (beam, trial, t) of a record occurs once), e.g. copied from spt_candidates_read; not modified
+ *   windows  HOST, as for spt_peak_filter
+ *   d_peaks  DEVICE, room for n records: the survivors, order arbitrary
+ *   d_count  DEVICE, one 64-bit word: set to the number of survivors
+ * Enqueues on cuda_stream and returns; read d_count / d_peaks after synchronising that stream.  The plan's own peak
+ * list (spt_peaks_count / spt_peaks_read) and candidate list are not touched.
+ * SPT_ERR_STATE if the plan has not dedispersed or searched yet (that is where its device tables are made).
+ * First call on a device: it looks up the block's device address (cudaGetSymbolAddress, which also makes the runtime
+ *   load the library's device code if nothing did before); make that first call during set-up, before any stream
+ *   capture.  Later calls on that device only launch kernels.
+ * One block per device, shared by every call, plan and thread: it still holds the previous call's contents (the call
+ *   clears what it needs first), and two calls that overlap on the GPU -- different streams, or different threads --
+ *   race on it and give wrong survivors.  Order them (one stream, or events) yourself.
+ * ----------------------------------------------------------------------------------------------------- */
+#define SPT_PEAKS_STATIC_MAX 262144
+int spt_peak_filter_static(spt_plan* plan, const spt_candidate* d_cand /*DEVICE*/, int64_t n, const int32_t* windows /*HOST*/,
+                           int32_t nwindows, spt_candidate* d_peaks /*DEVICE*/, uint64_t* d_count /*DEVICE*/, void* cuda_stream);
+
+/* -------------------------------------------------------------------------------------------------------
  * spt_search_host -- the whole path from HOST memory: H2D copy of h_fb (uint8 [nbeam][nchan][nsamp]; pinned
  * memory makes the copy asynchronous), spt_dedisperse + spt_single_pulse_search into a library-owned DM
  * transform, then the candidate count back to the host.  Synchronous.  Candidates are then read with

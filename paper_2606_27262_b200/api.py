@@ -41,6 +41,8 @@ class spt_sift_params(ctypes.Structure):
                 ("coinc_beam_fraction", ctypes.c_double)]
 
 
+PEAKS_STATIC_MAX = 262144       # SPT_PEAKS_STATIC_MAX of include/spt.h: records spt_peak_filter_static takes at most
+
 CAND_DTYPE = np.dtype([("beam", "<i4"), ("trial", "<i4"), ("t", "<i4"), ("width", "<i4"), ("snr", "<f4")])
 
 # every symbol include/spt.h declares: name -> (restype, argtypes)
@@ -69,6 +71,7 @@ SYMBOLS = {
     "spt_candidates_read": (ctypes.c_int, [_vp, _vp, _i64, _P(_i64)]),
     "spt_search_host": (ctypes.c_int, [_vp, _vp, _i32, _f32, _vp, _P(_i64), _P(_i32)]),
     "spt_peak_filter": (ctypes.c_int, [_vp, _P(_i32), _i32, _vp]),
+    "spt_peak_filter_static": (ctypes.c_int, [_vp, _vp, _i64, _P(_i32), _i32, _vp, _vp, _vp]),
     "spt_peaks_count": (ctypes.c_int, [_vp, _P(_i64)]),
     "spt_peaks_read": (ctypes.c_int, [_vp, _vp, _i64, _P(_i64)]),
     "spt_corner_turn": (ctypes.c_int, [_vp, _i32, _i64, _i32, _i32, _i32, _vp, _vp]),
@@ -298,6 +301,20 @@ class Plan:
         k = ctypes.c_int64()
         _check(lib().spt_peaks_read(self._h, out.ctypes.data, int(n.value), ctypes.byref(k)), "spt_peaks_read")
         return out[: int(k.value)]
+
+    def peak_filter_static(self, d_cand, n: int, windows: Sequence[int], d_peaks, d_count, stream=None) -> None:
+        """spt_peak_filter_static: the peak filter for callers that may not allocate device memory (a real-time loop that
+        cannot take the device-wide stall of a cudaMalloc; a process whose memory another allocator owns).  Working
+        memory is a fixed block inside libspt.so, so n <= PEAKS_STATIC_MAX.  d_cand: CUDA tensor holding n candidate
+        records (20 bytes each) of a search made with this plan; d_peaks: CUDA tensor with room for n records; d_count:
+        CUDA int64 tensor of one element.  Only enqueues: synchronise the stream before reading d_count / d_peaks.  Calls
+        share the block: do not let two of them overlap on the GPU."""
+        w = (ctypes.c_int32 * len(windows))(*[int(x) for x in windows])
+        rc = lib().spt_peak_filter_static(self._h, _dev_ptr(d_cand), int(n), w, len(windows), _dev_ptr(d_peaks),
+                                          _dev_ptr(d_count), _stream_ptr(stream))
+        if rc == SPT_ERR_UNSUPPORTED:
+            raise SptError(rc, "spt_peak_filter_static: " + lib().spt_last_error().decode())
+        _check(rc, "spt_peak_filter_static")
 
     def segment_info(self):
         """(min_history, min_history_search, granule) in raw samples for spt_segment_push / spt_segment_search."""

@@ -14,7 +14,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libspt.so")
-SOURCES = ["api.cu", "plan.cpp", "dedisperse.cu", "sps.cu", "peaks.cu", "stream.cu", "sift.cu", "cutout.cu", "probe.cu"]
+SOURCES = ["api.cu", "plan.cpp", "dedisperse.cu", "sps.cu", "peaks.cu", "peaks_static.cu", "stream.cu", "sift.cu", "cutout.cu", "probe.cu"]
 HEADERS = ["internal.h", "kernels.h", os.path.join("..", "..", "include", "spt.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=false",

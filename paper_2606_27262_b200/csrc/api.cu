@@ -1147,6 +1147,30 @@ int spt_peak_filter(spt_plan* plan, const int32_t* windows, int32_t nwindows, vo
     return SPT_OK;
 }
 
+int spt_peak_filter_static(spt_plan* plan, const spt_candidate* d_cand, int64_t n, const int32_t* windows, int32_t nwindows,
+                           spt_candidate* d_peaks, uint64_t* d_count, void* cuda_stream) {
+    if (!plan || !windows || nwindows < 1 || nwindows > 8 || n < 0 || !d_count || (n > 0 && (!d_cand || !d_peaks)))
+        return SPT_ERR_INVALID;
+    for (int32_t i = 0; i < nwindows; ++i)
+        if (windows[i] < 1 || (windows[i] & 1) == 0 || windows[i] > 255) return SPT_ERR_INVALID;
+    if (n > SPT_PEAKS_STATIC_MAX) {
+        g_last_error = "spt_peak_filter_static: " + std::to_string((long long)n) + " records exceed the fixed working memory (" +
+                       std::to_string((long long)SPT_PEAKS_STATIC_MAX) + " records at most); use spt_peak_filter";
+        return SPT_ERR_UNSUPPORTED;
+    }
+    Plan& p = plan->p;
+    if (!p.dev) return SPT_ERR_STATE;       // the plan's device tables come from its first dedispersion / search, not from here
+    DeviceState* d = p.dev;
+    PeakArgs a{};
+    a.cand = d_cand; a.n = n; a.beam_stride = p.dmt_elems;
+    a.nout = d->nout; a.offset = d->offset; a.range_lo = d->range_lo; a.range_hi = d->range_hi;
+    int64_t nlaunch = 0;
+    SPT_CUDA(peaks_static_filter(a, windows, nwindows, d_peaks, (unsigned long long*)d_count, (long long)n, (cudaStream_t)cuda_stream,
+                                 &nlaunch));
+    p.launches += nlaunch;
+    return SPT_OK;
+}
+
 int spt_peaks_count(spt_plan* plan, int64_t* total) {
     if (!plan || !total) return SPT_ERR_INVALID;
     Plan& p = plan->p;

@@ -88,6 +88,10 @@ void launch_peaks_erase(const PeakArgs& a, const uint8_t* alive_before, const ui
 void launch_peaks_compact(const PeakArgs& a, const uint8_t* alive, spt_candidate* out, unsigned long long* out_count,
                           long long out_capacity, cudaStream_t st);
 
+// peaks_static.cu: the hash-table filter with its working memory in a fixed block inside the library image (no allocation)
+cudaError_t peaks_static_filter(PeakArgs a, const int32_t* windows, int32_t nwindows, spt_candidate* d_peaks,
+                                unsigned long long* d_count, long long capacity, cudaStream_t st, int64_t* nlaunch);
+
 void launch_corner_turn(const uint8_t* in, int32_t nbeam, int64_t nsamp, int32_t nchan, int32_t flip, int32_t spliced,
                         uint8_t* out, int64_t out_row_stride, int64_t out_beam_stride, int64_t out_t0, cudaStream_t st);
 void launch_keep_history(const uint8_t* src, uint8_t* dst, int64_t row_bytes, int64_t shift_bytes, int64_t keep_bytes,
