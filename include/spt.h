@@ -136,6 +136,11 @@ int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int6
  * cap is chosen by, for reports.  Any out pointer may be NULL. */
 int spt_plan_tiling_cost(spt_plan* plan, int32_t range, int64_t* ntasks, int64_t* task_entries, int64_t* task_variants,
                          int64_t* presum_rounds);
+/* The kernel instance the plan chose for a range (by its cost model, or as the options fixed it): packed words per trial
+ * per time tile (224 or 256), entry cap of a pre-summed group (8, 12 or 16), largest group in channels, and whether the
+ * range has a second table set for the 8-bit copy of its decimated series.  For reports.  Any out pointer may be NULL. */
+int spt_plan_tiling_choice(spt_plan* plan, int32_t range, int32_t* tile_words, int32_t* max_entries, int32_t* group,
+                           int32_t* has_compact);
 /* The delay row of one trial as the tiled kernel will apply it, reconstructed from those tables alone:
  * host_out[nchan] (HOST).  Must equal spt_plan_delays for every trial (checked by the CPU tests). */
 int spt_plan_tiling_delays(spt_plan* plan, int32_t trial, int32_t* host_out);
@@ -164,6 +169,12 @@ int spt_decimated(const spt_plan* plan, int32_t range, const uint16_t** d_ptr, i
 int spt_decimated_stride(const spt_plan* plan, int32_t range, int64_t* row_stride);
 /* Copy of one beam of that series without the row padding: host_out (HOST) uint16 [nchan][nsamp_k].  Synchronises. */
 int spt_decimated_read(spt_plan* plan, int32_t range, int32_t beam, uint16_t* host_out);
+/* Which form of that series the last spt_dedisperse read (read-only; for tests and reports).  A decimated series whose
+ * samples span fewer than 256 values -- quantised noise does -- is dedispersed from an 8-bit copy (sample minus the smallest
+ * sample of the series), decided on the device per call.  in_use = 1: the copy was made and read; floor_value = the smallest
+ * sample, span = largest minus smallest.  in_use = 0: the uint16 series was read (or the range has no copy: decim == 1,
+ * option "compact" = 0).  The results are the same either way.  Synchronises. */
+int spt_decimated_compact(spt_plan* plan, int32_t range, int32_t* in_use, uint32_t* floor_value, uint32_t* span);
 
 /* -------------------------------------------------------------------------------------------------------
  * spt_single_pulse_search -- a4 (readings C1-C5, D1 of DESIGN.md): per (beam, trial) with N = nout > 0

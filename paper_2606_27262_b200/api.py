@@ -58,11 +58,13 @@ SYMBOLS = {
     "spt_plan_set_option": (ctypes.c_int, [_vp, ctypes.c_char_p, _i64]),
     "spt_plan_tiling_info": (ctypes.c_int, [_vp, _i32, _P(_i64), _P(_i64), _P(_i64), _P(_i64), _P(_i64), _P(_i64)]),
     "spt_plan_tiling_cost": (ctypes.c_int, [_vp, _i32, _P(_i64), _P(_i64), _P(_i64), _P(_i64)]),
+    "spt_plan_tiling_choice": (ctypes.c_int, [_vp, _i32, _P(_i32), _P(_i32), _P(_i32), _P(_i32)]),
     "spt_plan_tiling_delays": (ctypes.c_int, [_vp, _i32, _vp]),
     "spt_dedisperse": (ctypes.c_int, [_vp, _vp, _i32, _vp, _vp]),
     "spt_decimated": (ctypes.c_int, [_vp, _i32, _P(_vp), _P(_i64)]),
     "spt_decimated_stride": (ctypes.c_int, [_vp, _i32, _P(_i64)]),
     "spt_decimated_read": (ctypes.c_int, [_vp, _i32, _i32, _vp]),
+    "spt_decimated_compact": (ctypes.c_int, [_vp, _i32, _P(_i32), _P(ctypes.c_uint32), _P(ctypes.c_uint32)]),
     "spt_single_pulse_search": (ctypes.c_int, [_vp, _vp, _i32, _f32, _vp]),
     "spt_search": (ctypes.c_int, [_vp, _vp, _i32, _vp, _f32, _vp]),
     "spt_trial_stats": (ctypes.c_int, [_vp, _i32, _i32, _P(_i64), _P(_i64), _P(ctypes.c_uint64)]),
@@ -207,6 +209,11 @@ class Plan:
         _check(lib().spt_plan_tiling_cost(self._h, rng, *[ctypes.byref(x) for x in v]), "spt_plan_tiling_cost")
         return {k: int(x.value) for k, x in zip(("ntasks", "task_entries", "task_variants", "presum_rounds"), v)}
 
+    def tiling_choice(self, rng: int) -> dict:
+        v = [ctypes.c_int32() for _ in range(4)]
+        _check(lib().spt_plan_tiling_choice(self._h, rng, *[ctypes.byref(x) for x in v]), "spt_plan_tiling_choice")
+        return {k: int(x.value) for k, x in zip(("tile_words", "max_entries", "group", "has_compact"), v)}
+
     def tiling_delays(self, d: int) -> np.ndarray:
         out = np.empty(self.nchan, dtype=np.int32)
         _check(lib().spt_plan_tiling_delays(self._h, d, out.ctypes.data), "spt_plan_tiling_delays")
@@ -235,6 +242,12 @@ class Plan:
         out = np.empty((self.nchan, int(n.value)), dtype=np.uint16)
         _check(lib().spt_decimated_read(self._h, rng, beam, out.ctypes.data), "spt_decimated_read")
         return out
+
+    def decimated_compact(self, rng: int) -> Tuple[bool, int, int]:
+        """(in_use, floor, span): whether the last dedispersion read range `rng`'s series through its 8-bit copy."""
+        u, f, sp = ctypes.c_int32(), ctypes.c_uint32(), ctypes.c_uint32()
+        _check(lib().spt_decimated_compact(self._h, rng, ctypes.byref(u), ctypes.byref(f), ctypes.byref(sp)), "spt_decimated_compact")
+        return bool(u.value), int(f.value), int(sp.value)
 
     def single_pulse_search(self, d_dmt, threshold: float, stream=None):
         nbeam = d_dmt.shape[0] if d_dmt.dim() == 2 else 1

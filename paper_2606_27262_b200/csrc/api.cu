@@ -4,6 +4,7 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -193,6 +194,72 @@ static int alloc_search_bufs(Plan* p, DeviceState::SearchBufs& b) {
     return ce == cudaSuccess ? SPT_OK : cuda_fail(ce, "search buffers");
 }
 
+// Every shared-memory address the kernel will form from one set of tables stays inside the region it belongs to: the variants
+// inside the variant region, the gather's reads inside the variant they read, the pre-sum's raw loads (the last lane's, in
+// the high half, including the words its aligned loads reach past the sample) inside the row that was staged for them.
+// compute-sanitizer is not available on the GPU pool (DESIGN.md section 6); this is the bounds check it would have made, done
+// on the host for every stage of every tile.  es: bytes per element of the series the tables address.
+static int check_tables(const Plan& p, const RangePlan& rp, int es) {
+    const int DT = p.opt_dm_tile, kh = rp.kh;
+    const int64_t rcap = kSmemDataBytes - (int64_t)rp.vcap_words * 4;
+    if (rp.vcap_words <= 0 || rcap <= 0 || (kh != 224 && kh != 256)) return SPT_ERR_STATE;
+    for (const TileDesc& td : rp.tiles)
+        if (td.nstage < 1 || td.stage0 < 0 || (size_t)(td.stage0 + td.nstage) + 1 > rp.sidx.size() || td.ntrial < 1 || td.ntrial > DT)
+            return SPT_ERR_STATE;
+    for (size_t is = 0; is + 1 < rp.sidx.size(); ++is) {
+        const StageIndex& si = rp.sidx[is];
+        if (si.blob_words * 4u > (uint32_t)kBlobBytes || si.nrows > (uint32_t)kMaxStageRows || si.nrows < 1) return SPT_ERR_STATE;
+        if ((size_t)si.blob_word0 + si.blob_words > rp.blob.size() || (size_t)si.row0 + si.nrows > rp.rows.size()) return SPT_ERR_STATE;
+        const uint32_t* b = &rp.blob[si.blob_word0];
+        const uint32_t ngrp = b[0];
+        if (ngrp < 1 || ngrp > (uint32_t)kMaxStageGroups || b[3] + ngrp * (uint32_t)DT / 2 > si.blob_words) return SPT_ERR_STATE;
+        int64_t raw_end = 0;
+        for (uint32_t k = 0; k < si.nrows; ++k) {
+            const RowDesc& r = rp.rows[si.row0 + k];
+            if (r.nelem <= 0 || (r.nelem & 15) || (r.soff & 15) || (r.astart & 15) || r.chan < 0 || r.chan >= p.nchan) return SPT_ERR_STATE;
+            raw_end = std::max<int64_t>(raw_end, (int64_t)r.soff + (int64_t)r.nelem * es);
+        }
+        if (raw_end > rcap) return SPT_ERR_STATE;
+        const uint16_t* toff = reinterpret_cast<const uint16_t*>(b + b[3]);
+        for (uint32_t g = 0; g < ngrp; ++g) {
+            const uint32_t* gh = b + kBlobHdrWords + 4 * g;
+            const int64_t vbase = gh[0] & 0xffffu, vlen = gh[1];
+            const int nent = (int)(gh[2] & 0xffu), ntog = (int)((gh[2] >> 8) & 0xffu), ncorr = (int)((gh[2] >> 16) & 0xffu);
+            const int nvar = (int)(gh[2] >> 24);
+            if (vlen < kh || (vlen & 3) || nvar < 1 || nvar > kMaxVar || nent < 1 || nent > kMaxEnt || ntog > nent) return SPT_ERR_STATE;
+            if (vbase + (int64_t)nvar * vlen > rp.vcap_words) return SPT_ERR_STATE;
+            const uint32_t* cd = b + (gh[3] & 0xffffu);
+            const uint32_t* vd = b + (gh[3] >> 16);
+            const int cls = ent_class(nent);
+            // the variants the pre-sum stores: whole variants of this group
+            for (int k = 0; k <= ntog; ++k)
+                if (vd[k] != 0xffffffffu && (vd[k] < vbase || (vd[k] - vbase) % vlen != 0 || (vd[k] - vbase) / vlen >= (uint32_t)nvar))
+                    return SPT_ERR_STATE;
+            for (int c = 0; c < ncorr; ++c) {
+                const uint32_t dst = vd[chain_words(cls) + 2 * c];
+                if (dst < vbase || (dst - vbase) % vlen != 0 || (dst - vbase) / vlen >= (uint32_t)nvar) return SPT_ERR_STATE;
+            }
+            // the gather: trial i reads kh words from its offset, inside one variant
+            for (int i = 0; i < DT; ++i) {
+                const int64_t rel = (int64_t)toff[g * DT + i] - vbase;
+                if (rel < 0 || rel / vlen >= nvar || rel % vlen + kh > vlen) return SPT_ERR_STATE;
+            }
+            // the pre-sum's raw loads: the lane with the last four words (u0 = vlen - 4), low and high half
+            for (int q = 0; q < cls; ++q) {
+                const int64_t w0 = cd[2 * q] & 0x3ffffu;               // aligned word (uint8) / 8-byte unit (uint16) of sample u = 0
+                const int64_t last = es == 1 ? w0 + (vlen - 4) + kh + 8 : w0 + 2 * (vlen - 4) + 2 * kh + 16;
+                bool inside = false;
+                for (uint32_t k = 0; k < si.nrows && !inside; ++k) {
+                    const RowDesc& r = rp.rows[si.row0 + k];
+                    inside = w0 >= r.soff && last <= (int64_t)r.soff + (int64_t)r.nelem * es;
+                }
+                if (!inside) return SPT_ERR_STATE;
+            }
+        }
+    }
+    return SPT_OK;
+}
+
 static int ensure_device(Plan* p) {
     if (p->dev) return SPT_OK;
     int ndev = 0;
@@ -202,6 +269,18 @@ static int ensure_device(Plan* p) {
     if (p->opt_kernel == 0 && !p->tiling_built) {
         const int rc = build_tiling(*p);
         if (rc != SPT_OK) return rc;
+    }
+    if (p->opt_kernel == 0) {
+        // the tables go to the kernel only after the host-side bounds check of every shared-memory address they lead to
+        // (there is no compute-sanitizer on the GPU pool to catch a table that is wrong for an untested plan shape)
+        const char* skip = std::getenv("SPT_CHECK_TABLES");
+        if (!(skip && skip[0] == '0'))
+            for (size_t i = 0; i < p->ranges.size(); ++i) {
+                if (p->ranges[i].tiles.empty()) continue;
+                int rc = check_tables(*p, p->ranges[i], p->ranges[i].decim == 1 ? 1 : 2);
+                if (rc == SPT_OK && i < p->compact.size() && !p->compact[i].tiles.empty()) rc = check_tables(*p, p->compact[i], 1);
+                if (rc != SPT_OK) { g_last_error = "kernel tables of range " + std::to_string(i) + " fail the bounds check"; return rc; }
+            }
     }
     DeviceState* d = new (std::nothrow) DeviceState();
     if (!d) return SPT_ERR_NOMEM;
@@ -256,6 +335,12 @@ static int ensure_device(Plan* p) {
         cudaError_t ce = cudaStreamCreateWithFlags(&d->own_stream, cudaStreamNonBlocking);
         if (ce != cudaSuccess) rc = cuda_fail(ce, "plan stream");
     }
+    if (rc == SPT_OK) {
+        // the zero fills above ran on the legacy default stream, which non-blocking streams (every torch.cuda.Stream) do not
+        // wait for: they must have landed before the first launch on such a stream
+        cudaError_t ce = cudaStreamSynchronize(cudaStreamLegacy);
+        if (ce != cudaSuccess) rc = cuda_fail(ce, "plan set-up");
+    }
     if (rc != SPT_OK) free_device(p);
     return rc;
 }
@@ -275,11 +360,15 @@ static int do_dedisperse(Plan* p, const uint8_t* d_fb, int32_t nbeam, int32_t* d
         if (!d->fb_pad) {
             const size_t bytes = (size_t)p->max_beams * p->nchan * pitch;
             SPT_CUDA(cudaMalloc((void**)&d->fb_pad, bytes));
-            SPT_CUDA(cudaMemset(d->fb_pad, 0, bytes));
+            SPT_CUDA(cudaMemsetAsync(d->fb_pad, 0, bytes, st));      // on st: ordered before the copy below on any stream
             d->fb_pad_stride = pitch;
         }
         SPT_CUDA(cudaMemcpy2DAsync(d->fb_pad, (size_t)pitch, d_fb, (size_t)p->nsamp, (size_t)p->nsamp,
                                    (size_t)nbeam * p->nchan, cudaMemcpyDeviceToDevice, st));
+        // the row padding repeats the row's last sample: the bounds pass below scans whole rows, and padding zeros would
+        // drag the smallest sample (the floor the packed lanes subtract) to 0 for every input like this one
+        launch_fill_row_pad_u8(d->fb_pad, pitch, p->nsamp, (int64_t)nbeam * p->nchan, st);
+        p->launches++;
         in = d->fb_pad;
         in_stride = pitch;
     }
@@ -634,72 +723,6 @@ static int ensure_tiling(Plan& p) {
     }
 }
 
-// Every shared-memory address the kernel will form from one set of tables stays inside the region it belongs to: the variants
-// inside the variant region, the gather's reads inside the variant they read, the pre-sum's raw loads (the last lane's, in
-// the high half, including the words its aligned loads reach past the sample) inside the row that was staged for them.
-// compute-sanitizer is not available on the GPU pool (DESIGN.md section 6); this is the bounds check it would have made, done
-// on the host for every stage of every tile.  es: bytes per element of the series the tables address.
-static int check_tables(const Plan& p, const RangePlan& rp, int es) {
-    const int DT = p.opt_dm_tile, kh = rp.kh;
-    const int64_t rcap = kSmemDataBytes - (int64_t)rp.vcap_words * 4;
-    if (rp.vcap_words <= 0 || rcap <= 0 || (kh != 224 && kh != 256)) return SPT_ERR_STATE;
-    for (const TileDesc& td : rp.tiles)
-        if (td.nstage < 1 || td.stage0 < 0 || (size_t)(td.stage0 + td.nstage) + 1 > rp.sidx.size() || td.ntrial < 1 || td.ntrial > DT)
-            return SPT_ERR_STATE;
-    for (size_t is = 0; is + 1 < rp.sidx.size(); ++is) {
-        const StageIndex& si = rp.sidx[is];
-        if (si.blob_words * 4u > (uint32_t)kBlobBytes || si.nrows > (uint32_t)kMaxStageRows || si.nrows < 1) return SPT_ERR_STATE;
-        if ((size_t)si.blob_word0 + si.blob_words > rp.blob.size() || (size_t)si.row0 + si.nrows > rp.rows.size()) return SPT_ERR_STATE;
-        const uint32_t* b = &rp.blob[si.blob_word0];
-        const uint32_t ngrp = b[0];
-        if (ngrp < 1 || ngrp > (uint32_t)kMaxStageGroups || b[3] + ngrp * (uint32_t)DT / 2 > si.blob_words) return SPT_ERR_STATE;
-        int64_t raw_end = 0;
-        for (uint32_t k = 0; k < si.nrows; ++k) {
-            const RowDesc& r = rp.rows[si.row0 + k];
-            if (r.nelem <= 0 || (r.nelem & 15) || (r.soff & 15) || (r.astart & 15) || r.chan < 0 || r.chan >= p.nchan) return SPT_ERR_STATE;
-            raw_end = std::max<int64_t>(raw_end, (int64_t)r.soff + (int64_t)r.nelem * es);
-        }
-        if (raw_end > rcap) return SPT_ERR_STATE;
-        const uint16_t* toff = reinterpret_cast<const uint16_t*>(b + b[3]);
-        for (uint32_t g = 0; g < ngrp; ++g) {
-            const uint32_t* gh = b + kBlobHdrWords + 4 * g;
-            const int64_t vbase = gh[0] & 0xffffu, vlen = gh[1];
-            const int nent = (int)(gh[2] & 0xffu), ntog = (int)((gh[2] >> 8) & 0xffu), ncorr = (int)((gh[2] >> 16) & 0xffu);
-            const int nvar = (int)(gh[2] >> 24);
-            if (vlen < kh || (vlen & 3) || nvar < 1 || nvar > kMaxVar || nent < 1 || nent > kMaxEnt || ntog > nent) return SPT_ERR_STATE;
-            if (vbase + (int64_t)nvar * vlen > rp.vcap_words) return SPT_ERR_STATE;
-            const uint32_t* cd = b + (gh[3] & 0xffffu);
-            const uint32_t* vd = b + (gh[3] >> 16);
-            const int cls = ent_class(nent);
-            // the variants the pre-sum stores: whole variants of this group
-            for (int k = 0; k <= ntog; ++k)
-                if (vd[k] != 0xffffffffu && (vd[k] < vbase || (vd[k] - vbase) % vlen != 0 || (vd[k] - vbase) / vlen >= (uint32_t)nvar))
-                    return SPT_ERR_STATE;
-            for (int c = 0; c < ncorr; ++c) {
-                const uint32_t dst = vd[chain_words(cls) + 2 * c];
-                if (dst < vbase || (dst - vbase) % vlen != 0 || (dst - vbase) / vlen >= (uint32_t)nvar) return SPT_ERR_STATE;
-            }
-            // the gather: trial i reads kh words from its offset, inside one variant
-            for (int i = 0; i < DT; ++i) {
-                const int64_t rel = (int64_t)toff[g * DT + i] - vbase;
-                if (rel < 0 || rel / vlen >= nvar || rel % vlen + kh > vlen) return SPT_ERR_STATE;
-            }
-            // the pre-sum's raw loads: the lane with the last four words (u0 = vlen - 4), low and high half
-            for (int q = 0; q < cls; ++q) {
-                const int64_t w0 = cd[2 * q] & 0x3ffffu;               // aligned word (uint8) / 8-byte unit (uint16) of sample u = 0
-                const int64_t last = es == 1 ? w0 + (vlen - 4) + kh + 8 : w0 + 2 * (vlen - 4) + 2 * kh + 16;
-                bool inside = false;
-                for (uint32_t k = 0; k < si.nrows && !inside; ++k) {
-                    const RowDesc& r = rp.rows[si.row0 + k];
-                    inside = w0 >= r.soff && last <= (int64_t)r.soff + (int64_t)r.nelem * es;
-                }
-                if (!inside) return SPT_ERR_STATE;
-            }
-        }
-    }
-    return SPT_OK;
-}
-
 int spt_plan_tiling_info(spt_plan* plan, int32_t range, int64_t* ntiles_dm, int64_t* nstages, int64_t* ngroups,
                          int64_t* nvariants, int64_t* ntiles_t, int64_t* max_stage_words) {
     if (!plan) return SPT_ERR_INVALID;
@@ -749,6 +772,21 @@ int spt_plan_tiling_cost(spt_plan* plan, int32_t range, int64_t* ntasks, int64_t
     if (task_entries) *task_entries = rp.task_entries;
     if (task_variants) *task_variants = rp.task_variants;
     if (presum_rounds) *presum_rounds = rp.presum_rounds;
+    return SPT_OK;
+}
+
+int spt_plan_tiling_choice(spt_plan* plan, int32_t range, int32_t* tile_words, int32_t* max_entries, int32_t* group,
+                           int32_t* has_compact) {
+    if (!plan) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (range < 0 || range >= (int32_t)p.ranges.size()) return SPT_ERR_SHAPE;
+    const int rc = ensure_tiling(p);
+    if (rc != SPT_OK) return rc;
+    const RangePlan& rp = p.ranges[range];
+    if (tile_words) *tile_words = rp.kh;
+    if (max_entries) *max_entries = rp.max_ent;
+    if (group) *group = p.opt_group ? p.opt_group : (rp.max_ent > 8 ? 16 : 8);
+    if (has_compact) *has_compact = ((size_t)range < p.compact.size() && !p.compact[range].tiles.empty()) ? 1 : 0;
     return SPT_OK;
 }
 
@@ -878,6 +916,25 @@ int spt_decimated_read(spt_plan* plan, int32_t range, int32_t beam, uint16_t* ho
     const uint16_t* src = p.dev->r[range].series + (size_t)beam * p.nchan * rp.stride_k;
     SPT_CUDA(cudaMemcpy2D(host_out, (size_t)rp.nsamp_k * 2, src, (size_t)rp.stride_k * 2, (size_t)rp.nsamp_k * 2,
                           (size_t)p.nchan, cudaMemcpyDeviceToHost));
+    return SPT_OK;
+}
+
+int spt_decimated_compact(spt_plan* plan, int32_t range, int32_t* in_use, uint32_t* floor_value, uint32_t* span) {
+    if (!plan || !in_use) return SPT_ERR_INVALID;
+    Plan& p = plan->p;
+    if (range < 0 || range >= (int32_t)p.ranges.size()) return SPT_ERR_SHAPE;
+    *in_use = 0;
+    if (floor_value) *floor_value = 0;
+    if (span) *span = 0;
+    if (!p.dev || p.dev->nbeam_dedisp == 0) return SPT_ERR_STATE;
+    const RangeDev& rd = p.dev->r[range];
+    if (!rd.series8 || p.ranges[range].nsamp_k <= 0) return SPT_OK;     // no copy for this range (decim == 1, option off, tables)
+    SPT_CUDA(cudaStreamSynchronize(p.dev->dedisp_stream));
+    uint32_t info[4] = {0, 0, 0, 0};
+    SPT_CUDA(cudaMemcpy(info, rd.cinfo, sizeof(info), cudaMemcpyDeviceToHost));
+    *in_use = info[2] == 1u ? 1 : 0;
+    if (floor_value) *floor_value = info[3];
+    if (span) *span = info[0];
     return SPT_OK;
 }
 
@@ -1278,7 +1335,10 @@ int spt_segment_push(spt_plan* plan, const uint8_t* d_new, int32_t nbeam, int64_
     if (!d->work[0]) {
         for (int i = 0; i < 2; ++i) {
             SPT_CUDA(cudaMalloc((void**)&d->work[i], bytes));
-            SPT_CUDA(cudaMemset(d->work[i], 0, bytes));           // the stream starts on a history of zeros
+            // the stream starts on a history of zeros; on the caller's stream, so that the history copy and the corner turn
+            // below are ordered behind it whatever kind of stream that is (a plain cudaMemset runs on the legacy default
+            // stream, which a non-blocking stream does not wait for)
+            SPT_CUDA(cudaMemsetAsync(d->work[i], 0, bytes, st));
         }
         d->work_cur = 0;
     }

@@ -52,6 +52,23 @@ __global__ void decimate_kernel(const uint8_t* __restrict__ x, int64_t in_row_st
             dst[j] = (uint16_t)s;
         }
     }
+    // The row padding (rows are 16-element multiples) repeats the row's last sample.  No stored output reads it, but the
+    // passes over whole rows do -- the bounds of the series and its 8-bit copy -- and padding zeros would make every series
+    // whose length is not a multiple of 16 look as if it spanned [0, max]: no 8-bit copy, no floor for the packed lanes.
+    if (q == quads - 1) {
+        const int64_t pad_end = min((nsamp_k + 15) & ~(int64_t)15, out_row_stride);
+        const uint16_t last = dst[nsamp_k - 1];                    // written by this thread just above
+        for (int64_t j = nsamp_k; j < pad_end; ++j) dst[j] = last;
+    }
+}
+
+// The same for a padded copy of a uint8 filterbank whose rows are not 16-byte multiples (one thread per row).
+__global__ void fill_row_pad_u8_kernel(uint8_t* __restrict__ x, int64_t pitch, int64_t nsamp, int64_t nrows) {
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= nrows) return;
+    uint8_t* row = x + r * pitch;
+    const uint8_t last = row[nsamp - 1];
+    for (int64_t j = nsamp; j < pitch; ++j) row[j] = last;
 }
 
 // Largest and smallest sample of a uint8 filterbank -> maxval[0], maxval[1] (bounds for the ranges that read the raw input).
@@ -72,7 +89,7 @@ __global__ void max_u8_kernel(const uint4* __restrict__ x, int64_t n16, uint32_t
     }
 }
 
-// The same for a decimated (uint16) series; its zero row padding, where there is any, only makes the bound looser.
+// The same for a decimated (uint16) series (its row padding repeats real samples: decimate_kernel).
 __global__ void max_u16_kernel(const uint4* __restrict__ x, int64_t n16, uint32_t* __restrict__ maxval) {
     uint32_t m = 0, lo = 0xffffffffu;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (int64_t)gridDim.x * blockDim.x) {
@@ -109,6 +126,11 @@ void launch_max_u16(const uint16_t* x, int64_t nelem, uint32_t* maxval, cudaStre
     max_u16_kernel<<<sm_count() * 8, 256, 0, st>>>(reinterpret_cast<const uint4*>(x), n16, maxval);
 }
 
+void launch_fill_row_pad_u8(uint8_t* x, int64_t pitch, int64_t nsamp, int64_t nrows, cudaStream_t st) {
+    if (nrows <= 0 || nsamp <= 0 || pitch <= nsamp) return;
+    fill_row_pad_u8_kernel<<<(unsigned)((nrows + 255) / 256), 256, 0, st>>>(x, pitch, nsamp, nrows);
+}
+
 void launch_max_u8(const uint8_t* x, int64_t nbytes, uint32_t* maxval, cudaStream_t st) {
     const int64_t n16 = nbytes / 16;          // rows are 16-byte multiples
     if (n16 <= 0) return;
@@ -118,8 +140,8 @@ void launch_max_u8(const uint8_t* x, int64_t nbytes, uint32_t* maxval, cudaStrea
 // 8-bit copy of a decimated series: c = y - (smallest sample of the series), made only when the series spans less than 256
 // (quantised noise does: its decimated sums sit within a few sigma of k times the mean).  info[0..3] = {largest value of
 // the copy, 0 (its floor), flag: 1 = the copy is valid, bias = the smallest sample (added back per channel when the lanes
-// are widened)}.  The dedispersion of the range is enqueued twice, on the copy and on the uint16 series; each launch looks
-// at the flag and one of them returns at once.
+// are widened)}.  The dedispersion of the range is one dual launch (dedisp_dual_kernel): every block looks at the flag and
+// takes the copy with the copy's tables, or the uint16 series with its own.
 __global__ void compact_u16_kernel(const uint4* __restrict__ y, uint2* __restrict__ c, int64_t n8, const uint32_t* __restrict__ maxval,
                                    uint32_t* __restrict__ info) {
     const uint32_t vmax = __ldg(maxval), vmin = __ldg(maxval + 1);

@@ -464,16 +464,24 @@ int build_tiling(Plan& p) {
             // second set of tables for the 8-bit copy of the decimated series (the delay table is shared by value: a few MB)
             // Both sets run in one kernel instance, so they share tile width and entry cap: the copy's choice (it is the set
             // that runs on well-behaved data), and the same DM tiles and skews, so that a block does the same tile either way.
+            // The uint16 rows are twice as large, so the copy's choice may not build for them (build_range_auto may have
+            // rejected exactly that combination): the range then keeps the tables chosen for the uint16 series alone and
+            // has no 8-bit copy -- a working plan, one launch on the uint16 series -- instead of failing the whole plan.
+            RangePlan own = p.ranges[i];
             p.compact[i] = p.ranges[i];
-            if ((rc = build_range_auto(p, p.compact[i], true)) != SPT_OK) return rc;
-            if (p.compact[i].max_ent != p.ranges[i].max_ent || p.compact[i].kh != p.ranges[i].kh) {
+            bool ok = build_range_auto(p, p.compact[i], true) == SPT_OK;
+            if (ok && (p.compact[i].max_ent != p.ranges[i].max_ent || p.compact[i].kh != p.ranges[i].kh)) {
                 const int G = p.opt_group ? p.opt_group : (p.compact[i].max_ent > 8 ? 16 : 8);
                 p.ranges[i].kh = p.compact[i].kh;
-                if ((rc = build_range(p, p.ranges[i], G, p.compact[i].max_ent, false)) != SPT_OK) return rc;
+                ok = build_range(p, p.ranges[i], G, p.compact[i].max_ent, false) == SPT_OK;
             }
-            if (p.compact[i].ntile_t != p.ranges[i].ntile_t || p.compact[i].tiles.size() != p.ranges[i].tiles.size() ||
-                p.compact[i].skew != p.ranges[i].skew)
-                return SPT_ERR_STATE;
+            if (ok && (p.compact[i].ntile_t != p.ranges[i].ntile_t || p.compact[i].tiles.size() != p.ranges[i].tiles.size() ||
+                       p.compact[i].skew != p.ranges[i].skew))
+                ok = false;
+            if (!ok) {
+                p.ranges[i] = std::move(own);
+                p.compact[i] = RangePlan();
+            }
         }
     }
     p.tiling_built = true;

@@ -10,7 +10,8 @@
 //   small exact int32 S' and  snr_w >= threshold  <=>  S' >= tau_w = (threshold*N*sigma*sqrt(w) + w*(Sx - N*m))/N.  Every
 //   (t, w) costs one LDS, one subtract and one add-max against the integer floor of tau_w; only samples that pass
 //   it run the evaluation above, which decides.  The exact path (any plan the ABI accepts) evaluates every (t, w).
-// HBM bound by design (one compulsory read of the DM transform; the second pass of a row re-reads it from L2).
+// Designed around one compulsory HBM read of the DM transform (the second pass of a row re-reads it from L2); as measured the
+// kernel is bound by instruction issue and load latency, not by HBM (0.21 of the copy bandwidth on config 3: DESIGN.md section 5.4).
 #include <cuda_runtime.h>
 
 #include <atomic>
@@ -25,7 +26,7 @@ constexpr int kSpsWarps = kSpsThreads / 32;
 #define SPS_ITERS 7
 #endif
 constexpr int kIters = SPS_ITERS;                   // 128-element warp rows per warp per segment
-constexpr int kWarpSpan = kIters * 128;             // 640 consecutive elements per warp
+constexpr int kWarpSpan = kIters * 128;             // 896 consecutive elements per warp
 constexpr int kSegLoad = kSpsWarps * kWarpSpan;     // 14336 elements staged per segment (outputs + halo of the widest boxcar)
 constexpr int kCOff = 3;                            // s_c[kCOff + 1 + e] = inclusive prefix through element e (16-byte aligned rows)
 constexpr int kEpt = 8;                             // outputs per thread per sub-block of the fast path

@@ -179,3 +179,43 @@ def check_candidates_dense(orc, plan, cands, oracle_ranges, widths, threshold, b
         d0 += ndm
     assert seen == mine.size, "candidate with a trial index outside the plan"
     return stats
+
+
+def check_segment_against_oracle(orc, plan, dmt_beam, orows, trials, widths, threshold, nnew, cands, s_row, q_row, sentinel=None):
+    """One pushed stream segment of one beam (reading F), for the trials named.  orows[d] = the ORACLE's dedispersed row d of
+    the oracle's stream buffer.  Checked: the window the search reads (the last nnew/k + wmax - 1 outputs of the row) equals
+    the oracle's, bit for bit; with `sentinel`, nothing before the window was written; the window's exact statistics; the
+    candidates of the segment's start positions under rules D2 (identical except within SNR_TOL of the threshold)."""
+    _, _, dec, nout, off = plan.trial_table()
+    got = {}
+    for c in cands:
+        got.setdefault(int(c["trial"]), []).append((int(c["t"]), int(c["width"]), float(c["snr"])))
+    nchecked = 0
+    for d in trials:
+        n, k = int(nout[d]), int(dec[d])
+        row = orows[d]
+        assert row.size == n
+        win = min(n, nnew // k + max(widths) - 1)
+        mine = dmt_beam[off[d]: off[d] + n]
+        assert np.array_equal(mine[n - win:], row[n - win:]), ("window of trial", d)
+        if sentinel is not None:
+            assert np.all(mine[: n - win] == sentinel), ("outputs before the window of trial", d)
+        sx, sxx, t, bw, snr = orc.search_segment(row, widths, threshold, nnew // k)
+        assert (int(s_row[d]), int(q_row[d])) == (sx, sxx), ("statistics of trial", d)
+        g = sorted(got.get(d, []))
+        exp = sorted(zip(t.tolist(), bw.tolist(), snr.tolist()))
+        near = [x for x in exp if abs(x[2] - threshold) <= SNR_TOL]
+        assert abs(len(g) - len(exp)) <= len(near), (d, len(g), len(exp))
+        ge = {x[0]: x for x in g}
+        for (tt, ww, ss) in exp:
+            if tt in ge:
+                assert ge[tt][1] == ww and abs(ge[tt][2] - ss) <= SNR_TOL, (d, tt)
+            else:
+                assert abs(ss - threshold) <= SNR_TOL
+        et = {x[0] for x in exp}
+        for (tt, ww, ss) in g:                                    # an event only the CUDA path has sits at the threshold too
+            assert tt in et or abs(ss - threshold) <= 2 * SNR_TOL, (d, tt, ss)
+        lo = n - win
+        assert all(lo <= x[0] < lo + nnew // k for x in g)        # only this segment's start positions
+        nchecked += len(exp)
+    return nchecked

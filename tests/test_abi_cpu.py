@@ -144,6 +144,23 @@ def test_tiling_odd_shapes(api):
         p.tiling_info(r)              # includes the bounds check of every shared-memory address the tables lead to
 
 
+@pytest.mark.parametrize("opts", [{}, {"max_entries": 12}, {"max_entries": 12, "tile_words": 224}, {"max_entries": 16}])
+def test_tiling_large_decimation(api, opts):
+    """Ranges decimated by 32 and 64 (their uint16 rows are the widest a stage holds) with the 12- and 16-entry caps: the
+    plan builds, both table sets -- the uint16 series' and the 8-bit copy's, rebuilt to share one kernel instance -- pass the
+    bounds check, and the factorised tables give back every delay.  (If the shared instance cannot be built for the uint16
+    tables the range falls back to its own tables without an 8-bit copy; the plan still has to work.)"""
+    nchan = 1024
+    p = api.Plan(500.0, -200.0 / nchan, nchan, 1.31072e-3, 1 << 17, [(0.0, 0.2, 64, 1), (100.0, 4.0, 130, 32), (700.0, 8.0, 70, 64)],
+                 [1, 2, 4], options=opts)
+    for d in list(range(0, p.ntrials, 7)) + [p.ntrials - 1]:
+        assert np.array_equal(p.tiling_delays(d), p.delays(d)), d
+    for r in range(3):
+        info = p.tiling_info(r)
+        assert info["max_stage_words"] <= 227 * 1024 // 4
+    p.close()
+
+
 def test_device_calls_fail_loudly_without_gpu(api):
     import torch
     if torch.cuda.is_available():

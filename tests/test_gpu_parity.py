@@ -159,6 +159,30 @@ def test_odd_shapes(cuda, api, orc, fill, options):
             assert np.array_equal(plan.decimated_read(ri), rr.series)
 
 
+def test_rows_that_are_not_16_sample_multiples_keep_the_8bit_copy(cuda, api, orc):
+    """5003 samples: the input rows, and the decimated rows (2501 and 625 samples), all end in padding.  The padding must
+    not count in the bounds of a series: with Gaussian bytes the decimated ranges still take their 8-bit copy (floor > 0).
+    Run on a non-blocking stream: the padded input copy and its one-time zero fill are ordered on the caller's stream."""
+    w = Shape(420.0, -1.0, 71, 5003, [(3.0, 0.7, 77, 1), (60.0, 1.1, 41, 2), (100.0, 2.0, 5, 8)], [1, 3, 7, 20], 4.5)
+    rs = np.random.default_rng(6)
+    fb = rs.normal(128, 10, size=(w.nchan, w.nsamp)).round().clip(0, 255).astype(np.uint8)
+    ref = oracle_path(orc, w, fb)
+    with cuda.cuda.stream(cuda.cuda.Stream()):
+        plan, dmt, cands = run_gpu(cuda, api, w, fb[None])
+        for ri, rr in enumerate(ref):
+            if rr.decim > 1:
+                assert rr.series.shape[1] % 16 != 0
+                in_use, floor, span = plan.decimated_compact(ri)
+                assert in_use and floor == int(rr.series.min()) and span == int(rr.series.max()) - floor, (ri, in_use, floor, span)
+                assert np.array_equal(plan.decimated_read(ri), rr.series)
+            else:
+                assert plan.decimated_compact(ri) == (False, 0, 0)
+    check_dmt_against_oracle(plan, dmt, ref)
+    check_stats_against_oracle(plan, ref)
+    st = check_candidates_against_oracle(orc, plan, cands, ref, w.widths, w.threshold)
+    assert st["oracle"] > 0
+
+
 def test_all255_wide_band_lane_limits(cuda, api, orc):
     """4096 channels of 255 at decimation 4: int32 outputs reach 4096*255*4 and every packed lane flush is needed."""
     w = Shape(500.0, -0.048828125, 4096, 4096, [(0.0, 0.2, 70, 1), (0.0, 1.0, 70, 4)], [1, 2, 1024], 6.0)

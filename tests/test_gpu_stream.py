@@ -4,7 +4,7 @@ last nnew/decim outputs of every trial continue the previous push's."""
 import numpy as np
 import pytest
 
-from helpers import check_dmt_against_oracle, make_plan
+from helpers import check_dmt_against_oracle, check_segment_against_oracle, make_plan
 from test_gpu_parity import Shape, oracle_path
 
 pytestmark = pytest.mark.gpu
@@ -119,9 +119,18 @@ def test_segment_search_matches_the_oracle_window(cuda, api, orc, whole_rows):
     _, _, dec, nout, off = plan.trial_table()
     total = 0
     d_dmt = cuda.zeros((1, plan.dmt_elems_per_beam), dtype=cuda.int32, device="cuda")
+    blocks = []
     for i in range(3):
         blk = rs.normal(128, 12, size=(1, nnew, nchan)).round().clip(0, 255).astype(np.uint8)
         blk[0, 1000 + 300 * i: 1003 + 300 * i, :] += 20            # a zero-DM spike per segment
+        blocks.append(blk)
+    bufs = orc.overlap_save_buffers([blk[0] for blk in blocks], w.nsamp, flip=False)
+    for i, blk in enumerate(blocks):
+        # the rows the oracle's search is given are the ORACLE's dedispersion of the stream buffer, so that the pair
+        # (push, search) is checked end to end; the GPU's own rows must equal them over the window the search reads
+        orows = []
+        for rr in oracle_path(orc, w, bufs[i], search=False):
+            orows += [rr.dmt[rr.rowoff[j]: rr.rowoff[j + 1]] for j in range(len(rr.nout))]
         d_dmt = plan.segment_push(cuda.from_numpy(blk).cuda(), d_dmt=d_dmt, whole_rows=whole_rows)
         plan.segment_search(d_dmt, nnew, w.threshold)
         n, ovf = plan.candidates_count()
@@ -129,24 +138,58 @@ def test_segment_search_matches_the_oracle_window(cuda, api, orc, whole_rows):
         cands = plan.candidates_read()
         s_all, q_all = plan.trial_stats_all(1)
         dmt = d_dmt.cpu().numpy()[0]
-        got = {}
-        for c in cands:
-            got.setdefault(int(c["trial"]), []).append((int(c["t"]), int(c["width"]), float(c["snr"])))
-        for d in range(plan.ntrials):
-            row = dmt[off[d]: off[d] + nout[d]]     # (whole_rows = False: only its tail, the window, is defined)
-            sx, sxx, t, bw, snr = orc.search_segment(row, widths, w.threshold, nnew // int(dec[d]))
-            assert (int(s_all[0, d]), int(q_all[0, d])) == (sx, sxx), d
-            g = sorted(got.get(d, []))
-            exp = sorted(zip(t.tolist(), bw.tolist(), snr.tolist()))
-            near = [x for x in exp if abs(x[2] - w.threshold) <= 1e-3]
-            assert abs(len(g) - len(exp)) <= len(near), (d, len(g), len(exp))
-            ge = {x[0]: x for x in g}
-            for (tt, ww, ss) in exp:
-                if tt in ge:
-                    assert ge[tt][1] == ww and abs(ge[tt][2] - ss) <= 1e-3, (d, tt)
-                else:
-                    assert abs(ss - w.threshold) <= 1e-3
-            lo = nout[d] - (nnew // int(dec[d]) + max(widths) - 1)
-            assert all(lo <= x[0] < lo + nnew // int(dec[d]) for x in g)      # only this segment's start positions
+        check_segment_against_oracle(orc, plan, dmt, orows, range(plan.ntrials), widths, w.threshold, nnew, cands, s_all[0], q_all[0])
         total += n
     assert total > 1000
+
+
+def test_push_on_a_non_blocking_stream_takes_the_8bit_body_with_a_tail(cuda, api, orc):
+    """Two things no other stream test does.  (1) The pushes run on a torch.cuda.Stream(), a non-blocking stream that does
+    not wait for the legacy default stream: the library's one-time zero fill of its working buffers has to be ordered on
+    the caller's stream, or it can land after the first block.  (2) Gaussian bytes, as the telescope's are: once the buffer
+    holds no more start-up zeros the decimated series span fewer than 256 values, so the decimated ranges of a tail-only
+    push (whole_rows = 0) run the dual kernel's 8-BIT body with tail > 0 -- asserted through spt_decimated_compact -- and
+    their outputs are compared with the oracle's dedispersion of the oracle's stream buffer."""
+    nchan, nnew, nbeam = 256, 2048, 2
+    widths = [1, 2, 4, 16]
+    w = Shape(500.0, -200.0 / nchan, nchan, 0, [(0.0, 0.2, 70, 1), (10.0, 0.5, 40, 2), (30.0, 1.0, 33, 4)], widths, 6.0, nbeam=nbeam)
+    probe = api.Plan(w.fch1, w.foff, nchan, w.tsamp, 1 << 16, w.ranges, w.widths)
+    _, hsearch, _ = probe.segment_info()
+    w.nsamp = hsearch + nnew + 1024
+    npush = (w.nsamp + nnew - 1) // nnew + 2                        # the last two pushes see a buffer without start-up zeros
+    rs = np.random.default_rng(12)
+    blocks = [rs.normal(128, 10, size=(nnew, nbeam, nchan)).round().clip(0, 255).astype(np.uint8) for _ in range(npush)]
+    plan = make_plan(api, w, nbeam=nbeam)
+    refs = [orc.overlap_save_buffers([blk[:, b, :] for blk in blocks], w.nsamp, flip=True) for b in range(nbeam)]
+    _, _, dec, nout, off = plan.trial_table()
+    SENT = -123456789
+    s = cuda.cuda.Stream()
+    took_8bit = 0
+    with cuda.cuda.stream(s):
+        for i, blk in enumerate(blocks):
+            d_dmt = cuda.full((nbeam, plan.dmt_elems_per_beam), SENT, dtype=cuda.int32, device="cuda")
+            plan.segment_push(cuda.from_numpy(blk).cuda(), flip=True, d_dmt=d_dmt, stream=s, spliced=True, whole_rows=False)
+            s.synchronize()
+            dmt = d_dmt.cpu().numpy()
+            if i >= npush - 2:
+                for ri in (1, 2):
+                    in_use, floor, span = plan.decimated_compact(ri)
+                    assert in_use and floor > 0 and span < 256, (i, ri, in_use, floor, span)
+                    took_8bit += 1
+            elif i == 0:
+                assert not plan.decimated_compact(1)[0]             # zeros and noise together span more than a byte
+            if 0 < i < npush - 2:
+                continue                                            # the oracle's time goes to the first push and the 8-bit ones
+            for b in range(nbeam):
+                ref = oracle_path(orc, w, refs[b][i], search=False)
+                d = 0
+                for rr in ref:
+                    for j in range(len(rr.nout)):
+                        n, k = int(nout[d]), int(dec[d])
+                        tail = min(n, nnew // k + max(widths) - 1)
+                        got = dmt[b][off[d]: off[d] + n]
+                        exp = rr.dmt[rr.rowoff[j]: rr.rowoff[j + 1]]
+                        assert np.array_equal(got[n - tail:], exp[n - tail:]), (i, b, d)
+                        assert np.all(got[: n - tail] == SENT), (i, b, d)
+                        d += 1
+    assert took_8bit == 4
