@@ -1,11 +1,11 @@
-"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (default options): sampled outputs
-the oracle computes one by one, whole rows / statistics / candidates of sampled trials, and properties that hold at
-any size (DM 0 = plain channel sum; every trial's sum of outputs = sum of the samples it covers is implied by the
-sampled rows)."""
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (default options).  Configs 2, 3 and 5
+(and config 3's plan on uniform bytes): EVERY output of the DM transform, every trial's statistics and the whole candidate
+list against the oracle.  Config 4: complete beams (all outputs, statistics, candidates) plus, for all 64 beams, row-sum
+identities that hold at any size.  Config 6 (Band 5): every output, statistics and the candidate list."""
 import numpy as np
 import pytest
 
-from helpers import SNR_TOL, check_candidates_against_oracle, check_candidates_dense, check_dmt_against_oracle, check_plan_against_oracle, check_stats_against_oracle, make_plan
+from helpers import SNR_TOL, check_segment_against_oracle, check_candidates_against_oracle, check_candidates_dense, check_dmt_against_oracle, check_plan_against_oracle, check_stats_against_oracle, make_plan
 
 pytestmark = pytest.mark.gpu
 
@@ -200,6 +200,27 @@ def test_cfg6_band5_full(cuda, api, orc, synth):
     assert found == len(strong), (found, len(strong))
 
 
+def test_cfg6_band5_full_every_output(cuda, api, orc, synth):
+    """Band 5 complete: the only full-size workload whose ranges run the 224-word, 12-entry kernel instances the
+    cost model picks by default -- asserted below -- so every output, every trial's statistics and the whole candidate list
+    (about 2e6 records, compared through dense rows) go against the oracle, not a sample."""
+    w = synth.workload(6)
+    fb = synth.generate(w)
+    plan = make_plan(api, w, cand_capacity=1 << 26)
+    choice = [plan.tiling_choice(r) for r in range(len(w.ranges))]
+    assert any(c["tile_words"] == 224 or c["max_entries"] == 12 for c in choice), choice
+    check_plan_against_oracle(orc, plan, w, stride=499)
+    d_dmt = plan.search(cuda.from_numpy(fb[None]).cuda(), w.threshold)
+    total, ovf = plan.candidates_count()
+    assert not ovf, total
+    cands = plan.candidates_read()
+    assert cands.size == total
+    s_all, q_all = plan.trial_stats_all(1)
+    st = full_beam_parity(orc, plan, w, fb, d_dmt[0], cands, s_all[0], q_all[0], dense=True)
+    assert st["gpu"] == total and st["oracle"] > 1000
+    assert st["near_threshold_only_oracle"] + st["near_threshold_only_gpu"] <= max(25, 1e-4 * st["oracle"]), st
+
+
 def full_beam_parity(orc, plan, w, fb, d_dmt_beam, cands_beam, s_row, q_row, dense=False):
     """One beam complete: every output, every trial's exact statistics, the whole candidate list (rules D2)."""
     ref = orc.run_path(fb, w.fch1, w.foff, w.tsamp, w.ranges, w.widths, w.threshold, do_search=True)
@@ -254,13 +275,12 @@ def test_cfg3_shape_uniform_bytes_full_every_output(cuda, api, orc, synth):
     assert st["gpu"] == total
 
 
-CFG4_BEAMS_CHECKED = (0, 1, 7, 8, 15, 27, 28, 29, 31, 32, 40, 47, 48, 56, 62, 63)   # incl. both sides of the 2^31-byte
-                                                                                   # (7|8) and 2^31-element (28|29) offsets
+CFG4_BEAMS_CHECKED = tuple(range(64))      # all of them (both sides of the 2^31-byte (7|8) and 2^31-element (28|29) offsets)
 
 
 def test_cfg4_multibeam_batch_full(cuda, api, orc, synth):
-    """Config 4: 64 beams in one launch (64-bit offsets: 18 GiB of DM transform).  16 beams complete against the oracle
-    (every output, statistic, candidate); on ALL 64 beams the sum of every row against the prefix-sum identity
+    """Config 4: 64 beams in one launch (64-bit offsets: 18 GiB of DM transform).  All 64 beams complete against the oracle
+    (every output, statistic, candidate: about 5 s of the oracle per beam); also, on all beams, the sum of every row against the prefix-sum identity
     sum_t out[d][t] = sum_c (P_c[delay + nout] - P_c[delay]) evaluated from the raw input with the oracle's delay table, and
     the kernel's sum of squares against the DM transform it was computed from."""
     w = synth.workload(4)
@@ -286,7 +306,7 @@ def test_cfg4_multibeam_batch_full(cuda, api, orc, synth):
         st = full_beam_parity(orc, plan, w, h_fb[b], d_dmt[b], cands[starts[b]: starts[b + 1]], s_all[b], q_all[b])
         assert st["gpu"] == starts[b + 1] - starts[b]
         ncheck += 1
-    assert ncheck == 16
+    assert ncheck == nb == 64
     # all 64 beams: row sums from channel prefix sums of the input (independent of any dedispersion code)
     delays = [orc.delay_table(w.fch1, w.foff, w.nchan, w.tsamp, lo, step, ndm, k) for (lo, step, ndm, k) in w.ranges]
     offs = cuda.from_numpy(off).cuda()
@@ -310,3 +330,68 @@ def test_cfg4_multibeam_batch_full(cuda, api, orc, synth):
         lo_ = cuda.where(offs > 0, cs[(offs - 1).clamp(min=0)], cuda.zeros_like(hi))
         qq = cuda.where(live, hi - lo_, cuda.zeros_like(hi)).cpu().numpy().astype(np.uint64)
         assert np.array_equal(q_all[b], qq), ("row sums of squares", b)
+
+
+def test_stream_push_bench_geometry(cuda, api, orc, synth):
+    """The configuration `bench.py --stream` times: config 3's plan on a 149,504-sample buffer, 102,400 new
+    samples per push, time-spliced blocks cut from one long synthetic beam, tail-only pushes.  From the second push on the
+    buffer holds Gaussian bytes only, the decimated series fit their 8-bit copies, and the decimated ranges run the dual
+    kernel's 8-bit body with tail > 0 over 293 time tiles -- asserted, not assumed.  After the second push EVERY row's window
+    goes against the oracle's dedispersion of the oracle's buffer, nothing outside the windows may be written, and the
+    segment search (statistics, candidates) is checked on every third trial from the oracle's rows; after the third push a
+    sixteenth of the trials (an oracle plan of every 16th DM) is compared the same way."""
+    w = synth.workload(3)
+    nnew = 102400
+    probe = api.Plan(w.fch1, w.foff, w.nchan, w.tsamp, 1 << 17, w.ranges, w.widths)
+    _, hsearch, _ = probe.segment_info()
+    probe.close()
+    nsamp = nnew + (hsearch + 511) // 512 * 512
+    assert nsamp == 149504
+    plan = api.Plan(w.fch1, w.foff, w.nchan, w.tsamp, nsamp, w.ranges, w.widths, max_beams=1, cand_capacity=1 << 26)
+    npush = 3
+    fb = synth.generate(synth.workload(3, nsamp=nnew * npush))
+    blocks = [np.ascontiguousarray(fb[:, i * nnew:(i + 1) * nnew].T) for i in range(npush)]          # [t][chan]
+    bufs = orc.overlap_save_buffers(blocks, nsamp, flip=False)
+    _, _, dec, nout, off = plan.trial_table()
+    SENT = -123456789
+    d_dmt = cuda.empty((1, plan.dmt_elems_per_beam), dtype=cuda.int32, device="cuda")
+    for i in range(npush):
+        d_dmt.fill_(SENT)
+        plan.segment_push(cuda.from_numpy(blocks[i][:, None, :]).cuda(), False, d_dmt, spliced=True, whole_rows=False)
+        plan.segment_search(d_dmt, nnew, w.threshold)
+        if i == 0:
+            continue                                     # start-up zeros in the buffer: the uint16 body (covered at small sizes)
+        for ri in (1, 2):
+            in_use, floor, span = plan.decimated_compact(ri)
+            assert in_use and floor > 0 and span < 256, (i, ri, in_use, floor, span)
+        total, ovf = plan.candidates_count()
+        assert not ovf
+        cands = plan.candidates_read()
+        s_all, q_all = plan.trial_stats_all(1)
+        dmt = d_dmt.cpu().numpy()[0]
+        if i == 1:
+            ranges, pick = w.ranges, (lambda ndm: range(ndm))
+        else:                                            # every 16th DM of each range: the same doubles (16 * step is exact)
+            ranges = [(lo, step * 16, (ndm + 15) // 16, k) for (lo, step, ndm, k) in w.ranges]
+            pick = (lambda ndm: range(0, ndm, 16))
+        ref = orc.run_path(bufs[i], w.fch1, w.foff, w.tsamp, ranges, w.widths, w.threshold, do_search=False)
+        orows, trials, d0 = {}, [], 0
+        for (lo, step, ndm, k), rr in zip(w.ranges, ref):
+            for j, dl in enumerate(pick(ndm)):
+                orows[d0 + dl] = rr.dmt[rr.rowoff[j]: rr.rowoff[j + 1]]
+                trials.append(d0 + dl)
+            d0 += ndm
+        assert d0 == plan.ntrials == 4501
+        searched = trials[::3] if i == 1 else trials
+        # the search part (Python per trial) on a subset; the windows and the sentinel on every trial of `trials`
+        n = check_segment_against_oracle(orc, plan, dmt, orows, searched, w.widths, w.threshold, nnew, cands, s_all[0], q_all[0],
+                                         sentinel=SENT)
+        assert n > 100
+        for d in trials:
+            if d in searched:
+                continue
+            nn, k = int(nout[d]), int(dec[d])
+            win = min(nn, nnew // k + max(w.widths) - 1)
+            mine = dmt[off[d]: off[d] + nn]
+            assert np.array_equal(mine[nn - win:], orows[d][nn - win:]), (i, d)
+            assert np.all(mine[: nn - win] == SENT), (i, d)

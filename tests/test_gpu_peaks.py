@@ -100,3 +100,24 @@ def test_empty_and_error_paths(cuda, api, synth):
     with pytest.raises(api.SptError) as e:
         plan.peak_filter((4,))
     assert e.value.code == api.SPT_ERR_INVALID
+
+
+def test_dense_plane_at_volume(cuda, api, orc, synth):
+    """The dense-plane lookups at the density they exist for (PAPER.md:96 on unmitigated RFI): config 5's beam -- zero-DM
+    spikes and persistent narrowband RFI put a sizeable fraction of all cells above threshold -- searched over 48 trials of
+    two DM ranges across the whole 2^18-sample row, millions of records.  The plane over all beams (lookup 2), the
+    one-beam plane (3) and the hash table (1) must each keep exactly what the oracle's filter keeps of the same list."""
+    w5 = synth.workload(5)
+    fb = synth.generate(w5)
+    w = Shape(w5.fch1, w5.foff, w5.nchan, w5.nsamp, [(0.0, 0.2, 32, 1), (500.0, 0.5, 16, 2)], w5.widths, w5.threshold)
+    plan = make_plan(api, w, cand_capacity=1 << 24)
+    d_dmt = plan.search(cuda.from_numpy(fb[None]).cuda(), w.threshold)
+    total, ovf = plan.candidates_count()
+    assert not ovf and total > 1_000_000, total
+    cands = plan.candidates_read()
+    del d_dmt
+    expect = as_set(oracle_filter_of_list(orc, plan, cands, (3, 11)))
+    assert 0 < len(expect) < cands.size // 10
+    for lookup in (2, 3, 1):
+        plan.set_option("peaks_lookup", lookup)
+        assert as_set(plan.peak_filter((3, 11))) == expect, lookup
