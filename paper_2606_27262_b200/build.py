@@ -18,7 +18,7 @@ SOURCES = ["api.cu", "plan.cpp", "dedisperse.cu", "sps.cu", "peaks.cu", "peaks_s
 HEADERS = ["internal.h", "kernels.h", os.path.join("..", "..", "include", "spt.h")]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "--fmad=false",
-         "-Xcompiler", "-fPIC,-ffp-contract=off,-O2", "-Xptxas", "-v", "-shared", "-cudart", "static"]
+         "-Xcompiler", "-fPIC,-ffp-contract=off,-O2,-pthread", "-Xptxas", "-v", "-shared", "-cudart", "static"]
 
 
 def _stale() -> bool:

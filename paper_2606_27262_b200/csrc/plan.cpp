@@ -7,7 +7,11 @@
 #include <cmath>
 #include <cstring>
 #include <cstdlib>
+#include <functional>
 #include <map>
+#include <new>
+#include <system_error>
+#include <thread>
 #include <utility>
 
 #include "internal.h"
@@ -457,9 +461,10 @@ static int build_range_auto(const Plan& p, RangePlan& rp, bool compact);
 int build_tiling(Plan& p) {
     p.compact.clear();
     p.compact.resize(p.ranges.size());
-    for (size_t i = 0; i < p.ranges.size(); ++i) {
-        int rc;
-        if ((rc = build_range_auto(p, p.ranges[i], false)) != SPT_OK) return rc;
+    // the ranges are independent of each other: one thread each (every thread touches only its own RangePlan entries)
+    auto build_one = [&p](size_t i) -> int {
+        const int rc = build_range_auto(p, p.ranges[i], false);
+        if (rc != SPT_OK) return rc;
         if (p.ranges[i].decim > 1 && p.opt_compact) {
             // second set of tables for the 8-bit copy of the decimated series (the delay table is shared by value: a few MB)
             // Both sets run in one kernel instance, so they share tile width and entry cap: the copy's choice (it is the set
@@ -483,7 +488,30 @@ int build_tiling(Plan& p) {
                 p.compact[i] = RangePlan();
             }
         }
+        return SPT_OK;
+    };
+    std::vector<int> rcs(p.ranges.size(), SPT_OK);
+    auto guarded = [&](size_t i) {
+        try {
+            rcs[i] = build_one(i);
+        } catch (const std::bad_alloc&) {
+            rcs[i] = SPT_ERR_NOMEM;
+        }
+    };
+    {
+        std::vector<std::thread> workers;
+        for (size_t i = 1; i < p.ranges.size(); ++i) {
+            try {
+                workers.emplace_back(guarded, i);
+            } catch (const std::system_error&) {
+                guarded(i);
+            }
+        }
+        if (!p.ranges.empty()) guarded(0);
+        for (auto& t : workers) t.join();
     }
+    for (int rc : rcs)
+        if (rc != SPT_OK) return rc;
     p.tiling_built = true;
     return SPT_OK;
 }
@@ -495,9 +523,9 @@ int build_tiling(Plan& p) {
 static int build_range_auto(const Plan& p, RangePlan& rp, const bool compact) {
     const int khs[2] = {256, 224};
     const int caps[2] = {8, 12};
-    bool have = false;
-    double best = 0.0;
-    RangePlan keep;
+    // the candidates the options leave, in the order the choice prefers on equal cost ...
+    struct Cand { int kh, use_cap, G; bool last; RangePlan plan; int rc; };
+    std::vector<Cand> cands;
     for (int kh : khs) {
         if (p.opt_kh != 0 && kh != p.opt_kh) continue;
         if (p.opt_kh == 0 && kh != 256 && p.opt_dm_tile != 64) continue;     // the narrow tile exists for 64-trial tiles only
@@ -505,19 +533,45 @@ static int build_range_auto(const Plan& p, RangePlan& rp, const bool compact) {
             if (p.opt_max_ent != 0 && cap != p.opt_max_ent && !(p.opt_max_ent == 16 && cap == 12)) continue;
             const int use_cap = (p.opt_max_ent == 16) ? 16 : cap;
             if (p.opt_max_ent == 0 && p.opt_group != 0 && p.opt_group <= 8 && cap > 8) continue;
-            RangePlan cand = rp;
-            cand.kh = kh;
             const int G = p.opt_group ? p.opt_group : (use_cap > 8 ? 16 : 8);
-            const int rc = build_range(p, cand, G, use_cap, compact);
-            if (rc != SPT_OK) {
-                if (!have && kh == khs[1] && cap == caps[1]) return rc;
-                continue;
-            }
-            // a margin for the decimated uint16 series, whose pre-sum the constants fit less well: stay with the default there
-            double c = modelled_cost(cand);
-            if (!(kh == 256 && use_cap == 8)) c *= (rp.decim == 1 || compact) ? 1.03 : 1.10;
-            if (!have || c < best) { best = c; keep = std::move(cand); have = true; }
+            cands.push_back(Cand{kh, use_cap, G, kh == khs[1] && cap == caps[1], RangePlan(), SPT_OK});
         }
+    }
+    // ... each built on its own thread (a plan is built per band; the tables of one candidate of the config-3
+    // plan take about a second, and build_range only reads the plan and writes its own RangePlan)
+    auto build_one = [&](Cand& c) {
+        try {
+            c.plan = rp;
+            c.plan.kh = c.kh;
+            c.rc = build_range(p, c.plan, c.G, c.use_cap, compact);
+        } catch (const std::bad_alloc&) {
+            c.rc = SPT_ERR_NOMEM;
+        }
+    };
+    {
+        std::vector<std::thread> workers;
+        for (size_t i = 1; i < cands.size(); ++i) {
+            try {
+                workers.emplace_back(build_one, std::ref(cands[i]));
+            } catch (const std::system_error&) {
+                build_one(cands[i]);                                          // no more threads: build it here
+            }
+        }
+        if (!cands.empty()) build_one(cands[0]);
+        for (auto& t : workers) t.join();
+    }
+    bool have = false;
+    double best = 0.0;
+    RangePlan keep;
+    for (Cand& c : cands) {
+        if (c.rc != SPT_OK) {
+            if (!have && c.last) return c.rc;
+            continue;
+        }
+        // a margin for the decimated uint16 series, whose pre-sum the constants fit less well: stay with the default there
+        double cost = modelled_cost(c.plan);
+        if (!(c.kh == 256 && c.use_cap == 8)) cost *= (rp.decim == 1 || compact) ? 1.03 : 1.10;
+        if (!have || cost < best) { best = cost; keep = std::move(c.plan); have = true; }
     }
     if (!have) return SPT_ERR_UNSUPPORTED;
     rp = std::move(keep);
