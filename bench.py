@@ -34,7 +34,38 @@ UNIT = "DM-trial*chan*samples/s"
 # `ncu --set full` capture of the dominant kernel, as `ncu -i ... --page raw --csv --print-units base` wrote it
 # (profiles/r02_final_raw.md names the commands); roofline.traffic and the shared-memory / issue-slot fractions are read
 # from this file, per launch.
-NCU_RAW_CSV = os.path.join(ROOT, "profiles", "r02_final_raw.csv")
+NCU_RAW_CSV = os.path.join(ROOT, "profiles", "r03_final_raw.csv")
+NCU_STAMP = os.path.join(ROOT, "profiles", "r03_final_raw.stamp.json")   # written by `python bench.py --stamp-ncu` beside the CSV
+
+
+def sources_sha16():
+    """Hash of everything libspt.so is built from: says whether the ncu capture still describes the kernels that run."""
+    import hashlib
+    from paper_2606_27262_b200 import build
+    h = hashlib.sha256()
+    for f in sorted(build.SOURCES + build.HEADERS):
+        with open(os.path.join(build.CSRC, f), "rb") as fh:
+            h.update(f.encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
+def stamp_ncu():
+    """Run here (where .git is) after copying a new capture to profiles/: records the commit and the source hash it was made at."""
+    import subprocess
+    commit = subprocess.run(["git", "rev-parse", "HEAD"], cwd=ROOT, capture_output=True, text=True).stdout.strip()
+    dirty = bool(subprocess.run(["git", "status", "--porcelain", "--", "paper_2606_27262_b200/csrc", "include"], cwd=ROOT,
+                                capture_output=True, text=True).stdout.strip())
+    out = {"csv": os.path.relpath(NCU_RAW_CSV, ROOT), "commit": commit, "sources_dirty_at_stamp": dirty, "sources_sha16": sources_sha16()}
+    json.dump(out, open(NCU_STAMP, "w"), indent=1)
+    print(json.dumps(out))
+
+
+def ncu_source():
+    """Where roofline.traffic / frac_lds / issue_frac come from, and whether the kernels have changed since (stale)."""
+    st = json.load(open(NCU_STAMP)) if os.path.exists(NCU_STAMP) else {}
+    return {"csv": os.path.relpath(NCU_RAW_CSV, ROOT), "captured_at_commit": st.get("commit"),
+            "captured_sources_sha16": st.get("sources_sha16"), "sources_sha16_now": sources_sha16(),
+            "stale": st.get("sources_sha16") != sources_sha16()}
 CAND_CAPACITY = {1: 1 << 20, 2: 1 << 24, 3: 1 << 26, 4: 1 << 27, 5: 1 << 29, 6: 1 << 26}
 
 
@@ -331,14 +362,18 @@ class Measurement:
         sampler = ClockSampler(local_rank)
         sampler.start()
         self.barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]      # one event between steps: median and min
+        e0, e1 = ev[0], ev[-1]
         e0.record(self.stream)
-        for _ in range(steps):
+        for i in range(steps):
             ncand, ovf = self.step()
-        e1.record(self.stream)
+            ev[i + 1].record(self.stream)
         self.barrier()
         clocks = sampler.stop()
         ms_total = self.shard.max_over_ranks(e0.elapsed_time(e1), device="cuda")
+        per = sorted(ev[i].elapsed_time(ev[i + 1]) for i in range(steps))
+        self.step_ms = {"median": per[len(per) // 2] if len(per) % 2 else 0.5 * (per[len(per) // 2 - 1] + per[len(per) // 2]),
+                        "min": per[0], "max": per[-1], "note": "this rank's steps, each between its own pair of CUDA events"}
         nl = self.plan.launches() - launches0
         if getattr(self, "graph", None) is not None:
             nl = steps * self.graph_launches
@@ -534,7 +569,8 @@ def run_ours(args, rank, world, local_rank):
             inst = c.get("smsp__inst_executed.sum")
             rd, wr = c.get("dram__bytes_read.sum"), c.get("dram__bytes_write.sum")
             roof["traffic"] = (rd + wr) if (rd is not None and wr is not None) else None
-            roof["traffic_source"] = "profiles/r02_final_raw.csv: dram__bytes_read.sum + dram__bytes_write.sum of this kernel, one launch"
+            roof["traffic_source"] = "dram__bytes_read.sum + dram__bytes_write.sum of this kernel, one launch, from the committed ncu capture"
+            roof["ncu_source"] = ncu_source()       # "stale": true = the sources changed after the capture: counters of an older kernel
             if wf:
                 roof["lds_wavefronts_per_launch"] = wf
                 roof["frac_lds"] = wf / (dom_ms * 1e-3) / lds_peak
@@ -578,7 +614,8 @@ def run_ours(args, rank, world, local_rank):
     # vs_baseline stays null: BASELINE.md holds no published number for this metric on this workload (the paper's figures
     # are whole-pipeline beams per A100); the oracle's rate on the host cores is reported in cpu_baseline, not as a baseline ratio
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warm,
-            "ms_per_step": ms_total / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_total / steps, "ms_per_step_stats": getattr(m, "step_ms", None),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "int32", "data": "synthetic", "config": workload_config(w, world),
             "launch": {"per_range": [plan.tiling_choice(r) for r in range(len(w.ranges))],     # what the plan actually chose
                        "dm_tile": args.dm_tile or 64,
@@ -779,13 +816,16 @@ def main():
     ap.add_argument("--all-configs", action="store_true")
     ap.add_argument("--stream", action="store_true")
     ap.add_argument("--cutouts", action="store_true")
+    ap.add_argument("--stamp-ncu", action="store_true", help="record the commit and source hash of profiles/r03_final_raw.csv (no GPU)")
     ap.add_argument("--graph", action="store_true", help="replay a CUDA graph of spt_search instead of calling it every step")
     ap.add_argument("--two-calls", action="store_true", help="step = spt_dedisperse + spt_single_pulse_search instead of spt_search")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.stamp_ncu:
+        stamp_ncu()
+    elif args.impl == "reference":
         run_reference(args, rank, world)
     elif args.all_configs:
         run_all_configs(args, local_rank)

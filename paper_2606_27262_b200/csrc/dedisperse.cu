@@ -16,49 +16,67 @@ namespace spt {
 
 // ---------------------------------------------------------------------------------------------------------------
 // a2. Time decimation by k = 2^m.  One thread makes four consecutive outputs from 4k input bytes (k 32-bit words),
-// each word reduced with DP4A against a byte mask.  HBM bound: reads nchan*nsamp bytes, writes 2*nchan*nsamp/k.
+// each word reduced with DP4A against a byte mask.  HBM bound: reads nchan*nsamp bytes, writes 2*nchan*nsamp/k.  The bounds
+// of the series (maxval[0] = largest, maxval[1] = smallest sample; the caller resets them) come out of the same pass.
 // ---------------------------------------------------------------------------------------------------------------
 __global__ void decimate_kernel(const uint8_t* __restrict__ x, int64_t in_row_stride, int64_t in_beam_stride,
                                 uint16_t* __restrict__ y, int64_t out_row_stride, int64_t out_beam_stride,
-                                int32_t nchan, int64_t nsamp_k, int32_t k) {
+                                int32_t nchan, int64_t nsamp_k, int32_t k, uint32_t* __restrict__ maxval) {
     const int64_t quads = (nsamp_k + 3) >> 2;  // groups of 4 outputs per row
     const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (q >= quads) return;
-    const int32_t c = blockIdx.y, b = blockIdx.z;
-    const uint8_t* src = x + (int64_t)b * in_beam_stride + (int64_t)c * in_row_stride;
-    uint16_t* dst = y + (int64_t)b * out_beam_stride + (int64_t)c * out_row_stride;
-    const int64_t j0 = q << 2;
-    uint32_t o[4] = {0u, 0u, 0u, 0u};
-    if (j0 + 4 <= nsamp_k) {
-        const uint32_t* w = reinterpret_cast<const uint32_t*>(src + j0 * k);  // 4-byte aligned: strides are multiples of 16
-        if (k == 2) {
-            const uint32_t w0 = __ldg(w), w1 = __ldg(w + 1);
-            o[0] = __dp4a(w0, 0x00000101u, 0u); o[1] = __dp4a(w0, 0x01010000u, 0u);
-            o[2] = __dp4a(w1, 0x00000101u, 0u); o[3] = __dp4a(w1, 0x01010000u, 0u);
-        } else {
-            const int wpo = k >> 2;  // words per output
+    uint32_t vmax = 0u, vmin = 0xffffffffu;    // bounds of the outputs this thread makes (threads past the row: neutral)
+    if (q < quads) {
+        const int32_t c = blockIdx.y, b = blockIdx.z;
+        const uint8_t* src = x + (int64_t)b * in_beam_stride + (int64_t)c * in_row_stride;
+        uint16_t* dst = y + (int64_t)b * out_beam_stride + (int64_t)c * out_row_stride;
+        const int64_t j0 = q << 2;
+        uint32_t o[4] = {0u, 0u, 0u, 0u};
+        if (j0 + 4 <= nsamp_k) {
+            const uint32_t* w = reinterpret_cast<const uint32_t*>(src + j0 * k);  // 4-byte aligned: strides are multiples of 16
+            if (k == 2) {
+                const uint32_t w0 = __ldg(w), w1 = __ldg(w + 1);
+                o[0] = __dp4a(w0, 0x00000101u, 0u); o[1] = __dp4a(w0, 0x01010000u, 0u);
+                o[2] = __dp4a(w1, 0x00000101u, 0u); o[3] = __dp4a(w1, 0x01010000u, 0u);
+            } else {
+                const int wpo = k >> 2;  // words per output
 #pragma unroll
-            for (int i = 0; i < 4; ++i)
-                for (int m = 0; m < wpo; ++m) o[i] = __dp4a(__ldg(w + i * wpo + m), 0x01010101u, o[i]);
+                for (int i = 0; i < 4; ++i)
+                    for (int m = 0; m < wpo; ++m) o[i] = __dp4a(__ldg(w + i * wpo + m), 0x01010101u, o[i]);
+            }
+            uint2 pk;
+            pk.x = o[0] | (o[1] << 16);
+            pk.y = o[2] | (o[3] << 16);
+            *reinterpret_cast<uint2*>(dst + j0) = pk;
+            vmax = max(max(o[0], o[1]), max(o[2], o[3]));
+            vmin = min(min(o[0], o[1]), min(o[2], o[3]));
+        } else {  // ragged tail of the row
+            for (int64_t j = j0; j < nsamp_k; ++j) {
+                uint32_t s = 0;
+                for (int m = 0; m < k; ++m) s += src[j * k + m];
+                dst[j] = (uint16_t)s;
+                vmax = max(vmax, s);
+                vmin = min(vmin, s);
+            }
         }
-        uint2 pk;
-        pk.x = o[0] | (o[1] << 16);
-        pk.y = o[2] | (o[3] << 16);
-        *reinterpret_cast<uint2*>(dst + j0) = pk;
-    } else {  // ragged tail of the row
-        for (int64_t j = j0; j < nsamp_k; ++j) {
-            uint32_t s = 0;
-            for (int m = 0; m < k; ++m) s += src[j * k + m];
-            dst[j] = (uint16_t)s;
+        // The row padding (rows are 16-element multiples) repeats the row's last sample.  No stored output reads it, but the
+        // pass that makes the 8-bit copy runs over whole rows, and the lanes of discarded outputs next to a valid one must
+        // stay inside the bounds the kernel was given.
+        if (q == quads - 1) {
+            const int64_t pad_end = min((nsamp_k + 15) & ~(int64_t)15, out_row_stride);
+            const uint16_t last = dst[nsamp_k - 1];                    // written by this thread just above
+            for (int64_t j = nsamp_k; j < pad_end; ++j) dst[j] = last;
         }
     }
-    // The row padding (rows are 16-element multiples) repeats the row's last sample.  No stored output reads it, but the
-    // passes over whole rows do -- the bounds of the series and its 8-bit copy -- and padding zeros would make every series
-    // whose length is not a multiple of 16 look as if it spanned [0, max]: no 8-bit copy, no floor for the packed lanes.
-    if (q == quads - 1) {
-        const int64_t pad_end = min((nsamp_k + 15) & ~(int64_t)15, out_row_stride);
-        const uint16_t last = dst[nsamp_k - 1];                    // written by this thread just above
-        for (int64_t j = nsamp_k; j < pad_end; ++j) dst[j] = last;
+    // Bounds of the series (largest and smallest sample, over the real samples only) as a by-product: they bound the 16-bit lanes
+    // of the dedispersion and decide whether the series gets an 8-bit copy.  One warp reduction; the atomics are issued
+    // only by warps that improve on what is already known, which after the first few blocks is next to none.
+    if (maxval != nullptr) {
+        vmax = __reduce_max_sync(0xffffffffu, vmax);
+        vmin = __reduce_min_sync(0xffffffffu, vmin);
+        if ((threadIdx.x & 31) == 0) {
+            if (vmax > *reinterpret_cast<volatile uint32_t*>(maxval)) atomicMax(maxval, vmax);
+            if (vmin < *reinterpret_cast<volatile uint32_t*>(maxval + 1)) atomicMin(maxval + 1, vmin);
+        }
     }
 }
 
@@ -169,12 +187,12 @@ void launch_compact_u16(const uint16_t* y, uint8_t* c, int64_t nelem, const uint
 
 void launch_decimate(const uint8_t* x, int64_t in_row_stride, int64_t in_beam_stride, uint16_t* y,
                      int64_t out_row_stride, int64_t out_beam_stride, int32_t nchan, int32_t nbeam, int64_t nsamp_k,
-                     int32_t k, cudaStream_t st) {
+                     int32_t k, uint32_t* maxval, cudaStream_t st) {
     const int64_t quads = (nsamp_k + 3) >> 2;
     if (quads <= 0) return;
     dim3 grid((unsigned)((quads + 255) / 256), (unsigned)nchan, (unsigned)nbeam);
     decimate_kernel<<<grid, 256, 0, st>>>(x, in_row_stride, in_beam_stride, y, out_row_stride, out_beam_stride, nchan,
-                                          nsamp_k, k);
+                                          nsamp_k, k, maxval);
 }
 
 // ---------------------------------------------------------------------------------------------------------------

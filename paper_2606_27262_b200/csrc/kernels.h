@@ -11,7 +11,7 @@ int sm_count();   // SMs of the current device (dedisperse.cu)
 
 void launch_decimate(const uint8_t* x, int64_t in_row_stride, int64_t in_beam_stride, uint16_t* y,
                      int64_t out_row_stride, int64_t out_beam_stride, int32_t nchan, int32_t nbeam, int64_t nsamp_k,
-                     int32_t k, cudaStream_t st);
+                     int32_t k, uint32_t* maxval /* {largest, smallest} sample of the series, updated; may be NULL */, cudaStream_t st);
 void launch_fill_row_pad_u8(uint8_t* x, int64_t pitch, int64_t nsamp, int64_t nrows, cudaStream_t st);
 void launch_max_u16(const uint16_t* x, int64_t nelem, uint32_t* maxval, cudaStream_t st);
 void launch_max_u8(const uint8_t* x, int64_t nbytes, uint32_t* maxval, cudaStream_t st);
